@@ -1,0 +1,150 @@
+/* fdtd.h -- C ABI of the B200-native explicit Yee FDTD hot path (arXiv 2208.04371, ARTEMIS S-parameter workflow).
+ *
+ * What the library computes (citations: PAPER.md = /root/reference/PAPER.md; R* = readings in DESIGN.md):
+ *   one leapfrog time step  H^{n-1/2} -> H^{n+1/2},  E^n -> E^{n+1}  of the "conventional FDTD" on a Yee grid
+ *    with per-cell permittivity / conductivity / permeability coefficients,
+ *   PEC walls and PEC/lossy metal, an absorbing layer on chosen faces (realised as
+ *   CPML, R4), the soft port source of Eq. 3, the port voltage and current integrals of Eq. 4
+ *    and the DFT of their histories accumulated on the device every step.
+ *   S* (Eq. 1-2) is formed by the caller from fdtd_read_port_dft() of an "inc" and a "tot" run.
+ *
+ * Conventions
+ *   Grid      nx*ny*nz Yee cells, x fastest.  Cell (i,j,k) owns the samples
+ *               Ex(i+1/2,j,k) Ey(i,j+1/2,k) Ez(i,j,k+1/2) Hx(i,j+1/2,k+1/2) Hy(i+1/2,j,k+1/2) Hz(i+1/2,j+1/2,k)   (R1)
+ *             Caller-visible arrays hold exactly N = nx*ny*nz elements, index i + nx*(j + ny*k).  Propagation axis of
+ *             the ports is x, "vertical" is z (the paper uses y and z; a relabelling).
+ *   Walls     all six outer faces are PEC, behind any CPML.  Low-face tangential E is stored and forced to 0;
+ *             high-face tangential E is not stored and reads as 0 (R1).
+ *   Time      after n steps the E arrays hold E at t = n*dt, the H arrays hold H at t = (n-1/2)*dt (R5).
+ *   Pointers  every pointer argument documented "host or device" may be either; the library asks the CUDA runtime
+ *             which.  All other pointers are host pointers.  Nothing is retained after a call returns except the
+ *             workspace given to fdtd_commit().
+ *   Memory    the CALLER owns all device memory: one buffer of fdtd_workspace_bytes() bytes (256-byte aligned), and
+ *             a CUDA stream.  The library never allocates device memory.
+ *   Errors    every int-returning call returns FDTD_OK (0) or a negative code; fdtd_last_error() gives a message.
+ *             No exceptions, no abort, no printing.  There is NO CPU fallback: without a CUDA device
+ *             fdtd_commit() fails with FDTD_ECUDA.
+ *   Lifecycle fdtd_create -> {fdtd_set_boundary, fdtd_set_material_mode, fdtd_add_port, fdtd_set_dft,
+ *             fdtd_set_option} in any order -> fdtd_workspace_bytes -> fdtd_commit -> {fdtd_set_materials_*,
+ *             fdtd_step, fdtd_read_*, fdtd_write_fields, fdtd_reset} -> fdtd_destroy.
+ *             Calling out of order returns FDTD_ESTATE.  A freshly committed object is vacuum, all state zero.
+ *   Threads   one handle must not be used from two host threads at once.
+ */
+#ifndef FDTD_B200_H
+#define FDTD_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fdtd fdtd_t; /* opaque host object owned by the library */
+
+enum { FDTD_OK = 0, FDTD_EINVAL = -1, FDTD_ECFL = -2, FDTD_ESTATE = -3, FDTD_ENOMEM = -4, FDTD_ECUDA = -5, FDTD_ERANGE = -6 };
+enum { FDTD_F32 = 32, FDTD_F64 = 64 };
+enum { FDTD_W_DGAUSS = 0 /* Eq. 3 */, FDTD_W_GAUSS = 1, FDTD_W_GSINE = 2 };
+enum { FDTD_MAT_INDEXED = 0, FDTD_MAT_FULL = 1 };
+enum { FDTD_EX = 0, FDTD_EY, FDTD_EZ, FDTD_HX, FDTD_HY, FDTD_HZ };
+
+/* Options for fdtd_set_option (before commit). */
+enum {
+  FDTD_OPT_STEP_IMPL = 1,   /* 0 = auto, 1 = two-pass (H kernel, E kernel), 2 = fused E+H temporal blocking            */
+  FDTD_OPT_USE_GRAPH = 2,   /* 1 (default) = replay a captured CUDA graph per step; 0 = plain launches                  */
+  FDTD_OPT_GRAPH_UNROLL = 3 /* steps per captured graph (default 8)                                                     */
+};
+
+/* A port (Fig. 1a): a soft E_z source on a box of the plane i = is (surface 'e'), a voltage box and
+ * a current loop on the plane i = ip.
+ *   source   E_z[is, j, k] += amp * g((n+1)*dt)   for j in sj0..sj1 (inclusive), k in [sk0, sk1)          (R6, R8)
+ *            g: DGAUSS -2u exp(-u^2) (Eq. 3) | GAUSS exp(-u^2) | GSINE sin(2 pi f0 (t-t0)) exp(-u^2), u = (t-t0)/sigma
+ *   V        (dz / (vj1-vj0+1)) * sum_{j=vj0..vj1} sum_{k=vk0..vk1-1} E_z[ip, j, k]                        (Eq. 4, R7)
+ *   I        dz * sum_{k=lk0..lk1} (Hz[ip,lj1,k] - Hz[ip,lj0-1,k]) - dy * sum_{j=lj0..lj1} (Hy[ip,j,lk1] - Hy[ip,j,lk0-1])
+ *            -- the discrete Ampere loop, right-handed about +x, one cell away from metal occupying node columns
+ *            lj0+1..lj1-1 and planes lk0+1..lk1-1.  Needs lj0 >= 1 and lk0 >= 1.           (R7)
+ */
+typedef struct fdtd_port {
+  int has_source;
+  int is, sj0, sj1, sk0, sk1;
+  int waveform;
+  double amp, t0, sigma, f0;
+  int ip;
+  int vj0, vj1, vk0, vk1;
+  int lj0, lj1, lk0, lk1;
+} fdtd_port;
+
+/* Create a solver for an nx*ny*nz grid with cell size (dx,dy,dz) [m] and time step dt [s]; precision = FDTD_F32|F64
+ * is the arithmetic and storage type of the fields.  FDTD_ECFL if dt > 1/(c*sqrt(1/dx^2+1/dy^2+1/dz^2)) (PAPER.md:93,
+ * 116 run at 0.9 of it); FDTD_EINVAL if any n < 2, any d <= 0, dt <= 0 or a bad precision.  *out is set on success. */
+int fdtd_create(int nx, int ny, int nz, double dx, double dy, double dz, double dt, int precision, fdtd_t** out);
+
+/* CPML thickness in cells on the faces x-,x+,y-,y+,z-,z+ (0 = bare PEC wall; PML on every face but the
+ * ground).  cpml = NULL for defaults or {m, m_a, kappa_max, alpha_max, sigma_factor, eps_r_pml} (R4):
+ * sigma_max = sigma_factor*(m+1)/(eta0*d_axis*sqrt(eps_r_pml)).  FDTD_ERANGE if lo+hi > n on an axis. */
+int fdtd_set_boundary(fdtd_t*, const int pml_cells[6], const double* cpml);
+
+/* Declare how materials will be given after commit (decides the workspace size).  Default: INDEXED, has_mu = 0.
+ *   FDTD_MAT_INDEXED  one uint8 per cell into a table of <= 256 entries (a handful of materials)
+ *   FDTD_MAT_FULL     per-cell, per-component arrays (anisotropic eps_xx/yy/zz, sigma_xx/yy/zz)
+ * has_mu != 0 reserves room for per-entry / per-cell permeability. */
+int fdtd_set_material_mode(fdtd_t*, int mode, int has_mu);
+
+/* Add a port; *port_id (may be NULL) receives its index.  FDTD_ERANGE if a sample lies outside the grid. */
+int fdtd_add_port(fdtd_t*, const fdtd_port* p, int* port_id);
+
+/* Frequencies [Hz] of the running DFT of every port's V and I.  nf = 0 switches it off. */
+int fdtd_set_dft(fdtd_t*, const double* freqs_hz, int nf);
+
+int fdtd_set_option(fdtd_t*, int option, long value);
+
+/* Bytes of device memory fdtd_commit() needs with the settings made so far. */
+size_t fdtd_workspace_bytes(const fdtd_t*);
+
+/* Adopt the caller's device buffer (device pointer, >= fdtd_workspace_bytes(), 256-byte aligned) and CUDA stream
+ * (a cudaStream_t passed as void*; NULL = the legacy default stream), build the CPML / port tables, zero all state,
+ * set vacuum everywhere.  All later work is enqueued on that stream. */
+int fdtd_commit(fdtd_t*, void* device_workspace, size_t bytes, void* cuda_stream);
+
+/* Materials, component-sampled at the location of each E (eps_r, sigma) and H (mu_r) sample; the library never
+ * averages (R12).  sigma = +INFINITY marks a perfect conductor.  Coefficients (R3):
+ *   a = sigma*dt/(2*eps0*eps_r);  Ca = (1-a)/(1+a);  Cb = (dt/(eps0*eps_r))/(1+a);  Db = dt/(mu0*mu_r).
+ * indexed: idx = N uint8, host or device; eps_r, sigma, mu_r = host arrays [n_entries][3] (x,y,z component), mu_r may
+ *          be NULL (= 1) and must be NULL unless has_mu was declared.
+ * full:    eps_r[c], sigma[c], mu_r[c] = arrays of N elements of the field precision, host or device; mu_r may be NULL.
+ * May be called again later to change materials; fields are not touched. */
+int fdtd_set_materials_indexed(fdtd_t*, const uint8_t* idx, int n_entries, const double* eps_r, const double* sigma,
+                               const double* mu_r);
+int fdtd_set_materials_full(fdtd_t*, const void* const eps_r[3], const void* const sigma[3], const void* const mu_r[3]);
+
+/* Enqueue n full time steps (R5: psi_H, H; psi_E, E, walls; source; probes; DFT) on the stream.  Does not synchronise. */
+int fdtd_step(fdtd_t*, long n);
+
+/* Copy one field component (FDTD_EX..FDTD_HZ) to / from a caller array of N elements of the field precision, host or
+ * device.  Stream-ordered; synchronises the stream before returning when the caller array is in host memory.
+ * write_fields is the test hook for initial conditions and the resume path. */
+int fdtd_read_fields(fdtd_t*, int comp, void* dst);
+int fdtd_write_fields(fdtd_t*, int comp, const void* src);
+
+/* DFT accumulators of one port: V_reim and I_reim receive 2*nf doubles (re, im interleaved), host memory.
+ *   V^[m] = sum_n V^{n+1}  exp(-j 2 pi f_m (n+1)  dt) dt,   I^[m] = sum_n I^{n+1/2} exp(-j 2 pi f_m (n+1/2) dt) dt   (R8)
+ * Synchronises the stream. */
+int fdtd_read_port_dft(fdtd_t*, int port, double* V_reim, double* I_reim);
+/* V and I of the most recent step (debug / history recording).  Synchronises the stream. */
+int fdtd_read_port_last(fdtd_t*, int port, double* V, double* I);
+
+/* Zero fields, psi, DFT accumulators and the step counter; materials, ports and tables stay. */
+int fdtd_reset(fdtd_t*);
+
+long fdtd_step_count(const fdtd_t*);
+/* Number of kernel launches the library has enqueued since commit (graph nodes count individually). */
+long fdtd_launch_count(const fdtd_t*);
+/* Name of the step implementation in use after commit ("two_pass", "fused"), for reports. */
+const char* fdtd_impl_name(const fdtd_t*);
+const char* fdtd_last_error(const fdtd_t*);
+void fdtd_destroy(fdtd_t*);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FDTD_B200_H */
