@@ -1,0 +1,626 @@
+// fdtd_api.cu -- host plan and C ABI (include/fdtd.h) of the B200-native Yee FDTD hot path.
+//
+// The host side only validates arguments, builds small tables in fp64 (material table R3, CPML profile vectors R4,
+// port descriptors), carves the caller's workspace and enqueues kernels / CUDA graphs on the caller's stream.  Every
+// step of the method runs in the kernels of fdtd_kernels.cuh / fdtd_fused.cuh.  There is no CPU fallback.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <limits>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/fdtd.h"
+#include "fdtd_kernels.cuh"
+#include "fdtd_params.h"
+
+using namespace fdtd_b200;
+
+namespace {
+
+// R2: constants chosen so that c is exact.
+constexpr double kC0 = 299792458.0;
+constexpr double kPi = 3.14159265358979323846264338327950288;
+constexpr double kMu0 = 4.0e-7 * kPi;
+constexpr double kEps0 = 1.0 / (kMu0 * kC0 * kC0);
+constexpr double kEta0 = kMu0 * kC0;
+
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+}  // namespace
+
+// The opaque handle.  Precision-independent state lives here; the typed part is in Solver<T>.
+struct fdtd {
+  virtual ~fdtd() {}
+  int nx = 0, ny = 0, nz = 0;
+  double dx = 0, dy = 0, dz = 0, dt = 0;
+  int precision = FDTD_F32;
+  int npml[6] = {0, 0, 0, 0, 0, 0};
+  double cpml[6] = {3.0, 1.0, 1.0, 0.0, 0.8, 1.0};  // m, m_a, kappa_max, alpha_max, sigma_factor, eps_r_pml (R4)
+  int mat_mode = FDTD_MAT_INDEXED;
+  int has_mu = 0;
+  std::vector<PortDev> ports;
+  std::vector<double> freqs;
+  long opt_impl = 0, opt_graph = 1, opt_unroll = 8;
+  bool committed = false;
+  long nstep = 0;
+  long launches = 0;
+  std::string err;
+  cudaStream_t stream = nullptr;
+
+  int fail(int code, const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    err = buf;
+    return code;
+  }
+  int cuda_fail(cudaError_t e, const char* what) {
+    return fail(FDTD_ECUDA, "%s: %s", what, cudaGetErrorString(e));
+  }
+
+  size_t esize() const { return precision == FDTD_F64 ? 8 : 4; }
+  // padded geometry (fdtd_params.h)
+  int pitch() const { const int q = 128 / (int)esize(); return (nx + 1 + q - 1) / q * q; }
+  long long plane() const { return (long long)pitch() * (ny + 1); }
+  long long cells_padded() const { return plane() * (nz + 2); }
+  int S(int a) const { return npml[2 * a] + npml[2 * a + 1]; }
+
+  virtual size_t workspace_bytes() const = 0;
+  virtual int commit(void* ws, size_t bytes, void* stream) = 0;
+  virtual int set_materials_indexed(const uint8_t* idx, int ne, const double* eps, const double* sig, const double* mu) = 0;
+  virtual int set_materials_full(const void* const eps[3], const void* const sig[3], const void* const mu[3]) = 0;
+  virtual int step(long n) = 0;
+  virtual int read_field(int comp, void* dst) = 0;
+  virtual int write_field(int comp, const void* src) = 0;
+  virtual int read_port_dft(int port, double* V, double* I) = 0;
+  virtual int read_port_last(int port, double* V, double* I) = 0;
+  virtual int reset() = 0;
+  virtual const char* impl_name() const = 0;
+};
+
+namespace {
+
+bool is_device_ptr(const void* p) {
+  cudaPointerAttributes a;
+  if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+  return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+template <typename T>
+struct Solver : fdtd {
+  // workspace carve (byte offsets), filled by layout()
+  struct Carve {
+    size_t field[6], idx, tab, coef[9], psi[12], vec[18], ports, freqs, dftV, dftI, lastV, lastI, nstep, total;
+  };
+  char* ws = nullptr;
+  Carve cv{};
+  StepParams<T> sp{};
+  PortParams<T> pp{};
+  std::vector<T> h_tab;        // host staging of the material table (kept alive for the async upload)
+  std::vector<T> h_vec[18];
+  cudaGraphExec_t gexec = nullptr;
+  int graph_steps = 0;
+
+  ~Solver() override { if (gexec) cudaGraphExecDestroy(gexec); }
+
+  int mode() const { return (mat_mode == FDTD_MAT_FULL ? kModeFull : 0) | (has_mu ? kModeMu : 0); }
+  size_t psi_elems(int a) const {
+    if (S(a) == 0) return 0;
+    if (a == 0) return (size_t)S(0) * ny * nz;
+    if (a == 1) return (size_t)pitch() * S(1) * nz;
+    return (size_t)pitch() * ny * S(2);
+  }
+  static int psi_axis(int q) {  // axis of the derivative that drives psi array q
+    switch (q) { case pHxy: case pHzy: case pExy: case pEzy: return 1; case pHxz: case pHyz: case pExz: case pEyz: return 2; }
+    return 0;
+  }
+
+  Carve layout() const {
+    Carve c{};
+    size_t off = 0;
+    auto take = [&](size_t bytes) { const size_t o = off; off += align_up(bytes, 256); return o; };
+    const size_t fbytes = (size_t)cells_padded() * sizeof(T);
+    for (int f = 0; f < 6; ++f) c.field[f] = take(fbytes);
+    if (mat_mode == FDTD_MAT_INDEXED) {
+      c.idx = take((size_t)cells_padded());
+      c.tab = take(9 * kMaxTable * sizeof(T));
+    } else {
+      for (int q = 0; q < (has_mu ? 9 : 6); ++q) c.coef[q] = take(fbytes);
+    }
+    for (int q = 0; q < 12; ++q) c.psi[q] = take(psi_elems(psi_axis(q)) * sizeof(T));
+    for (int a = 0; a < 3; ++a)
+      for (int v = 0; v < 6; ++v) c.vec[a * 6 + v] = take((size_t)(S(a) > 0 ? S(a) : 1) * sizeof(T));
+    c.ports = take((ports.size() + 1) * sizeof(PortDev));
+    c.freqs = take((freqs.size() + 1) * sizeof(double));
+    c.dftV = take((ports.size() * freqs.size() + 1) * 2 * sizeof(double));
+    c.dftI = take((ports.size() * freqs.size() + 1) * 2 * sizeof(double));
+    c.lastV = take((ports.size() + 1) * sizeof(double));
+    c.lastI = take((ports.size() + 1) * sizeof(double));
+    c.nstep = take(sizeof(long long));
+    c.total = off;
+    return c;
+  }
+  size_t workspace_bytes() const override { return layout().total; }
+
+  T* field_origin(int f) const { return reinterpret_cast<T*>(ws + cv.field[f]) + plane(); }
+
+  int commit(void* w, size_t bytes, void* st) override;
+  int set_materials_indexed(const uint8_t* idx, int ne, const double* eps, const double* sig, const double* mu) override;
+  int set_materials_full(const void* const eps[3], const void* const sig[3], const void* const mu[3]) override;
+  int step(long n) override;
+  int read_field(int comp, void* dst) override { return copy_field(comp, dst, true); }
+  int write_field(int comp, const void* src) override { return copy_field(comp, const_cast<void*>(src), false); }
+  int read_port_dft(int port, double* V, double* I) override;
+  int read_port_last(int port, double* V, double* I) override;
+  int reset() override;
+  const char* impl_name() const override { return "two_pass"; }
+
+  int copy_field(int comp, void* user, bool to_user);
+  int copy3d(void* internal_origin, size_t elem, void* user, bool to_user);
+  void build_cpml_vectors();
+  void enqueue_step();
+  int build_graph();
+};
+
+// R4 (CPML, convolutional PML with recursive convolution): per axis, per slab coordinate s, at the E positions
+// (integer) and the H positions (half-integer):
+//   rho = depth into the layer in [0,1];  sigma = sigma_max rho^m;  kappa = 1 + (kappa_max-1) rho^m;
+//   alpha = alpha_max (1-rho)^m_a;  b = exp(-(sigma/kappa + alpha) dt/eps0);  c = sigma (b-1) / (kappa (sigma + kappa alpha))
+//   sigma_max = sigma_factor (m+1) / (eta0 d_axis sqrt(eps_r_pml)).
+template <typename T>
+void Solver<T>::build_cpml_vectors() {
+  const double m = cpml[0], ma = cpml[1], kmax = cpml[2], amax = cpml[3], sfac = cpml[4], erp = cpml[5];
+  const int nn[3] = {nx, ny, nz};
+  const double dd[3] = {dx, dy, dz};
+  for (int a = 0; a < 3; ++a) {
+    const int lo = npml[2 * a], hi = npml[2 * a + 1], n = nn[a], s_tot = lo + hi;
+    for (int v = 0; v < 6; ++v) h_vec[a * 6 + v].assign(s_tot > 0 ? s_tot : 1, T(v % 3 == 1 ? 0 : 1));
+    const double smax = sfac * (m + 1.0) / (kEta0 * dd[a] * std::sqrt(erp));
+    for (int s = 0; s < s_tot; ++s) {
+      const int u = s < lo ? s : n - hi + (s - lo);
+      for (int half = 0; half < 2; ++half) {
+        const double pos = u + 0.5 * half;
+        double rho = 0.0;
+        if (lo > 0 && pos < lo) rho = (lo - pos) / lo;
+        else if (hi > 0 && pos > n - hi) rho = (pos - (n - hi)) / hi;
+        const double g = std::pow(rho, m);
+        const double sg = smax * g, kp = 1.0 + (kmax - 1.0) * g, al = amax * std::pow(1.0 - rho, ma);
+        const double b = std::exp(-(sg / kp + al) * dt / kEps0);
+        const double c = sg == 0.0 ? 0.0 : sg * (b - 1.0) / (kp * (sg + kp * al));
+        h_vec[a * 6 + 3 * half + 0][s] = T(b);
+        h_vec[a * 6 + 3 * half + 1][s] = T(c);
+        h_vec[a * 6 + 3 * half + 2][s] = T(1.0 / kp);
+      }
+    }
+  }
+}
+
+template <typename T>
+int Solver<T>::commit(void* w, size_t bytes, void* st) {
+  if (committed) return fail(FDTD_ESTATE, "fdtd_commit: already committed");
+  int ndev = 0;
+  cudaError_t e = cudaGetDeviceCount(&ndev);
+  if (e != cudaSuccess || ndev == 0) { cudaGetLastError(); return fail(FDTD_ECUDA, "fdtd_commit: no CUDA device (there is no CPU fallback)"); }
+  if (!w || ((uintptr_t)w & 255)) return fail(FDTD_EINVAL, "fdtd_commit: workspace must be a 256-byte aligned device pointer");
+  if (!is_device_ptr(w)) return fail(FDTD_EINVAL, "fdtd_commit: workspace is not device memory");
+  cv = layout();
+  if (bytes < cv.total) return fail(FDTD_ENOMEM, "fdtd_commit: workspace of %zu bytes given, %zu needed", bytes, cv.total);
+  ws = static_cast<char*>(w);
+  stream = static_cast<cudaStream_t>(st);
+  if ((e = cudaMemsetAsync(ws, 0, cv.total, stream)) != cudaSuccess) return cuda_fail(e, "fdtd_commit: memset");
+
+  // step parameters
+  sp = StepParams<T>{};
+  sp.nx = nx; sp.ny = ny; sp.nz = nz; sp.P = pitch(); sp.PS = plane();
+  for (int f = 0; f < 6; ++f) sp.src[f] = sp.dst[f] = field_origin(f);
+  if (mat_mode == FDTD_MAT_INDEXED) {
+    sp.idx = reinterpret_cast<uint8_t*>(ws + cv.idx) + plane();
+    sp.tab = reinterpret_cast<T*>(ws + cv.tab);
+  } else {
+    for (int c = 0; c < 3; ++c) {
+      sp.Ca[c] = reinterpret_cast<T*>(ws + cv.coef[c]) + plane();
+      sp.Cb[c] = reinterpret_cast<T*>(ws + cv.coef[3 + c]) + plane();
+      if (has_mu) sp.Db[c] = reinterpret_cast<T*>(ws + cv.coef[6 + c]) + plane();
+    }
+  }
+  sp.db0 = T(dt / kMu0);
+  sp.idx_ = T(1.0 / dx); sp.idy_ = T(1.0 / dy); sp.idz_ = T(1.0 / dz);
+  for (int a = 0; a < 3; ++a) { sp.lo[a] = npml[2 * a]; sp.hi[a] = npml[2 * a + 1]; }
+  build_cpml_vectors();
+  for (int a = 0; a < 3; ++a) {
+    const T** tgt[6] = {&sp.bE[a], &sp.cE[a], &sp.kE[a], &sp.bH[a], &sp.cH[a], &sp.kH[a]};
+    for (int v = 0; v < 6; ++v) {
+      T* d = reinterpret_cast<T*>(ws + cv.vec[a * 6 + v]);
+      *tgt[v] = d;
+      const std::vector<T>& h = h_vec[a * 6 + v];
+      if ((e = cudaMemcpyAsync(d, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice, stream)) != cudaSuccess)
+        return cuda_fail(e, "fdtd_commit: upload CPML vectors");
+    }
+  }
+  for (int q = 0; q < 12; ++q) sp.psi[q] = reinterpret_cast<T*>(ws + cv.psi[q]);
+  sp.nstep = reinterpret_cast<long long*>(ws + cv.nstep);
+
+  // port parameters
+  pp = PortParams<T>{};
+  pp.P = sp.P; pp.PS = sp.PS;
+  pp.Ez = sp.src[kEz]; pp.Hy = sp.src[kHy]; pp.Hz = sp.src[kHz];
+  pp.ports = reinterpret_cast<PortDev*>(ws + cv.ports);
+  pp.nports = (int)ports.size();
+  pp.freqs = reinterpret_cast<double*>(ws + cv.freqs);
+  pp.nf = (int)freqs.size();
+  pp.dftV = reinterpret_cast<double*>(ws + cv.dftV);
+  pp.dftI = reinterpret_cast<double*>(ws + cv.dftI);
+  pp.lastV = reinterpret_cast<double*>(ws + cv.lastV);
+  pp.lastI = reinterpret_cast<double*>(ws + cv.lastI);
+  pp.nstep = sp.nstep;
+  pp.dt = dt; pp.dy = dy; pp.dz = dz;
+  if (!ports.empty() &&
+      (e = cudaMemcpyAsync(ws + cv.ports, ports.data(), ports.size() * sizeof(PortDev), cudaMemcpyHostToDevice, stream)) != cudaSuccess)
+    return cuda_fail(e, "fdtd_commit: upload ports");
+  if (!freqs.empty() &&
+      (e = cudaMemcpyAsync(ws + cv.freqs, freqs.data(), freqs.size() * sizeof(double), cudaMemcpyHostToDevice, stream)) != cudaSuccess)
+    return cuda_fail(e, "fdtd_commit: upload frequencies");
+
+  // vacuum everywhere
+  const long long np = cells_padded();
+  const unsigned nb = (unsigned)((np + 255) / 256);
+  if (mat_mode == FDTD_MAT_INDEXED) {
+    h_tab.assign(9 * kMaxTable, T(0));
+    for (int m = 0; m < kMaxTable; ++m)
+      for (int c = 0; c < 3; ++c) {
+        h_tab[c * kMaxTable + m] = T(1);
+        h_tab[(3 + c) * kMaxTable + m] = T(dt / kEps0);
+        h_tab[(6 + c) * kMaxTable + m] = T(dt / kMu0);
+      }
+    if ((e = cudaMemcpyAsync(ws + cv.tab, h_tab.data(), h_tab.size() * sizeof(T), cudaMemcpyHostToDevice, stream)) != cudaSuccess)
+      return cuda_fail(e, "fdtd_commit: upload table");
+  } else {
+    for (int c = 0; c < 3; ++c) {
+      k_fill<T><<<nb, 256, 0, stream>>>(reinterpret_cast<T*>(ws + cv.coef[c]), np, T(1));
+      k_fill<T><<<nb, 256, 0, stream>>>(reinterpret_cast<T*>(ws + cv.coef[3 + c]), np, T(dt / kEps0));
+      if (has_mu) k_fill<T><<<nb, 256, 0, stream>>>(reinterpret_cast<T*>(ws + cv.coef[6 + c]), np, T(dt / kMu0));
+    }
+  }
+  if ((e = cudaStreamSynchronize(stream)) != cudaSuccess) return cuda_fail(e, "fdtd_commit");
+  if ((e = cudaGetLastError()) != cudaSuccess) return cuda_fail(e, "fdtd_commit");
+  committed = true;
+  nstep = 0;
+  launches = 0;
+  return FDTD_OK;
+}
+
+// copy between a caller array of nx*ny*nz elements (host or device) and a padded internal array
+template <typename T>
+int Solver<T>::copy3d(void* internal_base, size_t elem, void* user, bool to_user) {
+  cudaMemcpy3DParms q{};
+  const cudaPitchedPtr in = make_cudaPitchedPtr(internal_base, (size_t)pitch() * elem, (size_t)pitch() * elem, ny + 1);
+  const cudaPitchedPtr us = make_cudaPitchedPtr(user, (size_t)nx * elem, (size_t)nx * elem, ny);
+  const cudaPos pin = make_cudaPos(0, 0, 1), pus = make_cudaPos(0, 0, 0);
+  if (to_user) { q.srcPtr = in; q.srcPos = pin; q.dstPtr = us; q.dstPos = pus; }
+  else         { q.srcPtr = us; q.srcPos = pus; q.dstPtr = in; q.dstPos = pin; }
+  q.extent = make_cudaExtent((size_t)nx * elem, ny, nz);
+  q.kind = cudaMemcpyDefault;
+  const cudaError_t e = cudaMemcpy3DAsync(&q, stream);
+  if (e != cudaSuccess) return cuda_fail(e, "3-D copy");
+  if (!is_device_ptr(user)) {
+    const cudaError_t e2 = cudaStreamSynchronize(stream);
+    if (e2 != cudaSuccess) return cuda_fail(e2, "3-D copy");
+  }
+  return FDTD_OK;
+}
+
+template <typename T>
+int Solver<T>::copy_field(int comp, void* user, bool to_user) {
+  if (!committed) return fail(FDTD_ESTATE, "fields are available after fdtd_commit");
+  if (comp < 0 || comp > 5 || !user) return fail(FDTD_EINVAL, "bad component or null pointer");
+  return copy3d(ws + cv.field[comp], sizeof(T), user, to_user);
+}
+
+template <typename T>
+int Solver<T>::set_materials_indexed(const uint8_t* idx, int ne, const double* eps, const double* sig, const double* mu) {
+  if (!committed) return fail(FDTD_ESTATE, "fdtd_set_materials_indexed: call after fdtd_commit");
+  if (mat_mode != FDTD_MAT_INDEXED) return fail(FDTD_ESTATE, "fdtd_set_materials_indexed: handle is in FULL mode");
+  if (!idx || !eps || !sig || ne < 1 || ne > kMaxTable) return fail(FDTD_EINVAL, "fdtd_set_materials_indexed: bad arguments");
+  if (mu && !has_mu) return fail(FDTD_EINVAL, "fdtd_set_materials_indexed: mu_r given but has_mu was not declared");
+  for (int q = 0; q < 3 * ne; ++q) {
+    if (!(eps[q] > 0) || !(sig[q] >= 0) || (mu && !(mu[q] > 0)))
+      return fail(FDTD_EINVAL, "fdtd_set_materials_indexed: entry %d: need eps_r > 0, sigma >= 0, mu_r > 0", q / 3);
+  }
+  // R3: a = sigma dt / (2 eps0 eps_r); Ca = (1-a)/(1+a); Cb = (dt/(eps0 eps_r))/(1+a); sigma = +inf -> PEC (0, 0)
+  h_tab.assign(9 * kMaxTable, T(0));
+  for (int m = 0; m < kMaxTable; ++m) {
+    const int s = m < ne ? m : 0;  // indices beyond the table alias entry 0 (never produce wild values)
+    for (int c = 0; c < 3; ++c) {
+      const double er = eps[3 * s + c], sg = sig[3 * s + c], mr = mu ? mu[3 * s + c] : 1.0;
+      double ca = 0.0, cb = 0.0;
+      if (!std::isinf(sg)) { const double a = sg * dt / (2.0 * kEps0 * er); ca = (1.0 - a) / (1.0 + a); cb = (dt / (kEps0 * er)) / (1.0 + a); }
+      h_tab[c * kMaxTable + m] = T(ca);
+      h_tab[(3 + c) * kMaxTable + m] = T(cb);
+      h_tab[(6 + c) * kMaxTable + m] = T(dt / (kMu0 * mr));
+    }
+  }
+  cudaError_t e = cudaMemcpyAsync(ws + cv.tab, h_tab.data(), h_tab.size() * sizeof(T), cudaMemcpyHostToDevice, stream);
+  if (e != cudaSuccess) return cuda_fail(e, "fdtd_set_materials_indexed: upload table");
+  const int r = copy3d(ws + cv.idx, 1, const_cast<uint8_t*>(idx), false);
+  if (r != FDTD_OK) return r;
+  if ((e = cudaStreamSynchronize(stream)) != cudaSuccess) return cuda_fail(e, "fdtd_set_materials_indexed");
+  return FDTD_OK;
+}
+
+template <typename T>
+int Solver<T>::set_materials_full(const void* const eps[3], const void* const sig[3], const void* const mu[3]) {
+  if (!committed) return fail(FDTD_ESTATE, "fdtd_set_materials_full: call after fdtd_commit");
+  if (mat_mode != FDTD_MAT_FULL) return fail(FDTD_ESTATE, "fdtd_set_materials_full: handle is in INDEXED mode");
+  if (!eps || !sig) return fail(FDTD_EINVAL, "fdtd_set_materials_full: null argument");
+  for (int c = 0; c < 3; ++c) if (!eps[c] || !sig[c]) return fail(FDTD_EINVAL, "fdtd_set_materials_full: null array");
+  if (mu && !has_mu) return fail(FDTD_EINVAL, "fdtd_set_materials_full: mu_r given but has_mu was not declared");
+  if (mu) for (int c = 0; c < 3; ++c) if (!mu[c]) return fail(FDTD_EINVAL, "fdtd_set_materials_full: null mu array");
+  const long long np = cells_padded();
+  const unsigned nb = (unsigned)((np + 255) / 256);
+  cudaError_t e;
+  for (int c = 0; c < 3; ++c) {
+    T* ca = reinterpret_cast<T*>(ws + cv.coef[c]);
+    T* cb = reinterpret_cast<T*>(ws + cv.coef[3 + c]);
+    if ((e = cudaMemsetAsync(ca, 0, np * sizeof(T), stream)) != cudaSuccess) return cuda_fail(e, "memset");
+    if ((e = cudaMemsetAsync(cb, 0, np * sizeof(T), stream)) != cudaSuccess) return cuda_fail(e, "memset");
+    int r = copy3d(ca, sizeof(T), const_cast<void*>(eps[c]), false);
+    if (r != FDTD_OK) return r;
+    if ((r = copy3d(cb, sizeof(T), const_cast<void*>(sig[c]), false)) != FDTD_OK) return r;
+    k_coef_E<T><<<nb, 256, 0, stream>>>(ca, cb, np, dt, kEps0);
+    if (has_mu) {
+      T* db = reinterpret_cast<T*>(ws + cv.coef[6 + c]);
+      if (mu) {
+        if ((e = cudaMemsetAsync(db, 0, np * sizeof(T), stream)) != cudaSuccess) return cuda_fail(e, "memset");
+        if ((r = copy3d(db, sizeof(T), const_cast<void*>(mu[c]), false)) != FDTD_OK) return r;
+        k_coef_H<T><<<nb, 256, 0, stream>>>(db, np, dt, kMu0);
+      } else {
+        k_fill<T><<<nb, 256, 0, stream>>>(db, np, T(dt / kMu0));
+      }
+    }
+  }
+  if ((e = cudaStreamSynchronize(stream)) != cudaSuccess) return cuda_fail(e, "fdtd_set_materials_full");
+  if ((e = cudaGetLastError()) != cudaSuccess) return cuda_fail(e, "fdtd_set_materials_full");
+  return FDTD_OK;
+}
+
+// ---- one step = H pass, E pass, sources, probes + DFT (R5) -------------------------------------------------------
+template <typename T, int MODE>
+static void launch_two_pass(const StepParams<T>& sp, cudaStream_t st) {
+  constexpr int V = VecOf<T>::V;
+  const int nvec = (sp.nx + V - 1) / V;
+  int bx = 1;
+  while (bx < nvec && bx < 128) bx <<= 1;
+  const int by = 128 / bx;
+  const dim3 block(bx, by, 1), grid((nvec + bx - 1) / bx, (sp.ny + by - 1) / by, sp.nz);
+  k_update_H<T, MODE><<<grid, block, 0, st>>>(sp);
+  k_update_E<T, MODE><<<grid, block, 0, st>>>(sp);
+}
+
+template <typename T>
+void Solver<T>::enqueue_step() {
+  switch (mode()) {
+    case 0: launch_two_pass<T, 0>(sp, stream); break;
+    case 1: launch_two_pass<T, 1>(sp, stream); break;
+    case 2: launch_two_pass<T, 2>(sp, stream); break;
+    default: launch_two_pass<T, 3>(sp, stream); break;
+  }
+  launches += 2;
+  if (!ports.empty()) {
+    bool any_src = false;
+    for (const PortDev& q : ports) any_src = any_src || q.has_source;
+    if (any_src) { k_source<T><<<1, 256, 0, stream>>>(pp); ++launches; }
+    const dim3 grid((unsigned)ports.size(), (unsigned)(freqs.empty() ? 1 : (freqs.size() + 63) / 64), 1);
+    k_probe_dft<T><<<grid, 128, 0, stream>>>(pp);
+    ++launches;
+  }
+}
+
+template <typename T>
+int Solver<T>::build_graph() {
+  if (gexec) return FDTD_OK;
+  const long before = launches;
+  cudaError_t e = cudaStreamBeginCapture(stream, cudaStreamCaptureModeThreadLocal);
+  if (e != cudaSuccess) return cuda_fail(e, "graph capture begin");
+  for (int s = 0; s < (int)opt_unroll; ++s) enqueue_step();
+  cudaGraph_t g = nullptr;
+  e = cudaStreamEndCapture(stream, &g);
+  launches = before;
+  if (e != cudaSuccess) return cuda_fail(e, "graph capture end");
+  e = cudaGraphInstantiate(&gexec, g, 0);
+  cudaGraphDestroy(g);
+  if (e != cudaSuccess) { gexec = nullptr; return cuda_fail(e, "graph instantiate"); }
+  graph_steps = (int)opt_unroll;
+  return FDTD_OK;
+}
+
+template <typename T>
+int Solver<T>::step(long n) {
+  if (!committed) return fail(FDTD_ESTATE, "fdtd_step: call after fdtd_commit");
+  if (n < 0) return fail(FDTD_EINVAL, "fdtd_step: n < 0");
+  long left = n;
+  if (opt_graph && stream != nullptr && left >= opt_unroll) {
+    const int r = build_graph();
+    if (r != FDTD_OK) return r;
+    const long per = launches;  // count the launches of one replay
+    (void)per;
+    long nodes = 2;
+    if (!ports.empty()) { nodes += 1; for (const PortDev& q : ports) if (q.has_source) { nodes += 1; break; } }
+    while (left >= graph_steps) {
+      const cudaError_t e = cudaGraphLaunch(gexec, stream);
+      if (e != cudaSuccess) return cuda_fail(e, "graph launch");
+      left -= graph_steps;
+      launches += nodes * graph_steps;
+    }
+  }
+  for (; left > 0; --left) enqueue_step();
+  const cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return cuda_fail(e, "fdtd_step");
+  nstep += n;
+  return FDTD_OK;
+}
+
+template <typename T>
+int Solver<T>::read_port_dft(int port, double* V, double* I) {
+  if (!committed) return fail(FDTD_ESTATE, "fdtd_read_port_dft: call after fdtd_commit");
+  if (port < 0 || port >= (int)ports.size() || !V || !I) return fail(FDTD_EINVAL, "fdtd_read_port_dft: bad port or null pointer");
+  const size_t nf = freqs.size();
+  cudaError_t e = cudaSuccess;
+  if (nf) {
+    e = cudaMemcpyAsync(V, pp.dftV + (size_t)port * nf * 2, nf * 2 * sizeof(double), cudaMemcpyDeviceToHost, stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(I, pp.dftI + (size_t)port * nf * 2, nf * 2 * sizeof(double), cudaMemcpyDeviceToHost, stream);
+  }
+  if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+  if (e != cudaSuccess) return cuda_fail(e, "fdtd_read_port_dft");
+  return FDTD_OK;
+}
+
+template <typename T>
+int Solver<T>::read_port_last(int port, double* V, double* I) {
+  if (!committed) return fail(FDTD_ESTATE, "fdtd_read_port_last: call after fdtd_commit");
+  if (port < 0 || port >= (int)ports.size() || !V || !I) return fail(FDTD_EINVAL, "fdtd_read_port_last: bad port or null pointer");
+  cudaError_t e = cudaMemcpyAsync(V, pp.lastV + port, sizeof(double), cudaMemcpyDeviceToHost, stream);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(I, pp.lastI + port, sizeof(double), cudaMemcpyDeviceToHost, stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+  if (e != cudaSuccess) return cuda_fail(e, "fdtd_read_port_last");
+  return FDTD_OK;
+}
+
+template <typename T>
+int Solver<T>::reset() {
+  if (!committed) return fail(FDTD_ESTATE, "fdtd_reset: call after fdtd_commit");
+  cudaError_t e = cudaSuccess;
+  const size_t fbytes = (size_t)cells_padded() * sizeof(T);
+  for (int f = 0; f < 6 && e == cudaSuccess; ++f) e = cudaMemsetAsync(ws + cv.field[f], 0, fbytes, stream);
+  for (int q = 0; q < 12 && e == cudaSuccess; ++q)
+    if (psi_elems(psi_axis(q))) e = cudaMemsetAsync(ws + cv.psi[q], 0, psi_elems(psi_axis(q)) * sizeof(T), stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(ws + cv.dftV, 0, cv.nstep + sizeof(long long) - cv.dftV, stream);
+  if (e != cudaSuccess) return cuda_fail(e, "fdtd_reset");
+  nstep = 0;
+  return FDTD_OK;
+}
+
+}  // namespace
+
+// ===================================================================================================================
+// C ABI
+// ===================================================================================================================
+extern "C" {
+
+int fdtd_create(int nx, int ny, int nz, double dx, double dy, double dz, double dt, int precision, fdtd_t** out) {
+  if (!out) return FDTD_EINVAL;
+  *out = nullptr;
+  if (nx < 2 || ny < 2 || nz < 2 || !(dx > 0) || !(dy > 0) || !(dz > 0) || !(dt > 0)) return FDTD_EINVAL;
+  if (precision != FDTD_F32 && precision != FDTD_F64) return FDTD_EINVAL;
+  if ((long long)nx * ny * nz > (1LL << 40) || nz > 65535 || ny > 65535 * 128) return FDTD_EINVAL;
+  // the explicit scheme is run at a CFL number of 0.9; the limit itself:
+  const double dt_max = 1.0 / (kC0 * std::sqrt(1.0 / (dx * dx) + 1.0 / (dy * dy) + 1.0 / (dz * dz)));
+  if (dt > dt_max) return FDTD_ECFL;
+  fdtd* h = nullptr;
+  if (precision == FDTD_F64) h = new (std::nothrow) Solver<double>();
+  else h = new (std::nothrow) Solver<float>();
+  if (!h) return FDTD_ENOMEM;
+  h->nx = nx; h->ny = ny; h->nz = nz; h->dx = dx; h->dy = dy; h->dz = dz; h->dt = dt; h->precision = precision;
+  *out = h;
+  return FDTD_OK;
+}
+
+int fdtd_set_boundary(fdtd_t* h, const int pml_cells[6], const double* cpml) {
+  if (!h) return FDTD_EINVAL;
+  if (h->committed) return h->fail(FDTD_ESTATE, "fdtd_set_boundary: call before fdtd_commit");
+  if (!pml_cells) return h->fail(FDTD_EINVAL, "fdtd_set_boundary: null pml_cells");
+  const int n[3] = {h->nx, h->ny, h->nz};
+  for (int a = 0; a < 3; ++a) {
+    if (pml_cells[2 * a] < 0 || pml_cells[2 * a + 1] < 0) return h->fail(FDTD_EINVAL, "fdtd_set_boundary: negative thickness");
+    if (pml_cells[2 * a] + pml_cells[2 * a + 1] > n[a]) return h->fail(FDTD_ERANGE, "fdtd_set_boundary: CPML thicker than the grid on axis %d", a);
+  }
+  if (cpml) {
+    if (!(cpml[0] >= 0) || !(cpml[1] >= 0) || !(cpml[2] >= 1) || !(cpml[3] >= 0) || !(cpml[4] >= 0) || !(cpml[5] > 0))
+      return h->fail(FDTD_EINVAL, "fdtd_set_boundary: need m, m_a >= 0, kappa_max >= 1, alpha_max >= 0, sigma_factor >= 0, eps_r_pml > 0");
+    for (int q = 0; q < 6; ++q) h->cpml[q] = cpml[q];
+  }
+  for (int q = 0; q < 6; ++q) h->npml[q] = pml_cells[q];
+  return FDTD_OK;
+}
+
+int fdtd_set_material_mode(fdtd_t* h, int mode, int has_mu) {
+  if (!h) return FDTD_EINVAL;
+  if (h->committed) return h->fail(FDTD_ESTATE, "fdtd_set_material_mode: call before fdtd_commit");
+  if (mode != FDTD_MAT_INDEXED && mode != FDTD_MAT_FULL) return h->fail(FDTD_EINVAL, "fdtd_set_material_mode: bad mode");
+  h->mat_mode = mode;
+  h->has_mu = has_mu ? 1 : 0;
+  return FDTD_OK;
+}
+
+int fdtd_add_port(fdtd_t* h, const fdtd_port* p, int* port_id) {
+  if (!h) return FDTD_EINVAL;
+  if (h->committed) return h->fail(FDTD_ESTATE, "fdtd_add_port: call before fdtd_commit");
+  if (!p) return h->fail(FDTD_EINVAL, "fdtd_add_port: null port");
+  auto in = [](int v, int lo, int hi) { return v >= lo && v < hi; };
+  if (p->has_source) {
+    if (!(in(p->is, 0, h->nx) && in(p->sj0, 0, h->ny) && in(p->sj1, p->sj0, h->ny) && in(p->sk0, 0, h->nz) && p->sk1 > p->sk0 && p->sk1 <= h->nz))
+      return h->fail(FDTD_ERANGE, "fdtd_add_port: source box outside the grid");
+    if (p->waveform < FDTD_W_DGAUSS || p->waveform > FDTD_W_GSINE || !(p->sigma > 0))
+      return h->fail(FDTD_EINVAL, "fdtd_add_port: bad waveform or sigma <= 0");
+  }
+  if (!(in(p->ip, 0, h->nx) && in(p->vj0, 0, h->ny) && in(p->vj1, p->vj0, h->ny) && in(p->vk0, 0, h->nz) && p->vk1 > p->vk0 && p->vk1 <= h->nz))
+    return h->fail(FDTD_ERANGE, "fdtd_add_port: voltage box outside the grid");
+  if (!(in(p->lj0, 1, h->ny) && in(p->lj1, p->lj0, h->ny) && in(p->lk0, 1, h->nz) && in(p->lk1, p->lk0, h->nz)))
+    return h->fail(FDTD_ERANGE, "fdtd_add_port: current loop outside the grid (needs lj0 >= 1, lk0 >= 1)");
+  PortDev q{};
+  q.has_source = p->has_source ? 1 : 0;
+  q.is = p->is; q.sj0 = p->sj0; q.sj1 = p->sj1; q.sk0 = p->sk0; q.sk1 = p->sk1;
+  q.waveform = p->waveform; q.amp = p->amp; q.t0 = p->t0; q.sigma = p->sigma; q.f0 = p->f0;
+  q.ip = p->ip; q.vj0 = p->vj0; q.vj1 = p->vj1; q.vk0 = p->vk0; q.vk1 = p->vk1;
+  q.lj0 = p->lj0; q.lj1 = p->lj1; q.lk0 = p->lk0; q.lk1 = p->lk1;
+  h->ports.push_back(q);
+  if (port_id) *port_id = (int)h->ports.size() - 1;
+  return FDTD_OK;
+}
+
+int fdtd_set_dft(fdtd_t* h, const double* freqs_hz, int nf) {
+  if (!h) return FDTD_EINVAL;
+  if (h->committed) return h->fail(FDTD_ESTATE, "fdtd_set_dft: call before fdtd_commit");
+  if (nf < 0 || (nf > 0 && !freqs_hz)) return h->fail(FDTD_EINVAL, "fdtd_set_dft: bad arguments");
+  h->freqs.assign(freqs_hz, freqs_hz + nf);
+  return FDTD_OK;
+}
+
+int fdtd_set_option(fdtd_t* h, int option, long value) {
+  if (!h) return FDTD_EINVAL;
+  if (h->committed) return h->fail(FDTD_ESTATE, "fdtd_set_option: call before fdtd_commit");
+  switch (option) {
+    case FDTD_OPT_STEP_IMPL: if (value < 0 || value > 2) break; h->opt_impl = value; return FDTD_OK;
+    case FDTD_OPT_USE_GRAPH: h->opt_graph = value ? 1 : 0; return FDTD_OK;
+    case FDTD_OPT_GRAPH_UNROLL: if (value < 1 || value > 1024) break; h->opt_unroll = value; return FDTD_OK;
+  }
+  return h->fail(FDTD_EINVAL, "fdtd_set_option: unknown option %d or bad value %ld", option, value);
+}
+
+size_t fdtd_workspace_bytes(const fdtd_t* h) { return h ? h->workspace_bytes() : 0; }
+int fdtd_commit(fdtd_t* h, void* ws, size_t bytes, void* stream) { return h ? h->commit(ws, bytes, stream) : FDTD_EINVAL; }
+int fdtd_set_materials_indexed(fdtd_t* h, const uint8_t* idx, int n_entries, const double* eps_r, const double* sigma, const double* mu_r) {
+  return h ? h->set_materials_indexed(idx, n_entries, eps_r, sigma, mu_r) : FDTD_EINVAL;
+}
+int fdtd_set_materials_full(fdtd_t* h, const void* const eps_r[3], const void* const sigma[3], const void* const mu_r[3]) {
+  return h ? h->set_materials_full(eps_r, sigma, mu_r) : FDTD_EINVAL;
+}
+int fdtd_step(fdtd_t* h, long n) { return h ? h->step(n) : FDTD_EINVAL; }
+int fdtd_read_fields(fdtd_t* h, int comp, void* dst) { return h ? h->read_field(comp, dst) : FDTD_EINVAL; }
+int fdtd_write_fields(fdtd_t* h, int comp, const void* src) { return h ? h->write_field(comp, src) : FDTD_EINVAL; }
+int fdtd_read_port_dft(fdtd_t* h, int port, double* V, double* I) { return h ? h->read_port_dft(port, V, I) : FDTD_EINVAL; }
+int fdtd_read_port_last(fdtd_t* h, int port, double* V, double* I) { return h ? h->read_port_last(port, V, I) : FDTD_EINVAL; }
+int fdtd_reset(fdtd_t* h) { return h ? h->reset() : FDTD_EINVAL; }
+long fdtd_step_count(const fdtd_t* h) { return h ? h->nstep : -1; }
+long fdtd_launch_count(const fdtd_t* h) { return h ? h->launches : -1; }
+const char* fdtd_impl_name(const fdtd_t* h) { return h && h->committed ? h->impl_name() : ""; }
+const char* fdtd_last_error(const fdtd_t* h) { return h ? h->err.c_str() : "null handle"; }
+void fdtd_destroy(fdtd_t* h) { delete h; }
+
+}  // extern "C"

@@ -1,0 +1,368 @@
+// fdtd_kernels.cuh -- sm_100a kernels of the two-pass Yee step (H pass, E pass) and of the port work.
+//
+// One leapfrog step (include/fdtd.h; R5; "conventional FDTD" on a "Yee-grid"):
+//   k_update_H : psi_H on the CPML slabs, then H^{n+1/2} = H^{n-1/2} - Db * curl E^n          (all cells)
+//   k_update_E : psi_E on the CPML slabs, then E^{n+1} = Ca E^n + Cb * curl H^{n+1/2}, walls   (all cells)
+//   k_source   : E_z += amp * g((n+1) dt) on the source boxes (Eq. 3)
+//   k_probe_dft: V, I of every port (Eq. 4) and their running DFT
+// Each thread of the field kernels owns 16 bytes of consecutive x cells (float4 / double2): every aligned operand
+// (own cell, y+-1 row, z+-1 plane) is one 128-bit load, the x+-1 operand is one extra scalar load that hits the same
+// or the neighbouring L1 line.  The zero halo of the layout (fdtd_params.h) removes all bounds tests.
+#pragma once
+#include <cuda_runtime.h>
+#include "fdtd_params.h"
+
+namespace fdtd_b200 {
+
+template <typename T> struct VecOf;
+template <> struct VecOf<float>  { static constexpr int V = 4; };
+template <> struct VecOf<double> { static constexpr int V = 2; };
+
+__device__ __forceinline__ void ldv(const float* p, float (&r)[4]) {
+  const float4 v = *reinterpret_cast<const float4*>(p);
+  r[0] = v.x; r[1] = v.y; r[2] = v.z; r[3] = v.w;
+}
+__device__ __forceinline__ void ldv(const double* p, double (&r)[2]) {
+  const double2 v = *reinterpret_cast<const double2*>(p);
+  r[0] = v.x; r[1] = v.y;
+}
+__device__ __forceinline__ void stv(float* p, const float (&r)[4]) {
+  *reinterpret_cast<float4*>(p) = make_float4(r[0], r[1], r[2], r[3]);
+}
+__device__ __forceinline__ void stv(double* p, const double (&r)[2]) {
+  *reinterpret_cast<double2*>(p) = make_double2(r[0], r[1]);
+}
+
+// slab coordinate of index u on an axis of n cells with lo / hi CPML cells, or -1 in the interior
+__device__ __forceinline__ int slab_coord(int u, int lo, int hi, int n) {
+  return u < lo ? u : (u >= n - hi ? lo + u - (n - hi) : -1);
+}
+
+// Material modes: bit 0 = full per-cell coefficient arrays (else uint8 index + table), bit 1 = permeability given.
+enum { kModeIndexed = 0, kModeFull = 1, kModeMu = 2 };
+
+// ------------------------------------------------------------------------------------------------------------------
+// H pass.  R5 step 1:  psiH = bH psiH + cH D+E ;  Hx -= Dbx (D+y Ez / kHy + psiHxy - D+z Ey / kHz - psiHxz)  etc.
+// ------------------------------------------------------------------------------------------------------------------
+template <typename T, int MODE>
+__global__ void __launch_bounds__(128) k_update_H(const StepParams<T> p) {
+  constexpr int V = VecOf<T>::V;
+  const int i0 = (blockIdx.x * blockDim.x + threadIdx.x) * V;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z;
+  if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && threadIdx.x == 0 && threadIdx.y == 0) *p.nstep += 1;
+  if (i0 >= p.nx || j >= p.ny) return;
+  const long long o = i0 + (long long)p.P * j + p.PS * k;
+
+  T ex[V], ey[V], ez[V], exk[V], eyk[V], exj[V], ezj[V], hx[V], hy[V], hz[V];
+  ldv(p.src[kEx] + o, ex); ldv(p.src[kEy] + o, ey); ldv(p.src[kEz] + o, ez);
+  ldv(p.src[kEx] + o + p.PS, exk); ldv(p.src[kEy] + o + p.PS, eyk);
+  ldv(p.src[kEx] + o + p.P, exj);  ldv(p.src[kEz] + o + p.P, ezj);
+  const T eyi = p.src[kEy][o + V], ezi = p.src[kEz][o + V];
+  ldv(p.src[kHx] + o, hx); ldv(p.src[kHy] + o, hy); ldv(p.src[kHz] + o, hz);
+
+  const int sj = slab_coord(j, p.lo[1], p.hi[1], p.ny);
+  const int sk = slab_coord(k, p.lo[2], p.hi[2], p.nz);
+  const bool xs = (i0 < p.lo[0]) || (i0 + V > p.nx - p.hi[0]);
+
+  T ax[V], ay[V], az[V];          // curl accumulators
+  T d0[V], d1[V], d2[V], d3[V];  // raw derivatives kept for the y / z slab psi updates
+  {
+    const T iky = sj >= 0 ? p.kH[1][sj] : T(1), ikz = sk >= 0 ? p.kH[2][sk] : T(1);
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      const T eyp = (v + 1 < V) ? ey[v + 1] : eyi;
+      const T ezp = (v + 1 < V) ? ez[v + 1] : ezi;
+      const T dyEz = (ezj[v] - ez[v]) * p.idy_, dzEy = (eyk[v] - ey[v]) * p.idz_;
+      const T dzEx = (exk[v] - ex[v]) * p.idz_, dxEz = (ezp - ez[v]) * p.idx_;
+      const T dxEy = (eyp - ey[v]) * p.idx_,    dyEx = (exj[v] - ex[v]) * p.idy_;
+      ax[v] = dyEz * iky - dzEy * ikz;
+      ay[v] = dzEx * ikz;
+      az[v] = -dyEx * iky;
+      // x terms need the per-cell kappa: done in the x-slab branch or here with kappa = 1
+      if (!xs) { ay[v] -= dxEz; az[v] += dxEy; }
+      else {
+        const int si = slab_coord(i0 + v, p.lo[0], p.hi[0], p.nx);
+        T ikx = T(1);
+        T pyx = T(0), pzx = T(0);
+        if (si >= 0 && i0 + v < p.nx) {
+          ikx = p.kH[0][si];
+          const long long q = si + (long long)(p.lo[0] + p.hi[0]) * (j + (long long)p.ny * k);
+          const T b = p.bH[0][si], c = p.cH[0][si];
+          pyx = b * p.psi[pHyx][q] + c * dxEz; p.psi[pHyx][q] = pyx;
+          pzx = b * p.psi[pHzx][q] + c * dxEy; p.psi[pHzx][q] = pzx;
+        }
+        ay[v] -= dxEz * ikx + pyx;
+        az[v] += dxEy * ikx + pzx;
+      }
+      d0[v] = dyEz; d1[v] = dyEx; d2[v] = dzEy; d3[v] = dzEx;
+    }
+  }
+  if (sj >= 0) {  // y slab: psiHxy (from D+y Ez), psiHzy (from D+y Ex)
+    const long long q = i0 + (long long)p.P * (sj + (long long)(p.lo[1] + p.hi[1]) * k);
+    const T b = p.bH[1][sj], c = p.cH[1][sj];
+    T a[V], d[V];
+    ldv(p.psi[pHxy] + q, a); ldv(p.psi[pHzy] + q, d);
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      a[v] = b * a[v] + c * d0[v]; d[v] = b * d[v] + c * d1[v];
+      if (i0 + v >= p.nx) { a[v] = T(0); d[v] = T(0); }
+      ax[v] += a[v]; az[v] -= d[v];
+    }
+    stv(p.psi[pHxy] + q, a); stv(p.psi[pHzy] + q, d);
+  }
+  if (sk >= 0) {  // z slab: psiHxz (from D+z Ey), psiHyz (from D+z Ex)
+    const long long q = i0 + (long long)p.P * (j + (long long)p.ny * sk);
+    const T b = p.bH[2][sk], c = p.cH[2][sk];
+    T a[V], d[V];
+    ldv(p.psi[pHxz] + q, a); ldv(p.psi[pHyz] + q, d);
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      a[v] = b * a[v] + c * d2[v]; d[v] = b * d[v] + c * d3[v];
+      if (i0 + v >= p.nx) { a[v] = T(0); d[v] = T(0); }
+      ax[v] -= a[v]; ay[v] += d[v];
+    }
+    stv(p.psi[pHxz] + q, a); stv(p.psi[pHyz] + q, d);
+  }
+  // Db: uniform dt/mu0, or per entry / per cell when permeability was given
+  T dbx[V], dby[V], dbz[V];
+  if (MODE & kModeMu) {
+    if (MODE & kModeFull) { ldv(p.Db[0] + o, dbx); ldv(p.Db[1] + o, dby); ldv(p.Db[2] + o, dbz); }
+    else {
+#pragma unroll
+      for (int v = 0; v < V; ++v) {
+        const int m = p.idx[o + v];
+        dbx[v] = p.tab[6 * kMaxTable + m]; dby[v] = p.tab[7 * kMaxTable + m]; dbz[v] = p.tab[8 * kMaxTable + m];
+      }
+    }
+  } else {
+#pragma unroll
+    for (int v = 0; v < V; ++v) { dbx[v] = p.db0; dby[v] = p.db0; dbz[v] = p.db0; }
+  }
+#pragma unroll
+  for (int v = 0; v < V; ++v) {
+    hx[v] -= dbx[v] * ax[v]; hy[v] -= dby[v] * ay[v]; hz[v] -= dbz[v] * az[v];
+    if (i0 + v >= p.nx) { hx[v] = T(0); hy[v] = T(0); hz[v] = T(0); }
+  }
+  stv(p.dst[kHx] + o, hx); stv(p.dst[kHy] + o, hy); stv(p.dst[kHz] + o, hz);
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// E pass.  R5 step 2:  psiE = bE psiE + cE D-H ;  Ex = Cax Ex + Cbx (D-y Hz / kEy + psiExy - D-z Hy / kEz - psiExz) ...
+// then the low-face wall rows are forced to zero (PEC walls; PAPER.md:46 for the ground).
+// ------------------------------------------------------------------------------------------------------------------
+template <typename T, int MODE>
+__global__ void __launch_bounds__(128) k_update_E(const StepParams<T> p) {
+  constexpr int V = VecOf<T>::V;
+  const int i0 = (blockIdx.x * blockDim.x + threadIdx.x) * V;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z;
+  if (i0 >= p.nx || j >= p.ny) return;
+  const long long o = i0 + (long long)p.P * j + p.PS * k;
+
+  T hx[V], hy[V], hz[V], hxk[V], hyk[V], hxj[V], hzj[V], ex[V], ey[V], ez[V];
+  ldv(p.src[kHx] + o, hx); ldv(p.src[kHy] + o, hy); ldv(p.src[kHz] + o, hz);
+  ldv(p.src[kHx] + o - p.PS, hxk); ldv(p.src[kHy] + o - p.PS, hyk);
+  ldv(p.src[kHx] + o - p.P, hxj);  ldv(p.src[kHz] + o - p.P, hzj);
+  const T hyi = p.src[kHy][o - 1], hzi = p.src[kHz][o - 1];
+  ldv(p.src[kEx] + o, ex); ldv(p.src[kEy] + o, ey); ldv(p.src[kEz] + o, ez);
+
+  const int sj = slab_coord(j, p.lo[1], p.hi[1], p.ny);
+  const int sk = slab_coord(k, p.lo[2], p.hi[2], p.nz);
+  const bool xs = (i0 < p.lo[0]) || (i0 + V > p.nx - p.hi[0]);
+
+  T ax[V], ay[V], az[V];
+  T d0[V], d1[V], d2[V], d3[V];  // raw derivatives kept for the y / z slab psi updates
+  {
+    const T iky = sj >= 0 ? p.kE[1][sj] : T(1), ikz = sk >= 0 ? p.kE[2][sk] : T(1);
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      const T hym = (v > 0) ? hy[v - 1] : hyi;
+      const T hzm = (v > 0) ? hz[v - 1] : hzi;
+      const T dyHz = (hz[v] - hzj[v]) * p.idy_, dzHy = (hy[v] - hyk[v]) * p.idz_;
+      const T dzHx = (hx[v] - hxk[v]) * p.idz_, dxHz = (hz[v] - hzm) * p.idx_;
+      const T dxHy = (hy[v] - hym) * p.idx_,    dyHx = (hx[v] - hxj[v]) * p.idy_;
+      ax[v] = dyHz * iky - dzHy * ikz;
+      ay[v] = dzHx * ikz;
+      az[v] = -dyHx * iky;
+      if (!xs) { ay[v] -= dxHz; az[v] += dxHy; }
+      else {
+        const int si = slab_coord(i0 + v, p.lo[0], p.hi[0], p.nx);
+        T ikx = T(1), pyx = T(0), pzx = T(0);
+        if (si >= 0 && i0 + v < p.nx) {
+          ikx = p.kE[0][si];
+          const long long q = si + (long long)(p.lo[0] + p.hi[0]) * (j + (long long)p.ny * k);
+          const T b = p.bE[0][si], c = p.cE[0][si];
+          pyx = b * p.psi[pEyx][q] + c * dxHz; p.psi[pEyx][q] = pyx;
+          pzx = b * p.psi[pEzx][q] + c * dxHy; p.psi[pEzx][q] = pzx;
+        }
+        ay[v] -= dxHz * ikx + pyx;
+        az[v] += dxHy * ikx + pzx;
+      }
+      d0[v] = dyHz; d1[v] = dyHx; d2[v] = dzHy; d3[v] = dzHx;
+    }
+  }
+  if (sj >= 0) {  // y slab: psiExy (from D-y Hz), psiEzy (from D-y Hx)
+    const long long q = i0 + (long long)p.P * (sj + (long long)(p.lo[1] + p.hi[1]) * k);
+    const T b = p.bE[1][sj], c = p.cE[1][sj];
+    T a[V], d[V];
+    ldv(p.psi[pExy] + q, a); ldv(p.psi[pEzy] + q, d);
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      a[v] = b * a[v] + c * d0[v]; d[v] = b * d[v] + c * d1[v];
+      if (i0 + v >= p.nx) { a[v] = T(0); d[v] = T(0); }
+      ax[v] += a[v]; az[v] -= d[v];
+    }
+    stv(p.psi[pExy] + q, a); stv(p.psi[pEzy] + q, d);
+  }
+  if (sk >= 0) {  // z slab: psiExz (from D-z Hy), psiEyz (from D-z Hx)
+    const long long q = i0 + (long long)p.P * (j + (long long)p.ny * sk);
+    const T b = p.bE[2][sk], c = p.cE[2][sk];
+    T a[V], d[V];
+    ldv(p.psi[pExz] + q, a); ldv(p.psi[pEyz] + q, d);
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      a[v] = b * a[v] + c * d2[v]; d[v] = b * d[v] + c * d3[v];
+      if (i0 + v >= p.nx) { a[v] = T(0); d[v] = T(0); }
+      ax[v] -= a[v]; ay[v] += d[v];
+    }
+    stv(p.psi[pExz] + q, a); stv(p.psi[pEyz] + q, d);
+  }
+  T cax[V], cay[V], caz[V], cbx[V], cby[V], cbz[V];
+  if (MODE & kModeFull) {
+    ldv(p.Ca[0] + o, cax); ldv(p.Ca[1] + o, cay); ldv(p.Ca[2] + o, caz);
+    ldv(p.Cb[0] + o, cbx); ldv(p.Cb[1] + o, cby); ldv(p.Cb[2] + o, cbz);
+  } else {
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      const int m = p.idx[o + v];
+      cax[v] = p.tab[0 * kMaxTable + m]; cay[v] = p.tab[1 * kMaxTable + m]; caz[v] = p.tab[2 * kMaxTable + m];
+      cbx[v] = p.tab[3 * kMaxTable + m]; cby[v] = p.tab[4 * kMaxTable + m]; cbz[v] = p.tab[5 * kMaxTable + m];
+    }
+  }
+  const bool wj = (j == 0), wk = (k == 0);
+#pragma unroll
+  for (int v = 0; v < V; ++v) {
+    const bool wi = (i0 + v == 0), pad = (i0 + v >= p.nx);
+    ex[v] = cax[v] * ex[v] + cbx[v] * ax[v];
+    ey[v] = cay[v] * ey[v] + cby[v] * ay[v];
+    ez[v] = caz[v] * ez[v] + cbz[v] * az[v];
+    if (wj || wk || pad) ex[v] = T(0);
+    if (wi || wk || pad) ey[v] = T(0);
+    if (wi || wj || pad) ez[v] = T(0);
+  }
+  stv(p.dst[kEx] + o, ex); stv(p.dst[kEy] + o, ey); stv(p.dst[kEz] + o, ez);
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// Port work.  The device step counter was already incremented by the first kernel of the step.
+// ------------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double waveform_dev(int kind, double t, double t0, double sigma, double f0) {
+  const double u = (t - t0) / sigma;
+  switch (kind) {
+    case 0: return -2.0 * u * exp(-u * u);                                   // Eq. 3
+    case 1: return exp(-u * u);
+    case 2: return sin(2.0 * 3.14159265358979323846 * f0 * (t - t0)) * exp(-u * u);
+  }
+  return 0.0;
+}
+
+// one block; ports in order so that overlapping source boxes add up deterministically
+template <typename T>
+__global__ void __launch_bounds__(256) k_source(const PortParams<T> p) {
+  const double t = (double)(*p.nstep) * p.dt;
+  for (int n = 0; n < p.nports; ++n) {
+    const PortDev q = p.ports[n];
+    if (!q.has_source) continue;
+    const T g = (T)(q.amp * waveform_dev(q.waveform, t, q.t0, q.sigma, q.f0));
+    const int nj = q.sj1 - q.sj0 + 1, ns = nj * (q.sk1 - q.sk0);
+    for (int s = threadIdx.x; s < ns; s += blockDim.x) {
+      const int j = q.sj0 + s % nj, k = q.sk0 + s / nj;
+      p.Ez[q.is + (long long)p.P * j + p.PS * k] += g;
+    }
+    __syncthreads();
+  }
+}
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int s = 16; s > 0; s >>= 1) v += __shfl_xor_sync(0xffffffffu, v, s);
+  return v;
+}
+
+// grid (nports, max(1, ceil(nf/64))), 128 threads.  Every block reduces V and I of its port (warp-shuffle partial
+// sums in fp64), then thread t accumulates frequency chunk*64 + t%64 of V (t < 64) or I (t >= 64).
+template <typename T>
+__global__ void __launch_bounds__(128) k_probe_dft(const PortParams<T> p) {
+  __shared__ double sh[2][4];
+  const PortDev q = p.ports[blockIdx.x];
+  const int nj = q.vj1 - q.vj0 + 1, nv = nj * (q.vk1 - q.vk0);
+  double sv = 0.0;
+  for (int s = threadIdx.x; s < nv; s += blockDim.x) {
+    const int j = q.vj0 + s % nj, k = q.vk0 + s / nj;
+    sv += (double)p.Ez[q.ip + (long long)p.P * j + p.PS * k];
+  }
+  // I = dz * sum_k (Hz[lj1,k] - Hz[lj0-1,k]) - dy * sum_j (Hy[j,lk1] - Hy[j,lk0-1])
+  const int nkl = q.lk1 - q.lk0 + 1, njl = q.lj1 - q.lj0 + 1;
+  double si = 0.0;
+  for (int s = threadIdx.x; s < nkl + njl; s += blockDim.x) {
+    if (s < nkl) {
+      const int k = q.lk0 + s;
+      si += p.dz * ((double)p.Hz[q.ip + (long long)p.P * q.lj1 + p.PS * k] -
+                    (double)p.Hz[q.ip + (long long)p.P * (q.lj0 - 1) + p.PS * k]);
+    } else {
+      const int j = q.lj0 + (s - nkl);
+      si -= p.dy * ((double)p.Hy[q.ip + (long long)p.P * j + p.PS * q.lk1] -
+                    (double)p.Hy[q.ip + (long long)p.P * j + p.PS * (q.lk0 - 1)]);
+    }
+  }
+  sv = warp_sum(sv); si = warp_sum(si);
+  const int w = threadIdx.x >> 5;
+  if ((threadIdx.x & 31) == 0) { sh[0][w] = sv; sh[1][w] = si; }
+  __syncthreads();
+  const double V = p.dz / (double)nj * (sh[0][0] + sh[0][1] + sh[0][2] + sh[0][3]);
+  const double I = sh[1][0] + sh[1][1] + sh[1][2] + sh[1][3];
+  if (blockIdx.y == 0 && threadIdx.x == 0) { p.lastV[blockIdx.x] = V; p.lastI[blockIdx.x] = I; }
+  const int m = blockIdx.y * 64 + (threadIdx.x & 63);
+  if (m < p.nf) {
+    const bool isI = threadIdx.x >= 64;
+    const double n = (double)(*p.nstep);
+    const double t = (isI ? n - 0.5 : n) * p.dt;
+    double s, c;
+    sincos(2.0 * 3.14159265358979323846 * p.freqs[m] * t, &s, &c);
+    const double a = (isI ? I : V) * p.dt;
+    double* acc = (isI ? p.dftI : p.dftV) + ((long long)blockIdx.x * p.nf + m) * 2;
+    acc[0] += a * c;
+    acc[1] -= a * s;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// Setup kernels (not on the timed path).
+// ------------------------------------------------------------------------------------------------------------------
+// full mode: arrays hold eps_r (in ca) and sigma (in cb) on entry, Ca and Cb on exit (R3)
+template <typename T>
+__global__ void k_coef_E(T* ca, T* cb, long long n, double dt, double eps0) {
+  const long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (q >= n) return;
+  const double er = (double)ca[q], sg = (double)cb[q];
+  if (er == 0.0) { ca[q] = T(0); cb[q] = T(0); return; }  // halo / pad cells: keep them inert
+  if (isinf(sg)) { ca[q] = T(0); cb[q] = T(0); return; }
+  const double a = sg * dt / (2.0 * eps0 * er);
+  ca[q] = (T)((1.0 - a) / (1.0 + a));
+  cb[q] = (T)((dt / (eps0 * er)) / (1.0 + a));
+}
+template <typename T>
+__global__ void k_coef_H(T* db, long long n, double dt, double mu0) {
+  const long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (q >= n) return;
+  const double mr = (double)db[q];
+  db[q] = mr == 0.0 ? T(0) : (T)(dt / (mu0 * mr));
+}
+template <typename T>
+__global__ void k_fill(T* a, long long n, T v) {
+  const long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (q < n) a[q] = v;
+}
+
+}  // namespace fdtd_b200

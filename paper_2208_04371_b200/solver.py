@@ -1,0 +1,146 @@
+"""`Solver`: a handle plus its torch workspace -- a convenience wrapper over the C-ABI functions of binding.py.
+
+Nothing here computes: setup arguments are marshalled to the library, the workspace is one torch uint8 CUDA tensor,
+the stream is torch's current stream.  Fields come back as torch CUDA tensors shaped [nz, ny, nx] (x fastest).
+"""
+from __future__ import annotations
+
+import numpy as np
+
+from . import binding as B
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_2208_04371_b200 needs a CUDA device: there is no CPU fallback")
+    return torch
+
+
+class Solver:
+    def __init__(self, nx, ny, nz, dx, dy, dz, dt, precision=B.FDTD_F32):
+        self.h = B.fdtd_create(nx, ny, nz, dx, dy, dz, dt, precision)
+        self.shape = (nz, ny, nx)
+        self.precision = precision
+        self.nf = 0
+        self.nports = 0
+        self.workspace = None
+
+    # ---- setup (before commit) ---------------------------------------------------------------------------------
+    def set_boundary(self, pml_cells, cpml=None):
+        B.fdtd_set_boundary(self.h, pml_cells, cpml)
+
+    def set_material_mode(self, mode, has_mu=False):
+        B.fdtd_set_material_mode(self.h, mode, has_mu)
+
+    def add_port(self, port: dict) -> int:
+        pid = B.fdtd_add_port(self.h, port)
+        self.nports = pid + 1
+        return pid
+
+    def set_dft(self, freqs_hz):
+        self.nf = int(np.asarray(freqs_hz).size)
+        B.fdtd_set_dft(self.h, freqs_hz)
+
+    def set_option(self, option, value):
+        B.fdtd_set_option(self.h, option, value)
+
+    def workspace_bytes(self):
+        return B.fdtd_workspace_bytes(self.h)
+
+    def commit(self, device="cuda:0"):
+        torch = _torch()
+        self.device = torch.device(device)
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(self.workspace_bytes(), dtype=torch.uint8, device=self.device)
+            self.stream = torch.cuda.current_stream(self.device)
+            B.fdtd_commit(self.h, self.workspace, self.stream.cuda_stream)
+
+    # ---- after commit ------------------------------------------------------------------------------------------
+    def set_materials_indexed(self, idx, eps_r, sigma, mu_r=None):
+        B.fdtd_set_materials_indexed(self.h, idx, eps_r, sigma, mu_r)
+
+    def set_materials_full(self, eps_r, sigma, mu_r=None):
+        B.fdtd_set_materials_full(self.h, eps_r, sigma, mu_r)
+
+    def step(self, n=1):
+        B.fdtd_step(self.h, n)
+
+    @property
+    def dtype(self):
+        torch = _torch()
+        return torch.float64 if self.precision == B.FDTD_F64 else torch.float32
+
+    def read_fields(self, comp, out=None):
+        if out is None:
+            out = _torch().empty(self.shape, dtype=self.dtype, device=self.device)
+        B.fdtd_read_fields(self.h, comp, out)
+        return out
+
+    def write_fields(self, comp, src):
+        B.fdtd_write_fields(self.h, comp, src)
+
+    def read_port_dft(self, port):
+        return B.fdtd_read_port_dft(self.h, port, self.nf)
+
+    def read_port_last(self, port):
+        return B.fdtd_read_port_last(self.h, port)
+
+    def reset(self):
+        B.fdtd_reset(self.h)
+
+    @property
+    def step_count(self):
+        return B.fdtd_step_count(self.h)
+
+    @property
+    def launch_count(self):
+        return B.fdtd_launch_count(self.h)
+
+    @property
+    def impl_name(self):
+        return B.fdtd_impl_name(self.h)
+
+    def synchronize(self):
+        self.stream.synchronize()
+
+    def destroy(self):
+        if getattr(self, "h", None):
+            B.fdtd_destroy(self.h)
+            self.h = None
+            self.workspace = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    # ---- a workload dict (workloads/__init__.py) -> a committed solver ------------------------------------------
+    @classmethod
+    def from_workload(cls, w: dict, precision=None, options=None, device="cuda:0", materials_on_device=False):
+        prec = precision if precision is not None else w["precision"]
+        s = cls(w["nx"], w["ny"], w["nz"], w["dx"], w["dy"], w["dz"], w["dt"], prec)
+        if w.get("periodic_y"):
+            raise ValueError("periodic-y is an oracle-only option")
+        s.set_boundary(w["pml"], w.get("cpml"))
+        m = w["materials"]
+        has_mu = m.get("mu_r") is not None
+        s.set_material_mode(B.FDTD_MAT_INDEXED if m["mode"] == "indexed" else B.FDTD_MAT_FULL, has_mu)
+        for p in w.get("ports", []):
+            s.add_port(p)
+        if len(w.get("freqs", [])):
+            s.set_dft(w["freqs"])
+        for k, v in (options or {}).items():
+            s.set_option(k, v)
+        s.commit(device)
+        np_dt = np.float64 if prec == B.FDTD_F64 else np.float32
+        if m["mode"] == "indexed":
+            idx = np.ascontiguousarray(m["idx"], dtype=np.uint8)
+            if materials_on_device:
+                idx = _torch().from_numpy(idx).to(s.device)
+            s.set_materials_indexed(idx, m["eps_r"], m["sigma"], m.get("mu_r"))
+        else:
+            conv = lambda xs: None if xs is None else [np.ascontiguousarray(x, dtype=np_dt) for x in xs]
+            s.set_materials_full(conv(m["eps_r"]), conv(m["sigma"]), conv(m.get("mu_r")))
+        return s

@@ -1,0 +1,228 @@
+"""Parity of the CUDA path (through the C ABI) with the fp64 CPU oracle, element by element, on seeded inputs.
+
+All tests need a B200: `pytest -m gpu`.  Sizes are chosen so that the oracle finishes in seconds while the grid
+still spans several thread blocks / tiles and a ragged tail in every axis.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import workloads as W
+from oracle import sparams as osp
+from oracle.yee import YeeOracle
+from paper_2208_04371_b200 import (FDTD_F32, FDTD_F64, FDTD_OPT_GRAPH_UNROLL, FDTD_OPT_STEP_IMPL, FDTD_OPT_USE_GRAPH,
+                                   FdtdError, Solver, sparams)
+
+from .parity_util import TOL, assert_fields, run_pair
+
+pytestmark = pytest.mark.gpu
+
+IMPLS = [1]  # FDTD_OPT_STEP_IMPL: 1 = two-pass kernels (2 = fused E+H kernel, added when it lands)
+
+
+@pytest.mark.parametrize("impl", IMPLS)
+@pytest.mark.parametrize("seed,indexed,with_mu,pml", [
+    (1, True, True, (3, 4, 2, 3, 0, 3)),
+    (2, False, False, (0, 3, 3, 0, 2, 2)),
+    (3, True, False, (2, 2, 2, 2, 2, 2)),
+    (4, False, True, (0, 0, 0, 0, 0, 0)),
+])
+@pytest.mark.parametrize("prec", [FDTD_F64, FDTD_F32])
+def test_random_box_every_term(seed, indexed, with_mu, pml, prec, impl):
+    """Random eps / sigma / mu blocks, PEC cells, kappa != 1, alpha != 0, mixed CPML faces, driven + passive port."""
+    w = W.random_box(seed, indexed=indexed, with_mu=with_mu, pml=pml, steps=60, precision=prec)
+    o, s, rep = run_pair(w, 60, precision=prec, options={FDTD_OPT_STEP_IMPL: impl}, checkpoints=[1, 2, 17, 60])
+    assert_fields(rep, prec)
+    dv, di = rep["dft_err"]
+    assert max(dv, di) <= (1e-11 if prec == FDTD_F64 else 1e-4)
+    for p in range(2):
+        vo, io = o.read_port_last(p)
+        vg, ig = s.read_port_last(p)
+        assert vg == pytest.approx(vo, rel=1e-3 if prec == FDTD_F32 else 1e-9, abs=1e-30 + 1e-5 * abs(vo))
+        assert ig == pytest.approx(io, rel=1e-3 if prec == FDTD_F32 else 1e-9, abs=1e-30 + 1e-5 * abs(io))
+
+
+@pytest.mark.parametrize("impl", IMPLS)
+@pytest.mark.parametrize("shape", [(21, 14, 12), (37, 5, 9), (130, 19, 7), (2, 2, 2), (5, 3, 2), (259, 34, 21)])
+@pytest.mark.parametrize("prec", [FDTD_F64, FDTD_F32])
+def test_ragged_shapes(shape, prec, impl):
+    """nx not a multiple of the vector width, tiny grids, several blocks in x with a tail."""
+    nx, ny, nz = shape
+    pml = tuple(min(3, n // 3) for n in (nx, nx, ny, ny, nz, nz))
+    if min(shape) < 6:
+        # too small for the generator's port boxes: a bare box with random initial fields instead
+        d = (5e-9, 4e-9, 6e-9)
+        dt = 0.95 * W.cfl_limit(*d)
+        r = W.rng_for(100 + nx)
+        one = np.ones((nz, ny, nx))
+        w = dict(name="tiny", nx=nx, ny=ny, nz=nz, dx=d[0], dy=d[1], dz=d[2], dt=dt, precision=prec, pml=[0] * 6,
+                 cpml=None, materials={"mode": "full", "eps_r": [one * 2.0] * 3, "sigma": [one * 1e3] * 3, "mu_r": None},
+                 ports=[], freqs=np.zeros(0), steps=30)
+        init = [r.standard_normal((nz, ny, nx)) * (1.0 if c < 3 else 1e-3) for c in range(6)]
+        # low-face tangential E is zero by construction (R1)
+        init[0][:, 0, :] = 0; init[0][0] = 0
+        init[1][:, :, 0] = 0; init[1][0] = 0
+        init[2][:, :, 0] = 0; init[2][:, 0, :] = 0
+        o, s, rep = run_pair(w, 30, precision=prec, options={FDTD_OPT_STEP_IMPL: impl}, init_fields=init)
+    else:
+        w = W.random_box(7, nx=nx, ny=ny, nz=nz, pml=pml, steps=50, precision=prec)
+        o, s, rep = run_pair(w, 50, precision=prec, options={FDTD_OPT_STEP_IMPL: impl}, checkpoints=[3, 50])
+    assert_fields(rep, prec)
+
+
+@pytest.mark.parametrize("impl", IMPLS)
+def test_P2_exact_discrete_eigenmode_on_gpu(impl):
+    """The pin P2 of the oracle, applied to the CUDA path directly (closed form, no oracle in the comparison)."""
+    nx, ny, nz = 24, 10, 14
+    dx, dy, dz = 5e-9, 4e-9, 6e-9
+    dt = 0.9 * W.cfl_limit(dx, dy, dz)
+    c0, mu0 = 299792458.0, 4e-7 * math.pi
+    m = (1, 2, 1)
+    kk = [m[a] * math.pi / (n * d) for a, (n, d) in enumerate([(nx, dx), (ny, dy), (nz, dz)])]
+    K = np.array([2 / d * math.sin(k * d / 2) for k, d in zip(kk, (dx, dy, dz))])
+    A = np.cross(K, [0.3, -1.0, 0.7])
+    k_, j_, i_ = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    kx, ky, kz = kk
+    Ex = A[0] * np.cos(kx * (i_ + .5) * dx) * np.sin(ky * j_ * dy) * np.sin(kz * k_ * dz)
+    Ey = A[1] * np.sin(kx * i_ * dx) * np.cos(ky * (j_ + .5) * dy) * np.sin(kz * k_ * dz)
+    Ez = A[2] * np.sin(kx * i_ * dx) * np.sin(ky * j_ * dy) * np.cos(kz * (k_ + .5) * dz)
+    cu = np.cross(K, A)
+    Hx = cu[0] * np.sin(kx * i_ * dx) * np.cos(ky * (j_ + .5) * dy) * np.cos(kz * (k_ + .5) * dz)
+    Hy = cu[1] * np.cos(kx * (i_ + .5) * dx) * np.sin(ky * j_ * dy) * np.cos(kz * (k_ + .5) * dz)
+    Hz = cu[2] * np.cos(kx * (i_ + .5) * dx) * np.cos(ky * (j_ + .5) * dy) * np.sin(kz * k_ * dz)
+    f = dt / (2 * mu0)
+    s = Solver(nx, ny, nz, dx, dy, dz, dt, FDTD_F64)
+    s.set_material_mode(1)
+    s.set_option(FDTD_OPT_STEP_IMPL, impl)
+    s.commit()
+    for c, a in enumerate([Ex, Ey, Ez, f * Hx, f * Hy, f * Hz]):
+        s.write_fields(c, np.ascontiguousarray(a))
+    wn = 2 / dt * math.asin(c0 * dt / 2 * np.linalg.norm(K))   # Yee dispersion relation
+    err = 0.0
+    for n in (1, 2, 50, 333):
+        s.step(n - s.step_count)
+        for c, a in enumerate([Ex, Ey, Ez]):
+            err = max(err, np.abs(s.read_fields(c).cpu().numpy() - a * math.cos(wn * n * dt)).max())
+    assert err / np.abs(A).max() < 1e-11
+
+
+@pytest.mark.parametrize("impl", IMPLS)
+def test_C0_cavity_full(impl):
+    """Config C0 as written: 32^3 fp64 PEC cavity, 2000 steps, fields <= 1e-11 of the running maximum."""
+    w = W.cavity_c0()
+    o, s, rep = run_pair(w, 2000, options={FDTD_OPT_STEP_IMPL: impl}, checkpoints=[100, 500, 1000, 2000])
+    assert_fields(rep, FDTD_F64)
+
+
+def _sstar(sim_inc, sim_tot, nports, module):
+    Vi, Ii, Vt = [], [], []
+    for p in range(nports):
+        v, i = sim_inc.read_port_dft(p)
+        Vi.append(v); Ii.append(i)
+        Vt.append(sim_tot.read_port_dft(p)[0])
+    return np.array(module.s_star_column(0, Vi, Ii, Vt))
+
+
+@pytest.mark.parametrize("impl", IMPLS)
+def test_C1_microstrip_fields_and_sparams(impl):
+    """Config C1 geometry at full size, first 1500 steps: fp32 fields, raw DFTs and S* (C1: tot == inc, R22)."""
+    w = W.microstrip_c1(steps=1500)
+    o, s, rep = run_pair(w, 1500, options={FDTD_OPT_STEP_IMPL: impl}, checkpoints=[100, 700, 1500])
+    assert_fields(rep, FDTD_F32)
+    So = _sstar(o, o, 2, osp)
+    Sg = _sstar(s, s, 2, sparams)
+    assert np.abs(So - Sg).max() <= 1e-3
+    assert np.abs(Sg[0]).max() == 0.0 and 0.5 < np.abs(Sg[1]).min()
+
+
+@pytest.mark.parametrize("impl", IMPLS)
+def test_C2_quarter_scale_inc_tot_sparams(impl):
+    """Config C2 at 1/4 linear scale (128x64x32), inc and tot runs, 1200 steps: fields and the S* column."""
+    sims = {}
+    for run in ("inc", "tot"):
+        w = W.interconnect_c2(run=run, div=4, steps=1200, npml=6, nf=32)
+        o, s, rep = run_pair(w, 1200, options={FDTD_OPT_STEP_IMPL: impl}, checkpoints=[300, 1200])
+        assert_fields(rep, FDTD_F32)
+        sims[run] = (o, s)
+    So = _sstar(sims["inc"][0], sims["tot"][0], 2, osp)
+    Sg = _sstar(sims["inc"][1], sims["tot"][1], 2, sparams)
+    assert np.abs(So - Sg).max() <= 1e-3
+
+
+@pytest.mark.parametrize("impl", IMPLS)
+def test_C4_eighth_scale_fp64_full_coefficients(impl):
+    """Config C4 at 1/8 linear scale (128x64x32), fp64, full anisotropic arrays, 4 ports: 1e-11."""
+    w = W.interconnect_c4(run="tot", div=8, steps=400, npml=5, nf=16)
+    o, s, rep = run_pair(w, 400, options={FDTD_OPT_STEP_IMPL: impl}, checkpoints=[50, 400])
+    assert_fields(rep, FDTD_F64)
+    assert max(rep["dft_err"]) <= 1e-11
+
+
+@pytest.mark.parametrize("impl", IMPLS)
+def test_C3_small_scale_indexed_six_face_cpml(impl):
+    """Config C3's generator at 1/8 linear scale (192x96x96): 64-entry table, six CPML faces, 4 ports, fp32."""
+    w = W.throughput_c3(div=8, steps=300, npml=6, nf=16)
+    o, s, rep = run_pair(w, 300, options={FDTD_OPT_STEP_IMPL: impl}, checkpoints=[20, 300])
+    assert_fields(rep, FDTD_F32)
+
+
+@pytest.mark.parametrize("impl", IMPLS)
+def test_graph_replay_equals_plain_launches(impl):
+    """fdtd_step(n) through CUDA-graph replay (unroll 4 + remainder) is bit-identical to one launch per step."""
+    w = W.random_box(11, nx=40, ny=22, nz=18, steps=27, precision=FDTD_F32)
+    out = []
+    for graph in (0, 1):
+        s = Solver.from_workload(w, options={FDTD_OPT_STEP_IMPL: impl, FDTD_OPT_USE_GRAPH: graph, FDTD_OPT_GRAPH_UNROLL: 4})
+        if graph:
+            s.step(27)
+        else:
+            for _ in range(27):
+                s.step(1)
+        assert s.step_count == 27
+        out.append([s.read_fields(c).cpu().numpy() for c in range(6)] + list(s.read_port_dft(0)))
+    for a, b in zip(*out):
+        assert np.array_equal(a, b)
+
+
+def test_reset_and_device_pointers():
+    """fdtd_reset zeroes the state; read/write accept device pointers; materials accept a device index array."""
+    import torch
+    w = W.random_box(12, steps=20, precision=FDTD_F32)
+    s = Solver.from_workload(w, materials_on_device=True)
+    s.step(20)
+    a = [s.read_fields(c).clone() for c in range(6)]
+    d0 = s.read_port_dft(0)
+    s.reset()
+    assert s.step_count == 0
+    assert all(float(s.read_fields(c).abs().max()) == 0.0 for c in range(6))
+    assert np.abs(s.read_port_dft(0)[0]).max() == 0.0
+    s.step(20)
+    for c in range(6):
+        assert torch.equal(a[c], s.read_fields(c))
+    assert np.array_equal(d0[0], s.read_port_dft(0)[0])
+    # write from a device tensor, read into a host array
+    s.write_fields(2, a[0])
+    host = np.empty(a[0].shape, dtype=np.float32)
+    s.read_fields(2, out=host)
+    assert np.array_equal(host, a[0].cpu().numpy())
+
+
+def test_error_codes_after_commit():
+    s = Solver(8, 8, 8, 1e-9, 1e-9, 1e-9, 1e-18, FDTD_F32)
+    s.set_boundary([2] * 6)
+    with pytest.raises(FdtdError) as e:
+        s.step(1)
+    assert e.value.code == -3   # FDTD_ESTATE
+    s.commit()
+    with pytest.raises(FdtdError) as e:
+        s.set_boundary([1] * 6)
+    assert e.value.code == -3
+    with pytest.raises(FdtdError) as e:
+        s.set_materials_full([np.ones(512, np.float32)] * 3, [np.zeros(512, np.float32)] * 3)
+    assert e.value.code == -3   # handle is in INDEXED mode
+    with pytest.raises(FdtdError) as e:
+        s.set_materials_indexed(np.zeros(512, np.uint8), [[1.0, 1.0, -2.0]], [[0.0, 0.0, 0.0]])
+    assert e.value.code == -1
+    s.step(3)
+    assert s.step_count == 3 and s.launch_count == 6
