@@ -1,0 +1,327 @@
+"""bench.py -- throughput of the Yee FDTD hot path on config C3 (BASELINE.json: "Mcell-updates/s per Yee E+H step").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload c3|c3s|c2|c4]
+
+One "step" is one full leapfrog step of the whole hot path (psi_H, H, psi_E, E, walls, source,
+probes, running DFT) over the whole grid.  One cell-update = all six components of one cell advanced one step (R27);
+N counts the CPML cells.  Prints ONE JSON line (rank 0).
+
+  value         N_cells * K * n_gpus / t   with inputs resident in HBM, t from CUDA events around fdtd_step(K) on the
+                solver's stream (barrier + synchronize on both sides, max over ranks)
+  e2e           the same job through the C ABI with HOST buffers inside the timed region: material index + table
+                host->device (fdtd_set_materials_indexed), fdtd_reset, K steps, every port's DFT device->host
+  roofline      dominant kernel: algorithmic bytes per launch / its average duration from CUDA events
+                (fdtd_profile_step) vs MEASURED_PEAKS.json hbm_gbs
+  cpu_baseline  the fp64 oracle, as it stands, on the host cores, on a bounded crop of the same workload (rank 0, N=1)
+  --impl reference   times the oracle instead (there is no installable reference implementation: /root/reference holds
+                a paper only); rank 0 alone works.
+
+Multi-GPU: the path does not shard in this build ("replicas only"): every rank runs an independent replica
+of the workload on its own GPU, no data-path collective; torch.distributed is used for the barrier and the max of the
+times only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "Mcell-updates/s per Yee E+H step"
+UNIT = "Mcell-updates/s"
+
+
+def workload(name, steps):
+    import workloads as W
+    if name == "c3":
+        return W.throughput_c3(steps=steps)
+    if name == "c3s":  # 1/4-scale C3 for quick checks of this script (not a bench line)
+        return W.throughput_c3(div=4, steps=steps, npml=16)
+    if name == "c2":
+        return W.interconnect_c2(steps=steps)
+    if name == "c4":
+        return W.interconnect_c4(steps=steps)
+    raise SystemExit(f"unknown workload {name}")
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, burst copy)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+# --------------------------------------------------------------------------------------------------------------------
+# clocks during the timed region (B200_PROFILING.md "clocks" line)
+# --------------------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    NAMES = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+
+    def __init__(self, device_index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        self.idx = device_index
+
+    def start(self):
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(self.idx), f"--query-gpu={self.Q}", "--format=csv,noheader",
+                                       "-lms", "100"], stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, smax, reasons, power = [], [], set(), []
+        for line in self.f.read().splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 9:
+                continue
+            try:
+                sm.append(float(c[1].split()[0]))
+                smax.append(float(c[2].split()[0]))
+                power.append(float(c[3].split()[0]))
+            except ValueError:
+                continue
+            for n, v in zip(self.NAMES, c[5:9]):
+                if v == "Active":
+                    reasons.add(n)
+        self.f.close()
+        os.unlink(self.f.name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(smax)), "reasons": sorted(reasons),
+                "samples": len(sm), "power_w_max": float(max(power))}
+
+
+# --------------------------------------------------------------------------------------------------------------------
+# the oracle on the host cores (cpu_baseline leg and --impl reference): bounded sample of the same workload
+# --------------------------------------------------------------------------------------------------------------------
+CPU_SAMPLE_LADDER = [(512, 384, 192), (384, 256, 160), (256, 192, 128), (192, 128, 96), (128, 96, 80)]
+
+
+def _oracle_on(shape):
+    import workloads as W
+    from oracle.yee import YeeOracle
+    nb = max(1, int(4096 * (shape[0] * shape[1] * shape[2]) / (1536 * 768 * 768)))   # same block density as C3
+    w = W.throughput_c3(shape=shape, steps=1, nblocks=nb)
+    return YeeOracle.from_workload(w), w["nx"] * w["ny"] * w["nz"]
+
+
+def oracle_sample(budget_s=15.0, steps=None, warmup=1, wall_s=150.0):
+    """Time the fp64 oracle as it stands on a bounded crop of C3.  With steps=None the step count fills budget_s on
+    the largest crop; with steps given (the --impl reference arm) the crop is the largest of CPU_SAMPLE_LADDER whose
+    steps+warmup steps are expected to fit in wall_s.  Returns (Mcell/s, s/step, steps, cores, description, shape)."""
+    from oracle.yee import num_threads
+    shape = CPU_SAMPLE_LADDER[0]
+    if steps is not None:
+        o, n = _oracle_on(CPU_SAMPLE_LADDER[-1])
+        o.step(1)
+        t = time.perf_counter()
+        o.step(2)
+        rate = 2 * n / (time.perf_counter() - t)            # cells/s estimate
+        del o
+        for shape in CPU_SAMPLE_LADDER:
+            if shape[0] * shape[1] * shape[2] * (steps + warmup) / rate <= wall_s:
+                break
+    o, n = _oracle_on(shape)
+    t = time.perf_counter()
+    o.step(max(1, warmup))
+    t1 = (time.perf_counter() - t) / max(1, warmup)
+    if steps is None:
+        steps = int(min(200, max(2, budget_s / t1)))
+    t = time.perf_counter()
+    o.step(steps)
+    el = time.perf_counter() - t
+    desc = (f"fp64 oracle (g++ -O2 -fopenmp), C3 generator cropped to {shape[0]}x{shape[1]}x{shape[2]} cells "
+            f"(64-entry indexed materials, 16-cell six-face CPML, 4 ports, 128-frequency DFT), {steps} steps")
+    return n * steps / el / 1e6, el / steps, steps, num_threads(), desc, shape
+
+
+def run_reference(args, rank):
+    if rank != 0:
+        return
+    # each "step" of this arm = one oracle step on the bounded crop; K steps after W warm-up steps
+    v, sps, k, cores, desc, shape = oracle_sample(steps=args.steps, warmup=args.warmup)
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": k,
+            "warmup": args.warmup, "ms_per_step": sps * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "c3 (bounded crop, CPU oracle)", "grid": list(shape)},
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0,
+            "note": "no installable reference exists (/root/reference is a paper); this arm is the CPU oracle"}
+    print(json.dumps(line), flush=True)
+
+
+# --------------------------------------------------------------------------------------------------------------------
+# algorithmic bytes per cell-update of the dominant kernel
+# --------------------------------------------------------------------------------------------------------------------
+def algorithmic_bytes(w, impl, kernel):
+    """Bytes one launch of `kernel` must move, from the per-cell figures of SURVEY 8(d) / DESIGN.md:
+    field words read and written once + the material operand + psi read+write on the slab cells."""
+    n = w["nx"] * w["ny"] * w["nz"]
+    es = 4 if w["precision"] == 32 else 8
+    full = w["materials"]["mode"] == "full"
+    mu = w["materials"].get("mu_r") is not None
+    lo_hi = w["pml"]
+    dims = (w["nx"], w["ny"], w["nz"])
+    slab = sum((lo_hi[2 * a] + lo_hi[2 * a + 1]) * n // dims[a] for a in range(3))   # slab cells summed over axes
+    psi_half = 2 * 2 * es * slab                     # two psi per slab-cell-axis per half step, read + write
+    h_bytes = n * (6 * es + 3 * es + ((3 * es if full else 1) if mu else 0)) + psi_half
+    e_bytes = n * (6 * es + 3 * es + (6 * es if full else 1)) + psi_half
+    if impl == "fused":
+        return n * (6 * es + 6 * es + (6 * es if full else 1) + ((3 * es if full else 0) if mu else 0)) + 2 * psi_half
+    return h_bytes if kernel == "H" else e_bytes
+
+
+# --------------------------------------------------------------------------------------------------------------------
+# our arm
+# --------------------------------------------------------------------------------------------------------------------
+def run_ours(args, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+
+    from paper_2208_04371_b200 import FDTD_OPT_STEP_IMPL, Solver, binding
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    K, Wm = args.steps, args.warmup
+    w = workload(args.workload, K)
+    n_cells = w["nx"] * w["ny"] * w["nz"]
+    opts = {FDTD_OPT_STEP_IMPL: args.step_impl} if args.step_impl else None
+    s = Solver.from_workload(w, options=opts, device=str(dev))
+    torch.cuda.synchronize(dev)
+
+    # ---- device-resident throughput: W warm-up steps, then exactly K timed steps -------------------------------------
+    s.step(Wm)
+    barrier()
+    clocks = ClockSampler(local_rank)
+    clocks.start()
+    l0 = s.launch_count
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(s.stream)
+    s.step(K)
+    e1.record(s.stream)
+    barrier()
+    ck = clocks.stop()
+    launches = s.launch_count - l0
+    t_ms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t_ms, op=dist.ReduceOp.MAX)
+    t_s = float(t_ms.item()) * 1e-3
+    value = n_cells * K * world / t_s / 1e6
+
+    # ---- per-kernel durations (CUDA events between the kernels, on the solver's stream) ------------------------------
+    ms = s.profile_step(max(3, min(20, K)))
+    impl = s.impl_name
+    if impl == "fused":
+        kname, kms = "k_step_fused", ms[0]
+    else:
+        kname, kms = ("k_update_E", ms[1]) if ms[1] >= ms[0] else ("k_update_H", ms[0])
+    ab = algorithmic_bytes(w, impl, "E" if kname == "k_update_E" else "H")
+    peak, peak_src = measured_peak()
+    achieved = ab / (kms * 1e-3) / 1e9
+    step_bytes = algorithmic_bytes(w, impl, "H") + (algorithmic_bytes(w, impl, "E") if impl != "fused" else 0)
+    roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": ab, "kernel_ms": kms,
+                "kernel_ms_all": {"H_or_fused": ms[0], "E": ms[1], "source": ms[2], "probe_dft": ms[3]},
+                "bytes_per_cell_update_step": step_bytes / n_cells,
+                "step_achieved_gbs": step_bytes * K / t_s / 1e9, "frac_of_8000": step_bytes * K / t_s / 1e9 / 8000.0}
+
+    # ---- end to end through the C ABI with host buffers ---------------------------------------------------------------
+    m = w["materials"]
+    e2e = None
+    if m["mode"] == "indexed":
+        idx_host = torch.from_numpy(np.ascontiguousarray(m["idx"], dtype=np.uint8)).pin_memory()
+        nports, nf = len(w["ports"]), len(w["freqs"])
+        barrier()
+        t0 = time.perf_counter()
+        s.set_materials_indexed(idx_host, m["eps_r"], m["sigma"], m.get("mu_r"))
+        s.reset()
+        s.step(K)
+        out = [s.read_port_dft(p) for p in range(nports)]          # device -> host, synchronises
+        torch.cuda.synchronize(dev)
+        te = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        h2d = idx_host.numel() + 9 * 256 * (4 if w["precision"] == 32 else 8)
+        d2h = nports * nf * 2 * 2 * 8
+        assert all(np.isfinite(v).all() and np.isfinite(i).all() for v, i in out)
+        e2e = {"value": n_cells * K * world / float(te.item()) / 1e6, "unit": UNIT,
+               "h2d_bytes_per_step": h2d / K, "d2h_bytes_per_step": d2h / K,
+               "what": "fdtd_set_materials_indexed(pinned host idx) + fdtd_reset + fdtd_step(K) + fdtd_read_port_dft x ports"}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+            "ms_per_step": t_s / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32" if w["precision"] == 32 else "f64", "data": "synthetic",
+            "config": {"workload": args.workload, "grid": [w["nx"], w["ny"], w["nz"]], "cells": n_cells,
+                       "materials": m["mode"], "cpml_cells": w["pml"], "ports": len(w["ports"]), "dft_freqs": len(w["freqs"]),
+                       "step_impl": impl, "l2": "inputs larger than L2 (no flush needed)" if n_cells * 24 > 2.6e8 else
+                       "grid fits in L2: launch-bound case, not a roofline case",
+                       "parallelism": "replicas only" if world > 1 else "1 GPU", "library": os.path.basename(binding.library_path())},
+            "clocks": ck, "e2e": e2e, "gpu_launches": launches, "roofline": roofline}
+    s.destroy()
+    del s
+    torch.cuda.empty_cache()
+    if rank == 0 and world == 1 and not args.no_cpu:
+        v, sps, k, cores, desc, _ = oracle_sample(budget_s=args.cpu_budget)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c3")
+    ap.add_argument("--step-impl", type=int, default=0, help="FDTD_OPT_STEP_IMPL: 0 auto, 1 two-pass, 2 fused")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--cpu-budget", type=float, default=15.0)
+    args = ap.parse_args()
+    args.warmup = max(3, args.warmup)
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+    run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

@@ -120,6 +120,12 @@ int fdtd_set_materials_full(fdtd_t*, const void* const eps_r[3], const void* con
 /* Enqueue n full time steps (R5: psi_H, H; psi_E, E, walls; source; probes; DFT) on the stream.  Does not synchronise. */
 int fdtd_step(fdtd_t*, long n);
 
+/* Run n full steps exactly like fdtd_step (plain launches, no graph) with CUDA events recorded on the stream between
+ * the kernels, and return the average device time per step, in milliseconds, of
+ *   ms_avg[0] = H pass (or the fused E+H kernel), ms_avg[1] = E pass (0 when fused), ms_avg[2] = source injection,
+ *   ms_avg[3] = probes + DFT.   This is the measurement hook of bench.py's roofline line.  Synchronises the stream. */
+int fdtd_profile_step(fdtd_t*, long n, double ms_avg[4]);
+
 /* Copy one field component (FDTD_EX..FDTD_HZ) to / from a caller array of N elements of the field precision, host or
  * device.  Stream-ordered; synchronises the stream before returning when the caller array is in host memory.
  * write_fields is the test hook for initial conditions and the resume path. */

@@ -54,6 +54,7 @@ SYMBOLS = {
     "fdtd_set_materials_indexed": (C.c_int, [_vp, _vp, C.c_int, _dp, _dp, _dp]),
     "fdtd_set_materials_full": (C.c_int, [_vp, C.POINTER(_vp), C.POINTER(_vp), C.POINTER(_vp)]),
     "fdtd_step": (C.c_int, [_vp, C.c_long]),
+    "fdtd_profile_step": (C.c_int, [_vp, C.c_long, _dp]),
     "fdtd_read_fields": (C.c_int, [_vp, C.c_int, _vp]),
     "fdtd_write_fields": (C.c_int, [_vp, C.c_int, _vp]),
     "fdtd_read_port_dft": (C.c_int, [_vp, C.c_int, _dp, _dp]),
@@ -179,6 +180,13 @@ def fdtd_set_materials_full(h, eps_r, sigma, mu_r=None):
 
 def fdtd_step(h, n=1):
     _check(h, lib().fdtd_step(h, int(n)))
+
+
+def fdtd_profile_step(h, n):
+    """n steps with CUDA events between the kernels; returns ms per step of [H|fused, E, source, probes+DFT]."""
+    ms = (C.c_double * 4)()
+    _check(h, lib().fdtd_profile_step(h, int(n), ms))
+    return list(ms)
 
 
 def fdtd_read_fields(h, comp, dst):

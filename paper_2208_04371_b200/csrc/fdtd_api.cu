@@ -77,6 +77,7 @@ struct fdtd {
   virtual int set_materials_indexed(const uint8_t* idx, int ne, const double* eps, const double* sig, const double* mu) = 0;
   virtual int set_materials_full(const void* const eps[3], const void* const sig[3], const void* const mu[3]) = 0;
   virtual int step(long n) = 0;
+  virtual int profile_step(long n, double* ms) = 0;
   virtual int read_field(int comp, void* dst) = 0;
   virtual int write_field(int comp, const void* src) = 0;
   virtual int read_port_dft(int port, double* V, double* I) = 0;
@@ -155,6 +156,7 @@ struct Solver : fdtd {
   int set_materials_indexed(const uint8_t* idx, int ne, const double* eps, const double* sig, const double* mu) override;
   int set_materials_full(const void* const eps[3], const void* const sig[3], const void* const mu[3]) override;
   int step(long n) override;
+  int profile_step(long n, double* ms) override;
   int read_field(int comp, void* dst) override { return copy_field(comp, dst, true); }
   int write_field(int comp, const void* src) override { return copy_field(comp, const_cast<void*>(src), false); }
   int read_port_dft(int port, double* V, double* I) override;
@@ -165,7 +167,7 @@ struct Solver : fdtd {
   int copy_field(int comp, void* user, bool to_user);
   int copy3d(void* internal_origin, size_t elem, void* user, bool to_user);
   void build_cpml_vectors();
-  void enqueue_step();
+  void enqueue_step(cudaEvent_t* ev = nullptr);
   int build_graph();
 };
 
@@ -392,34 +394,67 @@ int Solver<T>::set_materials_full(const void* const eps[3], const void* const si
 
 // ---- one step = H pass, E pass, sources, probes + DFT (R5) -------------------------------------------------------
 template <typename T, int MODE>
-static void launch_two_pass(const StepParams<T>& sp, cudaStream_t st) {
+static void launch_two_pass(const StepParams<T>& sp, cudaStream_t st, cudaEvent_t* ev) {
   constexpr int V = VecOf<T>::V;
   const int nvec = (sp.nx + V - 1) / V;
   int bx = 1;
   while (bx < nvec && bx < 128) bx <<= 1;
   const int by = 128 / bx;
   const dim3 block(bx, by, 1), grid((nvec + bx - 1) / bx, (sp.ny + by - 1) / by, sp.nz);
+  if (ev) cudaEventRecord(ev[0], st);
   k_update_H<T, MODE><<<grid, block, 0, st>>>(sp);
+  if (ev) cudaEventRecord(ev[1], st);
   k_update_E<T, MODE><<<grid, block, 0, st>>>(sp);
+  if (ev) cudaEventRecord(ev[2], st);
 }
 
 template <typename T>
-void Solver<T>::enqueue_step() {
+void Solver<T>::enqueue_step(cudaEvent_t* ev) {
   switch (mode()) {
-    case 0: launch_two_pass<T, 0>(sp, stream); break;
-    case 1: launch_two_pass<T, 1>(sp, stream); break;
-    case 2: launch_two_pass<T, 2>(sp, stream); break;
-    default: launch_two_pass<T, 3>(sp, stream); break;
+    case 0: launch_two_pass<T, 0>(sp, stream, ev); break;
+    case 1: launch_two_pass<T, 1>(sp, stream, ev); break;
+    case 2: launch_two_pass<T, 2>(sp, stream, ev); break;
+    default: launch_two_pass<T, 3>(sp, stream, ev); break;
   }
   launches += 2;
   if (!ports.empty()) {
     bool any_src = false;
     for (const PortDev& q : ports) any_src = any_src || q.has_source;
     if (any_src) { k_source<T><<<1, 256, 0, stream>>>(pp); ++launches; }
+    if (ev) cudaEventRecord(ev[3], stream);
     const dim3 grid((unsigned)ports.size(), (unsigned)(freqs.empty() ? 1 : (freqs.size() + 63) / 64), 1);
     k_probe_dft<T><<<grid, 128, 0, stream>>>(pp);
     ++launches;
+    if (ev) cudaEventRecord(ev[4], stream);
+  } else if (ev) {
+    cudaEventRecord(ev[3], stream);
+    cudaEventRecord(ev[4], stream);
   }
+}
+
+template <typename T>
+int Solver<T>::profile_step(long n, double* ms) {
+  if (!committed) return fail(FDTD_ESTATE, "fdtd_profile_step: call after fdtd_commit");
+  if (n < 1 || !ms) return fail(FDTD_EINVAL, "fdtd_profile_step: n < 1 or null pointer");
+  cudaEvent_t ev[5];
+  for (int q = 0; q < 5; ++q)
+    if (cudaEventCreate(&ev[q]) != cudaSuccess) return cuda_fail(cudaGetLastError(), "fdtd_profile_step: event");
+  for (int q = 0; q < 4; ++q) ms[q] = 0.0;
+  cudaError_t e = cudaSuccess;
+  for (long s = 0; s < n && e == cudaSuccess; ++s) {
+    enqueue_step(ev);
+    if ((e = cudaEventSynchronize(ev[4])) != cudaSuccess) break;
+    for (int q = 0; q < 4; ++q) {
+      float t = 0.f;
+      cudaEventElapsedTime(&t, ev[q], ev[q + 1]);
+      ms[q] += (double)t / (double)n;
+    }
+  }
+  for (int q = 0; q < 5; ++q) cudaEventDestroy(ev[q]);
+  if (e == cudaSuccess) e = cudaGetLastError();
+  if (e != cudaSuccess) return cuda_fail(e, "fdtd_profile_step");
+  nstep += n;
+  return FDTD_OK;
 }
 
 template <typename T>
@@ -612,6 +647,7 @@ int fdtd_set_materials_full(fdtd_t* h, const void* const eps_r[3], const void* c
   return h ? h->set_materials_full(eps_r, sigma, mu_r) : FDTD_EINVAL;
 }
 int fdtd_step(fdtd_t* h, long n) { return h ? h->step(n) : FDTD_EINVAL; }
+int fdtd_profile_step(fdtd_t* h, long n, double ms_avg[4]) { return h ? h->profile_step(n, ms_avg) : FDTD_EINVAL; }
 int fdtd_read_fields(fdtd_t* h, int comp, void* dst) { return h ? h->read_field(comp, dst) : FDTD_EINVAL; }
 int fdtd_write_fields(fdtd_t* h, int comp, const void* src) { return h ? h->write_field(comp, src) : FDTD_EINVAL; }
 int fdtd_read_port_dft(fdtd_t* h, int port, double* V, double* I) { return h ? h->read_port_dft(port, V, I) : FDTD_EINVAL; }

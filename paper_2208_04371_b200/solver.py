@@ -66,6 +66,9 @@ class Solver:
     def step(self, n=1):
         B.fdtd_step(self.h, n)
 
+    def profile_step(self, n=1):
+        return B.fdtd_profile_step(self.h, n)
+
     @property
     def dtype(self):
         torch = _torch()
