@@ -194,6 +194,24 @@ def algorithmic_bytes(w, impl, kernel):
 
 
 # --------------------------------------------------------------------------------------------------------------------
+# replicas: every rank runs the same workload on its own GPU; the job time is the max over ranks
+# --------------------------------------------------------------------------------------------------------------------
+def max_over_ranks(seconds, world, device):
+    """The slowest rank's time (torch.distributed MAX all-reduce when world > 1; works with gloo on CPU tensors)."""
+    import torch
+    t = torch.tensor([seconds], dtype=torch.float64, device=device)
+    if world > 1:
+        import torch.distributed as dist
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_throughput(n_cells, steps, world, seconds):
+    """Whole-job Mcell-updates/s: every rank advanced n_cells cells by `steps` steps in `seconds` (max over ranks)."""
+    return n_cells * steps * world / seconds / 1e6
+
+
+# --------------------------------------------------------------------------------------------------------------------
 # our arm
 # --------------------------------------------------------------------------------------------------------------------
 def run_ours(args, rank, world, local_rank):
@@ -234,11 +252,8 @@ def run_ours(args, rank, world, local_rank):
     barrier()
     ck = clocks.stop()
     launches = s.launch_count - l0
-    t_ms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t_ms, op=dist.ReduceOp.MAX)
-    t_s = float(t_ms.item()) * 1e-3
-    value = n_cells * K * world / t_s / 1e6
+    t_s = max_over_ranks(e0.elapsed_time(e1) * 1e-3, world, dev)
+    value = job_throughput(n_cells, K, world, t_s)
 
     # ---- per-kernel durations (CUDA events between the kernels, on the solver's stream) ------------------------------
     ms = s.profile_step(max(3, min(20, K)))
@@ -271,13 +286,11 @@ def run_ours(args, rank, world, local_rank):
         s.step(K)
         out = [s.read_port_dft(p) for p in range(nports)]          # device -> host, synchronises
         torch.cuda.synchronize(dev)
-        te = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(te, op=dist.ReduceOp.MAX)
-        h2d = idx_host.numel() + 9 * 256 * (4 if w["precision"] == 32 else 8)
+        te = max_over_ranks(time.perf_counter() - t0, world, dev)
+        h2d = idx_host.numel() + 12 * 256 * (4 if w["precision"] == 32 else 8)
         d2h = nports * nf * 2 * 2 * 8
         assert all(np.isfinite(v).all() and np.isfinite(i).all() for v, i in out)
-        e2e = {"value": n_cells * K * world / float(te.item()) / 1e6, "unit": UNIT,
+        e2e = {"value": job_throughput(n_cells, K, world, te), "unit": UNIT,
                "h2d_bytes_per_step": h2d / K, "d2h_bytes_per_step": d2h / K,
                "what": "fdtd_set_materials_indexed(pinned host idx) + fdtd_reset + fdtd_step(K) + fdtd_read_port_dft x ports"}
 

@@ -50,9 +50,11 @@ enum { FDTD_EX = 0, FDTD_EY, FDTD_EZ, FDTD_HX, FDTD_HY, FDTD_HZ };
 
 /* Options for fdtd_set_option (before commit). */
 enum {
-  FDTD_OPT_STEP_IMPL = 1,   /* 0 = auto, 1 = two-pass (H kernel, E kernel), 2 = fused E+H temporal blocking            */
+  FDTD_OPT_STEP_IMPL = 1,   /* 0 = auto (fused from 4 Mi cells up), 1 = two-pass (H kernel, E kernel, in place),
+                               2 = fused E+H kernel (temporal blocking over the half steps; a second field set)         */
   FDTD_OPT_USE_GRAPH = 2,   /* 1 (default) = replay a captured CUDA graph per step; 0 = plain launches                  */
-  FDTD_OPT_GRAPH_UNROLL = 3 /* steps per captured graph (default 8)                                                     */
+  FDTD_OPT_GRAPH_UNROLL = 3,/* steps per captured graph (default 8; rounded up to even for the fused step)              */
+  FDTD_OPT_FUSED_KZ = 4     /* planes per z chunk of the fused kernel (0 = auto)                                        */
 };
 
 /* A port (Fig. 1a): a soft E_z source on a box of the plane i = is (surface 'e'), a voltage box and

@@ -14,7 +14,11 @@
 #include <string>
 #include <vector>
 
+#include <cuda.h>
+#include <cudaTypedefs.h>
+
 #include "../../include/fdtd.h"
+#include "fdtd_fused.cuh"
 #include "fdtd_kernels.cuh"
 #include "fdtd_params.h"
 
@@ -45,7 +49,7 @@ struct fdtd {
   int has_mu = 0;
   std::vector<PortDev> ports;
   std::vector<double> freqs;
-  long opt_impl = 0, opt_graph = 1, opt_unroll = 8;
+  long opt_impl = 0, opt_graph = 1, opt_unroll = 8, opt_kz = 0, opt_cfg = 0;
   bool committed = false;
   long nstep = 0;
   long launches = 0;
@@ -98,18 +102,30 @@ template <typename T>
 struct Solver : fdtd {
   // workspace carve (byte offsets), filled by layout()
   struct Carve {
-    size_t field[6], idx, tab, coef[9], psi[12], vec[18], ports, freqs, dftV, dftI, lastV, lastI, nstep, total;
+    size_t field[6], field2[6], idx, tab, coef[9], psi[12], psiH2[6], vec[18], ports, freqs, dftV, dftI, lastV, lastI, nstep, total;
   };
   char* ws = nullptr;
   Carve cv{};
-  StepParams<T> sp{};
-  PortParams<T> pp{};
+  StepParams<T> sp{};      // two-pass: in place on set 0
+  PortParams<T> pp{};      // ports on set 0; pp2 on set 1
+  PortParams<T> pp2{};
+  // fused step: two field sets (ping-pong); fpar[c] reads set c and writes set 1-c; cur = set holding the current state
+  bool fused = false;
+  int cur = 0;
+  int kz = 0;
+  FusedParams<T> fpar[2];
+  cudaGraphExec_t gexec2 = nullptr;  // graph captured with cur == 1
   std::vector<T> h_tab;        // host staging of the material table (kept alive for the async upload)
   std::vector<T> h_vec[18];
   cudaGraphExec_t gexec = nullptr;
   int graph_steps = 0;
 
-  ~Solver() override { if (gexec) cudaGraphExecDestroy(gexec); }
+  ~Solver() override {
+    if (gexec) cudaGraphExecDestroy(gexec);
+    if (gexec2) cudaGraphExecDestroy(gexec2);
+  }
+  // auto: the fused kernel pays off once the grid no longer fits in L2 (small grids are launch-bound)
+  bool want_fused() const { return opt_impl == 2 || (opt_impl == 0 && (long long)nx * ny * nz >= (4LL << 20)); }
 
   int mode() const { return (mat_mode == FDTD_MAT_FULL ? kModeFull : 0) | (has_mu ? kModeMu : 0); }
   size_t psi_elems(int a) const {
@@ -129,13 +145,15 @@ struct Solver : fdtd {
     auto take = [&](size_t bytes) { const size_t o = off; off += align_up(bytes, 256); return o; };
     const size_t fbytes = (size_t)cells_padded() * sizeof(T);
     for (int f = 0; f < 6; ++f) c.field[f] = take(fbytes);
+    if (want_fused()) for (int f = 0; f < 6; ++f) c.field2[f] = take(fbytes);
     if (mat_mode == FDTD_MAT_INDEXED) {
       c.idx = take((size_t)cells_padded());
-      c.tab = take(9 * kMaxTable * sizeof(T));
+      c.tab = take(kTabWords * sizeof(T));
     } else {
       for (int q = 0; q < (has_mu ? 9 : 6); ++q) c.coef[q] = take(fbytes);
     }
     for (int q = 0; q < 12; ++q) c.psi[q] = take(psi_elems(psi_axis(q)) * sizeof(T));
+    if (want_fused()) for (int q = 0; q < 6; ++q) c.psiH2[q] = take(psi_elems(psi_axis(q)) * sizeof(T));
     for (int a = 0; a < 3; ++a)
       for (int v = 0; v < 6; ++v) c.vec[a * 6 + v] = take((size_t)(S(a) > 0 ? S(a) : 1) * sizeof(T));
     c.ports = take((ports.size() + 1) * sizeof(PortDev));
@@ -150,7 +168,7 @@ struct Solver : fdtd {
   }
   size_t workspace_bytes() const override { return layout().total; }
 
-  T* field_origin(int f) const { return reinterpret_cast<T*>(ws + cv.field[f]) + plane(); }
+  T* field_origin(int f, int set = 0) const { return reinterpret_cast<T*>(ws + (set ? cv.field2[f] : cv.field[f])) + plane(); }
 
   int commit(void* w, size_t bytes, void* st) override;
   int set_materials_indexed(const uint8_t* idx, int ne, const double* eps, const double* sig, const double* mu) override;
@@ -162,13 +180,15 @@ struct Solver : fdtd {
   int read_port_dft(int port, double* V, double* I) override;
   int read_port_last(int port, double* V, double* I) override;
   int reset() override;
-  const char* impl_name() const override { return "two_pass"; }
+  const char* impl_name() const override { return fused ? "fused" : "two_pass"; }
+  int build_fused();
+  void launch_fused(cudaEvent_t* ev);
 
   int copy_field(int comp, void* user, bool to_user);
   int copy3d(void* internal_origin, size_t elem, void* user, bool to_user);
   void build_cpml_vectors();
   void enqueue_step(cudaEvent_t* ev = nullptr);
-  int build_graph();
+  int build_graph(cudaGraphExec_t* out);
 };
 
 // R4 (CPML, convolutional PML with recursive convolution): per axis, per slab coordinate s, at the E positions
@@ -270,16 +290,25 @@ int Solver<T>::commit(void* w, size_t bytes, void* st) {
       (e = cudaMemcpyAsync(ws + cv.freqs, freqs.data(), freqs.size() * sizeof(double), cudaMemcpyHostToDevice, stream)) != cudaSuccess)
     return cuda_fail(e, "fdtd_commit: upload frequencies");
 
+  pp2 = pp;
+  fused = want_fused();
+  cur = 0;
+  if (fused) {
+    pp2.Ez = field_origin(kEz, 1); pp2.Hy = field_origin(kHy, 1); pp2.Hz = field_origin(kHz, 1);
+    const int r = build_fused();
+    if (r != FDTD_OK) return r;
+  }
+
   // vacuum everywhere
   const long long np = cells_padded();
   const unsigned nb = (unsigned)((np + 255) / 256);
   if (mat_mode == FDTD_MAT_INDEXED) {
-    h_tab.assign(9 * kMaxTable, T(0));
+    h_tab.assign(kTabWords, T(0));
     for (int m = 0; m < kMaxTable; ++m)
       for (int c = 0; c < 3; ++c) {
-        h_tab[c * kMaxTable + m] = T(1);
-        h_tab[(3 + c) * kMaxTable + m] = T(dt / kEps0);
-        h_tab[(6 + c) * kMaxTable + m] = T(dt / kMu0);
+        h_tab[8 * m + c] = T(1);
+        h_tab[8 * m + 3 + c] = T(dt / kEps0);
+        h_tab[kTabH + 4 * m + c] = T(dt / kMu0);
       }
     if ((e = cudaMemcpyAsync(ws + cv.tab, h_tab.data(), h_tab.size() * sizeof(T), cudaMemcpyHostToDevice, stream)) != cudaSuccess)
       return cuda_fail(e, "fdtd_commit: upload table");
@@ -322,7 +351,7 @@ template <typename T>
 int Solver<T>::copy_field(int comp, void* user, bool to_user) {
   if (!committed) return fail(FDTD_ESTATE, "fields are available after fdtd_commit");
   if (comp < 0 || comp > 5 || !user) return fail(FDTD_EINVAL, "bad component or null pointer");
-  return copy3d(ws + cv.field[comp], sizeof(T), user, to_user);
+  return copy3d(ws + (cur ? cv.field2[comp] : cv.field[comp]), sizeof(T), user, to_user);
 }
 
 template <typename T>
@@ -336,16 +365,16 @@ int Solver<T>::set_materials_indexed(const uint8_t* idx, int ne, const double* e
       return fail(FDTD_EINVAL, "fdtd_set_materials_indexed: entry %d: need eps_r > 0, sigma >= 0, mu_r > 0", q / 3);
   }
   // R3: a = sigma dt / (2 eps0 eps_r); Ca = (1-a)/(1+a); Cb = (dt/(eps0 eps_r))/(1+a); sigma = +inf -> PEC (0, 0)
-  h_tab.assign(9 * kMaxTable, T(0));
+  h_tab.assign(kTabWords, T(0));
   for (int m = 0; m < kMaxTable; ++m) {
     const int s = m < ne ? m : 0;  // indices beyond the table alias entry 0 (never produce wild values)
     for (int c = 0; c < 3; ++c) {
       const double er = eps[3 * s + c], sg = sig[3 * s + c], mr = mu ? mu[3 * s + c] : 1.0;
       double ca = 0.0, cb = 0.0;
       if (!std::isinf(sg)) { const double a = sg * dt / (2.0 * kEps0 * er); ca = (1.0 - a) / (1.0 + a); cb = (dt / (kEps0 * er)) / (1.0 + a); }
-      h_tab[c * kMaxTable + m] = T(ca);
-      h_tab[(3 + c) * kMaxTable + m] = T(cb);
-      h_tab[(6 + c) * kMaxTable + m] = T(dt / (kMu0 * mr));
+      h_tab[8 * m + c] = T(ca);
+      h_tab[8 * m + 3 + c] = T(cb);
+      h_tab[kTabH + 4 * m + c] = T(dt / (kMu0 * mr));
     }
   }
   cudaError_t e = cudaMemcpyAsync(ws + cv.tab, h_tab.data(), h_tab.size() * sizeof(T), cudaMemcpyHostToDevice, stream);
@@ -408,22 +437,119 @@ static void launch_two_pass(const StepParams<T>& sp, cudaStream_t st, cudaEvent_
   if (ev) cudaEventRecord(ev[2], st);
 }
 
+// ---- fused step: tensor maps for both ping-pong directions, launch --------------------------------------------------
+static PFN_cuTensorMapEncodeTiled_v12000 tensor_map_encoder() {
+  static PFN_cuTensorMapEncodeTiled_v12000 fn = nullptr;
+  if (!fn) {
+    void* q = nullptr;
+    cudaDriverEntryPointQueryResult st;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &q, cudaEnableDefault, &st) == cudaSuccess && st == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(q);
+  }
+  return fn;
+}
+
+template <typename T> struct FusedTile { static constexpr int TY = 8, NS = 4; };
+
+template <typename T, int MODE>
+static cudaError_t fused_set_attr() {
+  using C = FusedCfg<T, FusedTile<T>::TY, FusedTile<T>::NS>;
+  return cudaFuncSetAttribute(k_step_fused<T, MODE, C::TY, C::NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM);
+}
+template <typename T, int MODE>
+static void fused_launch(const FusedParams<T>& fp, cudaStream_t st) {
+  using C = FusedCfg<T, FusedTile<T>::TY, FusedTile<T>::NS>;
+  const StepParams<T>& sp = fp.sp;
+  const dim3 grid((sp.nx + C::TX - 1) / C::TX, (sp.ny + C::TY - 1) / C::TY, (sp.nz + fp.kz - 1) / fp.kz);
+  k_step_fused<T, MODE, C::TY, C::NS><<<grid, C::THREADS, C::SMEM, st>>>(fp);
+}
+
+template <typename T>
+int Solver<T>::build_fused() {
+  using C = FusedCfg<T, FusedTile<T>::TY, FusedTile<T>::NS>;
+  auto enc = tensor_map_encoder();
+  if (!enc) return fail(FDTD_ECUDA, "fdtd_commit: the driver does not export cuTensorMapEncodeTiled (fused step needs TMA)");
+  cudaError_t e = cudaSuccess;
+  switch (mode()) {
+    case 0: e = fused_set_attr<T, 0>(); break;
+    case 1: e = fused_set_attr<T, 1>(); break;
+    case 2: e = fused_set_attr<T, 2>(); break;
+    default: e = fused_set_attr<T, 3>(); break;
+  }
+  if (e != cudaSuccess) return cuda_fail(e, "fdtd_commit: shared memory opt-in of the fused kernel");
+  // planes per z chunk: long chunks amortise the two priming iterations; enough blocks for a few waves of 148 SMs
+  const long long tiles = (long long)((nx + C::TX - 1) / C::TX) * ((ny + C::TY - 1) / C::TY);
+  kz = opt_kz > 0 ? (int)opt_kz : 128;
+  if (opt_kz <= 0) while (kz > 16 && tiles * ((nz + kz - 1) / kz) < 4 * 148) kz /= 2;
+  if (kz > nz) kz = nz;
+
+  const cuuint64_t gdim[3] = {(cuuint64_t)pitch(), (cuuint64_t)(ny + 1), (cuuint64_t)(nz + 2)};
+  const cuuint32_t estr[3] = {1, 1, 1};
+  auto make = [&](CUtensorMap* tm, void* base, CUtensorMapDataType dt, size_t es, int bx, int by) -> bool {
+    const cuuint64_t gstr[2] = {(cuuint64_t)pitch() * es, (cuuint64_t)plane() * es};
+    const cuuint32_t box[3] = {(cuuint32_t)bx, (cuuint32_t)by, 1};
+    return enc(tm, dt, 3, base, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+               CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+  };
+  const CUtensorMapDataType fdt = sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
+  for (int c = 0; c < 2; ++c) {
+    FusedParams<T>& fp = fpar[c];
+    fp.sp = sp;
+    for (int f = 0; f < 6; ++f) { fp.sp.src[f] = field_origin(f, c); fp.sp.dst[f] = field_origin(f, 1 - c); }
+    for (int q = 0; q < 6; ++q) {
+      fp.psiH_src[q] = reinterpret_cast<T*>(ws + (c ? cv.psiH2[q] : cv.psi[q]));
+      fp.sp.psi[q] = reinterpret_cast<T*>(ws + (c ? cv.psi[q] : cv.psiH2[q]));
+    }
+    fp.kz = kz;
+    for (int f = 0; f < 6; ++f) {
+      if (!make(&fp.tm[f], ws + (c ? cv.field2[f] : cv.field[f]), fdt, sizeof(T), C::BX, f < 3 ? C::ROWS_E : C::ROWS_H))
+        return fail(FDTD_ECUDA, "fdtd_commit: cuTensorMapEncodeTiled failed for field %d", f);
+    }
+    if (mat_mode == FDTD_MAT_INDEXED) {
+      if (!make(&fp.tm[6], ws + cv.idx, CU_TENSOR_MAP_DATA_TYPE_UINT8, 1, C::TX, C::TY))
+        return fail(FDTD_ECUDA, "fdtd_commit: cuTensorMapEncodeTiled failed for the material index");
+    } else {
+      fp.tm[6] = fp.tm[0];
+    }
+  }
+  return FDTD_OK;
+}
+
+template <typename T>
+void Solver<T>::launch_fused(cudaEvent_t* ev) {
+  if (ev) cudaEventRecord(ev[0], stream);
+  switch (mode()) {
+    case 0: fused_launch<T, 0>(fpar[cur], stream); break;
+    case 1: fused_launch<T, 1>(fpar[cur], stream); break;
+    case 2: fused_launch<T, 2>(fpar[cur], stream); break;
+    default: fused_launch<T, 3>(fpar[cur], stream); break;
+  }
+  if (ev) { cudaEventRecord(ev[1], stream); cudaEventRecord(ev[2], stream); }
+  cur ^= 1;
+}
+
 template <typename T>
 void Solver<T>::enqueue_step(cudaEvent_t* ev) {
-  switch (mode()) {
-    case 0: launch_two_pass<T, 0>(sp, stream, ev); break;
-    case 1: launch_two_pass<T, 1>(sp, stream, ev); break;
-    case 2: launch_two_pass<T, 2>(sp, stream, ev); break;
-    default: launch_two_pass<T, 3>(sp, stream, ev); break;
+  if (fused) {
+    launch_fused(ev);
+    launches += 1;
+  } else {
+    switch (mode()) {
+      case 0: launch_two_pass<T, 0>(sp, stream, ev); break;
+      case 1: launch_two_pass<T, 1>(sp, stream, ev); break;
+      case 2: launch_two_pass<T, 2>(sp, stream, ev); break;
+      default: launch_two_pass<T, 3>(sp, stream, ev); break;
+    }
+    launches += 2;
   }
-  launches += 2;
+  const PortParams<T>& q = cur ? pp2 : pp;   // the set that now holds E^{n+1}, H^{n+1/2}
   if (!ports.empty()) {
     bool any_src = false;
-    for (const PortDev& q : ports) any_src = any_src || q.has_source;
-    if (any_src) { k_source<T><<<1, 256, 0, stream>>>(pp); ++launches; }
+    for (const PortDev& d : ports) any_src = any_src || d.has_source;
+    if (any_src) { k_source<T><<<1, 256, 0, stream>>>(q); ++launches; }
     if (ev) cudaEventRecord(ev[3], stream);
     const dim3 grid((unsigned)ports.size(), (unsigned)(freqs.empty() ? 1 : (freqs.size() + 63) / 64), 1);
-    k_probe_dft<T><<<grid, 128, 0, stream>>>(pp);
+    k_probe_dft<T><<<grid, 128, 0, stream>>>(q);
     ++launches;
     if (ev) cudaEventRecord(ev[4], stream);
   } else if (ev) {
@@ -458,20 +584,21 @@ int Solver<T>::profile_step(long n, double* ms) {
 }
 
 template <typename T>
-int Solver<T>::build_graph() {
-  if (gexec) return FDTD_OK;
+int Solver<T>::build_graph(cudaGraphExec_t* out) {
+  if (*out) return FDTD_OK;
   const long before = launches;
+  const int cur_before = cur;
   cudaError_t e = cudaStreamBeginCapture(stream, cudaStreamCaptureModeThreadLocal);
   if (e != cudaSuccess) return cuda_fail(e, "graph capture begin");
-  for (int s = 0; s < (int)opt_unroll; ++s) enqueue_step();
+  for (int s = 0; s < graph_steps; ++s) enqueue_step();
   cudaGraph_t g = nullptr;
   e = cudaStreamEndCapture(stream, &g);
   launches = before;
+  cur = cur_before;   // graph_steps is even when the step ping-pongs, so a replay ends on the set it started from
   if (e != cudaSuccess) return cuda_fail(e, "graph capture end");
-  e = cudaGraphInstantiate(&gexec, g, 0);
+  e = cudaGraphInstantiate(out, g, 0);
   cudaGraphDestroy(g);
-  if (e != cudaSuccess) { gexec = nullptr; return cuda_fail(e, "graph instantiate"); }
-  graph_steps = (int)opt_unroll;
+  if (e != cudaSuccess) { *out = nullptr; return cuda_fail(e, "graph instantiate"); }
   return FDTD_OK;
 }
 
@@ -480,15 +607,15 @@ int Solver<T>::step(long n) {
   if (!committed) return fail(FDTD_ESTATE, "fdtd_step: call after fdtd_commit");
   if (n < 0) return fail(FDTD_EINVAL, "fdtd_step: n < 0");
   long left = n;
-  if (opt_graph && stream != nullptr && left >= opt_unroll) {
-    const int r = build_graph();
+  graph_steps = (int)opt_unroll + ((fused && (opt_unroll & 1)) ? 1 : 0);
+  if (opt_graph && stream != nullptr && left >= graph_steps) {
+    cudaGraphExec_t* g = cur ? &gexec2 : &gexec;
+    const int r = build_graph(g);
     if (r != FDTD_OK) return r;
-    const long per = launches;  // count the launches of one replay
-    (void)per;
-    long nodes = 2;
+    long nodes = fused ? 1 : 2;
     if (!ports.empty()) { nodes += 1; for (const PortDev& q : ports) if (q.has_source) { nodes += 1; break; } }
     while (left >= graph_steps) {
-      const cudaError_t e = cudaGraphLaunch(gexec, stream);
+      const cudaError_t e = cudaGraphLaunch(*g, stream);
       if (e != cudaSuccess) return cuda_fail(e, "graph launch");
       left -= graph_steps;
       launches += nodes * graph_steps;
@@ -533,8 +660,12 @@ int Solver<T>::reset() {
   cudaError_t e = cudaSuccess;
   const size_t fbytes = (size_t)cells_padded() * sizeof(T);
   for (int f = 0; f < 6 && e == cudaSuccess; ++f) e = cudaMemsetAsync(ws + cv.field[f], 0, fbytes, stream);
+  for (int f = 0; f < 6 && e == cudaSuccess && fused; ++f) e = cudaMemsetAsync(ws + cv.field2[f], 0, fbytes, stream);
   for (int q = 0; q < 12 && e == cudaSuccess; ++q)
     if (psi_elems(psi_axis(q))) e = cudaMemsetAsync(ws + cv.psi[q], 0, psi_elems(psi_axis(q)) * sizeof(T), stream);
+  for (int q = 0; q < 6 && e == cudaSuccess && fused; ++q)
+    if (psi_elems(psi_axis(q))) e = cudaMemsetAsync(ws + cv.psiH2[q], 0, psi_elems(psi_axis(q)) * sizeof(T), stream);
+  cur = 0;
   if (e == cudaSuccess) e = cudaMemsetAsync(ws + cv.dftV, 0, cv.nstep + sizeof(long long) - cv.dftV, stream);
   if (e != cudaSuccess) return cuda_fail(e, "fdtd_reset");
   nstep = 0;
@@ -634,6 +765,7 @@ int fdtd_set_option(fdtd_t* h, int option, long value) {
     case FDTD_OPT_STEP_IMPL: if (value < 0 || value > 2) break; h->opt_impl = value; return FDTD_OK;
     case FDTD_OPT_USE_GRAPH: h->opt_graph = value ? 1 : 0; return FDTD_OK;
     case FDTD_OPT_GRAPH_UNROLL: if (value < 1 || value > 1024) break; h->opt_unroll = value; return FDTD_OK;
+    case FDTD_OPT_FUSED_KZ: if (value < 0 || value > 65535) break; h->opt_kz = value; return FDTD_OK;
   }
   return h->fail(FDTD_EINVAL, "fdtd_set_option: unknown option %d or bad value %ld", option, value);
 }

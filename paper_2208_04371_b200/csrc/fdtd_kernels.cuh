@@ -33,6 +33,27 @@ __device__ __forceinline__ void stv(double* p, const double (&r)[2]) {
   *reinterpret_cast<double2*>(p) = make_double2(r[0], r[1]);
 }
 
+// four consecutive table words with the widest loads the type allows (read-only path)
+template <typename T> struct Vec4 { T a, b, c, d; };
+__device__ __forceinline__ Vec4<float> ld4(const float* p) {
+  const float4 v = __ldg(reinterpret_cast<const float4*>(p));
+  return {v.x, v.y, v.z, v.w};
+}
+__device__ __forceinline__ Vec4<double> ld4(const double* p) {
+  const double2 u = __ldg(reinterpret_cast<const double2*>(p)), w = __ldg(reinterpret_cast<const double2*>(p) + 1);
+  return {u.x, u.y, w.x, w.y};
+}
+// the material indices of a thread's V consecutive cells in one load
+template <int V> __device__ __forceinline__ void ld_index(const uint8_t* p, unsigned char (&m)[V]);
+template <> __device__ __forceinline__ void ld_index<4>(const uint8_t* p, unsigned char (&m)[4]) {
+  const uchar4 q = __ldg(reinterpret_cast<const uchar4*>(p));
+  m[0] = q.x; m[1] = q.y; m[2] = q.z; m[3] = q.w;
+}
+template <> __device__ __forceinline__ void ld_index<2>(const uint8_t* p, unsigned char (&m)[2]) {
+  const uchar2 q = __ldg(reinterpret_cast<const uchar2*>(p));
+  m[0] = q.x; m[1] = q.y;
+}
+
 // slab coordinate of index u on an axis of n cells with lo / hi CPML cells, or -1 in the interior
 __device__ __forceinline__ int slab_coord(int u, int lo, int hi, int n) {
   return u < lo ? u : (u >= n - hi ? lo + u - (n - hi) : -1);
@@ -129,10 +150,12 @@ __global__ void __launch_bounds__(128) k_update_H(const StepParams<T> p) {
   if (MODE & kModeMu) {
     if (MODE & kModeFull) { ldv(p.Db[0] + o, dbx); ldv(p.Db[1] + o, dby); ldv(p.Db[2] + o, dbz); }
     else {
+      unsigned char m[V];
+      ld_index<V>(p.idx + o, m);
 #pragma unroll
       for (int v = 0; v < V; ++v) {
-        const int m = p.idx[o + v];
-        dbx[v] = p.tab[6 * kMaxTable + m]; dby[v] = p.tab[7 * kMaxTable + m]; dbz[v] = p.tab[8 * kMaxTable + m];
+        const Vec4<T> d = ld4(p.tab + kTabH + 4 * (int)m[v]);   // {Dbx, Dby, Dbz, -}
+        dbx[v] = d.a; dby[v] = d.b; dbz[v] = d.c;
       }
     }
   } else {
@@ -233,11 +256,13 @@ __global__ void __launch_bounds__(128) k_update_E(const StepParams<T> p) {
     ldv(p.Ca[0] + o, cax); ldv(p.Ca[1] + o, cay); ldv(p.Ca[2] + o, caz);
     ldv(p.Cb[0] + o, cbx); ldv(p.Cb[1] + o, cby); ldv(p.Cb[2] + o, cbz);
   } else {
+    unsigned char m[V];
+    ld_index<V>(p.idx + o, m);    // one 32-bit (16-bit) load for the thread's 4 (2) cells
 #pragma unroll
     for (int v = 0; v < V; ++v) {
-      const int m = p.idx[o + v];
-      cax[v] = p.tab[0 * kMaxTable + m]; cay[v] = p.tab[1 * kMaxTable + m]; caz[v] = p.tab[2 * kMaxTable + m];
-      cbx[v] = p.tab[3 * kMaxTable + m]; cby[v] = p.tab[4 * kMaxTable + m]; cbz[v] = p.tab[5 * kMaxTable + m];
+      const Vec4<T> a = ld4(p.tab + 8 * (int)m[v]);       // {Cax, Cay, Caz, Cbx}
+      const Vec4<T> b = ld4(p.tab + 8 * (int)m[v] + 4);   // {Cby, Cbz, -, -}
+      cax[v] = a.a; cay[v] = a.b; caz[v] = a.c; cbx[v] = a.d; cby[v] = b.a; cbz[v] = b.b;
     }
   }
   const bool wj = (j == 0), wk = (k == 0);

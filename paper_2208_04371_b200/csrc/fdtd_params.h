@@ -18,6 +18,10 @@ enum { kEx = 0, kEy, kEz, kHx, kHy, kHz };
 enum { pHxy = 0, pHzy, pHxz, pHyz, pHyx, pHzx, pExy, pEzy, pExz, pEyz, pEyx, pEzx };
 
 constexpr int kMaxTable = 256;
+// material table (indexed mode), one 32-byte (fp32) / 64-byte (fp64) record per entry so that a look-up is two
+// (four) 128-bit loads:  tab[8*m + 0..5] = Cax Cay Caz Cbx Cby Cbz, then tab[kTabH + 4*m + 0..2] = Dbx Dby Dbz.
+constexpr int kTabH = 8 * kMaxTable;
+constexpr int kTabWords = 12 * kMaxTable;
 
 template <typename T>
 struct StepParams {
@@ -28,7 +32,7 @@ struct StepParams {
   T* dst[6];        // fields written (== src for the two-pass in-place kernels)
   // materials
   const uint8_t* idx;   // indexed mode: one byte per cell, field geometry
-  const T* tab;         // indexed mode: [9][kMaxTable] = Ca x,y,z | Cb x,y,z | Db x,y,z
+  const T* tab;         // indexed mode: kTabWords words, layout above (kTabH)
   const T* Ca[3];       // full mode, field geometry
   const T* Cb[3];
   const T* Db[3];       // full mode with mu

@@ -18,7 +18,7 @@ from .parity_util import TOL, assert_fields, run_pair
 
 pytestmark = pytest.mark.gpu
 
-IMPLS = [1]  # FDTD_OPT_STEP_IMPL: 1 = two-pass kernels (2 = fused E+H kernel, added when it lands)
+IMPLS = [1, 2]  # FDTD_OPT_STEP_IMPL: 1 = two-pass kernels, 2 = fused E+H kernel (TMA-staged, ping-pong field sets)
 
 
 @pytest.mark.parametrize("impl", IMPLS)
@@ -225,4 +225,32 @@ def test_error_codes_after_commit():
         s.set_materials_indexed(np.zeros(512, np.uint8), [[1.0, 1.0, -2.0]], [[0.0, 0.0, 0.0]])
     assert e.value.code == -1
     s.step(3)
-    assert s.step_count == 3 and s.launch_count == 6
+    assert s.step_count == 3 and s.launch_count == 6 and s.impl_name == "two_pass"
+
+
+@pytest.mark.parametrize("prec", [FDTD_F64, FDTD_F32])
+@pytest.mark.parametrize("kz", [0, 5, 16])
+def test_fused_tiles_chunks_and_odd_step_counts(prec, kz):
+    """The fused kernel over several x tiles (nx > 2 tiles of 128 / 64 cells with a ragged tail), several y tiles, z
+    chunks that do not divide nz, odd step counts (the state then lives in the second field set) and graph replay."""
+    from paper_2208_04371_b200 import FDTD_OPT_FUSED_KZ
+    w = W.random_box(21, nx=300, ny=21, nz=23, pml=(5, 6, 4, 3, 2, 5), steps=31, precision=prec)
+    o, s, rep = run_pair(w, 31, precision=prec, checkpoints=[1, 2, 3, 13, 31],
+                         options={FDTD_OPT_STEP_IMPL: 2, FDTD_OPT_FUSED_KZ: kz, FDTD_OPT_GRAPH_UNROLL: 3})
+    assert s.impl_name == "fused"
+    assert_fields(rep, prec)
+    assert max(rep["dft_err"]) <= (1e-11 if prec == FDTD_F64 else 1e-4)
+
+
+def test_fused_equals_two_pass_closely():
+    """Same arithmetic in the same order: the two step implementations agree to a few ulps of the field maximum."""
+    w = W.throughput_c3(div=8, steps=100, npml=6, nf=8)
+    out = []
+    for impl in (1, 2):
+        s = Solver.from_workload(w, options={FDTD_OPT_STEP_IMPL: impl})
+        s.step(100)
+        out.append([s.read_fields(c).cpu().numpy().astype(np.float64) for c in range(6)])
+        s.destroy()
+    for c in range(6):
+        scale = max(np.abs(out[0][c]).max(), 1e-300)
+        assert np.abs(out[0][c] - out[1][c]).max() / scale < 2e-6
