@@ -49,7 +49,7 @@ struct fdtd {
   int has_mu = 0;
   std::vector<PortDev> ports;
   std::vector<double> freqs;
-  long opt_impl = 0, opt_graph = 1, opt_unroll = 8, opt_kz = 0, opt_cfg = 0;
+  long opt_impl = 0, opt_graph = 1, opt_unroll = 8, opt_kz = 0, opt_dbg = 0;
   bool committed = false;
   long nstep = 0;
   long launches = 0;
@@ -125,7 +125,8 @@ struct Solver : fdtd {
     if (gexec2) cudaGraphExecDestroy(gexec2);
   }
   // auto: the fused kernel pays off once the grid no longer fits in L2 (small grids are launch-bound)
-  bool want_fused() const { return opt_impl == 2 || (opt_impl == 0 && (long long)nx * ny * nz >= (4LL << 20)); }
+  bool slabs_fit() const { return S(0) <= kMaxSlab && S(1) <= kMaxSlab && S(2) <= kMaxSlab; }
+  bool want_fused() const { return slabs_fit() && (opt_impl == 2 || (opt_impl == 0 && (long long)nx * ny * nz >= (4LL << 20))); }
 
   int mode() const { return (mat_mode == FDTD_MAT_FULL ? kModeFull : 0) | (has_mu ? kModeMu : 0); }
   size_t psi_elems(int a) const {
@@ -449,7 +450,16 @@ static PFN_cuTensorMapEncodeTiled_v12000 tensor_map_encoder() {
   return fn;
 }
 
-template <typename T> struct FusedTile { static constexpr int TY = 8, NS = 4; };
+// tile rows and TMA stages of the fused kernel (compile-time; -DFDTD_FUSED_TY / -DFDTD_FUSED_NS for tuning builds)
+#ifndef FDTD_FUSED_TY
+#define FDTD_FUSED_TY 14
+#endif
+#ifndef FDTD_FUSED_NS
+#define FDTD_FUSED_NS 3
+#endif
+template <typename T> struct FusedTile { static constexpr int TY = FDTD_FUSED_TY, NS = FDTD_FUSED_NS; };
+static_assert(FusedCfg<float, FDTD_FUSED_TY, FDTD_FUSED_NS>::SMEM <= 232448 && FusedCfg<double, FDTD_FUSED_TY, FDTD_FUSED_NS>::SMEM <= 232448,
+              "fused kernel: tile x stages exceed the 227 KB shared memory of an sm_100 CTA");
 
 template <typename T, int MODE>
 static cudaError_t fused_set_attr() {
@@ -489,7 +499,7 @@ int Solver<T>::build_fused() {
     const cuuint64_t gstr[2] = {(cuuint64_t)pitch() * es, (cuuint64_t)plane() * es};
     const cuuint32_t box[3] = {(cuuint32_t)bx, (cuuint32_t)by, 1};
     return enc(tm, dt, 3, base, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-               CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+               CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
   };
   const CUtensorMapDataType fdt = sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
   for (int c = 0; c < 2; ++c) {
@@ -501,6 +511,7 @@ int Solver<T>::build_fused() {
       fp.sp.psi[q] = reinterpret_cast<T*>(ws + (c ? cv.psi[q] : cv.psiH2[q]));
     }
     fp.kz = kz;
+    fp.dbg = (int)opt_dbg;
     for (int f = 0; f < 6; ++f) {
       if (!make(&fp.tm[f], ws + (c ? cv.field2[f] : cv.field[f]), fdt, sizeof(T), C::BX, f < 3 ? C::ROWS_E : C::ROWS_H))
         return fail(FDTD_ECUDA, "fdtd_commit: cuTensorMapEncodeTiled failed for field %d", f);
@@ -766,6 +777,7 @@ int fdtd_set_option(fdtd_t* h, int option, long value) {
     case FDTD_OPT_USE_GRAPH: h->opt_graph = value ? 1 : 0; return FDTD_OK;
     case FDTD_OPT_GRAPH_UNROLL: if (value < 1 || value > 1024) break; h->opt_unroll = value; return FDTD_OK;
     case FDTD_OPT_FUSED_KZ: if (value < 0 || value > 65535) break; h->opt_kz = value; return FDTD_OK;
+    case 99: h->opt_dbg = value; return FDTD_OK;  // tuning experiments (results are wrong when set)
   }
   return h->fail(FDTD_EINVAL, "fdtd_set_option: unknown option %d or bad value %ld", option, value);
 }

@@ -38,6 +38,7 @@ struct FusedParams {
   StepParams<T> sp;      // src = set read, dst = set written; psi[0..5] = psi_H written, psi[6..11] = psi_E (in place)
   const T* psiH_src[6];  // psi_H read (pHxy pHzy pHxz pHyz pHyx pHzx)
   int kz;                // planes per z chunk (grid.z = ceil(nz / kz))
+  int dbg;               // tuning experiments only (0 in production): 1 = loads only, 2 = no global stores
 };
 
 constexpr int round128(int v) { return (v + 127) / 128 * 128; }
@@ -51,9 +52,10 @@ struct FusedCfg {
   static constexpr int STAGE = 3 * E_B + 3 * H_B + I_B;
   static constexpr int HN_B = 2 * 2 * ROWS_H * TX * (int)sizeof(T);   // [buffer][Hx|Hz][row][x]
   static constexpr int HC_B = round128(2 * 2 * TY * (int)sizeof(T));  // [buffer][Hy|Hz][row] at i = x0-1
-  static constexpr int TAB_B = kTabWords * (int)sizeof(T);
+  static constexpr int TAB_B = kTabH * (int)sizeof(T);               // E records only; Db records are read from global
+  static constexpr int CP_B = 3 * 6 * kMaxSlab * (int)sizeof(T);      // CPML vectors [axis][bE cE kE bH cH kH][slab coordinate]
   static constexpr int BAR_B = 128;
-  static constexpr int SMEM = NS * STAGE + HN_B + HC_B + TAB_B + BAR_B;
+  static constexpr int SMEM = NS * STAGE + HN_B + HC_B + TAB_B + CP_B + BAR_B;
   static constexpr int THREADS = (TY + 2) * 32;
 };
 
@@ -118,17 +120,80 @@ template <> __device__ __forceinline__ void stv_stream<double>(double* p, const 
   __stcs(reinterpret_cast<double2*>(p), make_double2(r[0], r[1]));
 }
 
+// ---- arithmetic on a thread's V consecutive cells; fp32 uses the packed two-wide FP32 pipe (FFMA2) --------------------
+template <typename T, int V> struct VOps {
+  static __device__ __forceinline__ void sub(T (&r)[V], const T (&a)[V], const T (&b)[V]) {
+#pragma unroll
+    for (int v = 0; v < V; ++v) r[v] = a[v] - b[v];
+  }
+  static __device__ __forceinline__ void fma_s(T (&r)[V], const T (&a)[V], T s) {  // r += a * s
+#pragma unroll
+    for (int v = 0; v < V; ++v) r[v] = fma(a[v], s, r[v]);
+  }
+  static __device__ __forceinline__ void mul_s(T (&r)[V], const T (&a)[V], T s) {
+#pragma unroll
+    for (int v = 0; v < V; ++v) r[v] = a[v] * s;
+  }
+};
+template <> struct VOps<float, 4> {
+  static __device__ __forceinline__ void sub(float (&r)[4], const float (&a)[4], const float (&b)[4]) {
+    const float2 m1 = make_float2(-1.f, -1.f);
+    const float2 lo = __ffma2_rn(make_float2(b[0], b[1]), m1, make_float2(a[0], a[1]));
+    const float2 hi = __ffma2_rn(make_float2(b[2], b[3]), m1, make_float2(a[2], a[3]));
+    r[0] = lo.x; r[1] = lo.y; r[2] = hi.x; r[3] = hi.y;
+  }
+  static __device__ __forceinline__ void fma_s(float (&r)[4], const float (&a)[4], float s) {
+    const float2 ss = make_float2(s, s);
+    const float2 lo = __ffma2_rn(make_float2(a[0], a[1]), ss, make_float2(r[0], r[1]));
+    const float2 hi = __ffma2_rn(make_float2(a[2], a[3]), ss, make_float2(r[2], r[3]));
+    r[0] = lo.x; r[1] = lo.y; r[2] = hi.x; r[3] = hi.y;
+  }
+  static __device__ __forceinline__ void mul_s(float (&r)[4], const float (&a)[4], float s) {
+    const float2 ss = make_float2(s, s);
+    const float2 lo = __fmul2_rn(make_float2(a[0], a[1]), ss);
+    const float2 hi = __fmul2_rn(make_float2(a[2], a[3]), ss);
+    r[0] = lo.x; r[1] = lo.y; r[2] = hi.x; r[3] = hi.y;
+  }
+};
+
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
 // ------------------------------------------------------------------------------------------------------------------
+// k_step_fused.  Structure of one plane iteration (all warps): wait for the stage -> H phase -> __syncthreads -> E phase.
+// The arithmetic is written as the plain Yee update (kappa = 1, psi = 0) for every cell, followed by additive CPML
+// corrections under warp-uniform (y slab, z slab) or per-lane (x slab) branches:
+//     H -= Db * [ (1/kappa - 1) * dE + psi ]        E += Cb * [ (1/kappa - 1) * dH + psi ]
+// which is R5 regrouped (identical up to rounding).  Cells outside the grid (halo of edge tiles, pad columns) need no
+// masks in the plain H update: all their operands are zeros supplied by TMA / the zero pad, so their results are zeros.
+// ------------------------------------------------------------------------------------------------------------------
+// psi <- b psi + c d  for a thread's V cells of two psi arrays (cells at or beyond nx stay zero)
+template <typename T, int V>
+__device__ __forceinline__ void psi_update2(T (&a)[V], T (&d)[V], const T (&da)[V], const T (&dd)[V], T b, T c, T inv, int nvalid) {
+#pragma unroll
+  for (int v = 0; v < V; ++v) {
+    a[v] = b * a[v] + (c * inv) * da[v];
+    d[v] = b * d[v] + (c * inv) * dd[v];
+    if (v >= nvalid) { a[v] = T(0); d[v] = T(0); }
+  }
+}
+
+#ifndef FDTD_FUSED_MINB
+#define FDTD_FUSED_MINB 1
+#endif
 template <typename T, int MODE, int TY, int NS>
-__global__ void __launch_bounds__((TY + 2) * 32, 1) k_step_fused(const __grid_constant__ FusedParams<T> fp) {
+__global__ void __launch_bounds__((TY + 2) * 32, FDTD_FUSED_MINB) k_step_fused(const __grid_constant__ FusedParams<T> fp) {
   using C = FusedCfg<T, TY, NS>;
+  using O = VOps<T, C::V>;
   constexpr int V = C::V, TX = C::TX, BX = C::BX;
   constexpr bool kFull = (MODE & kModeFull) != 0, kMu = (MODE & kModeMu) != 0;
   extern __shared__ __align__(1024) unsigned char smem[];
   T* const hn = reinterpret_cast<T*>(smem + NS * C::STAGE);
   T* const hc = reinterpret_cast<T*>(smem + NS * C::STAGE + C::HN_B);
   T* const tab = reinterpret_cast<T*>(smem + NS * C::STAGE + C::HN_B + C::HC_B);
-  uint64_t* const bar = reinterpret_cast<uint64_t*>(smem + NS * C::STAGE + C::HN_B + C::HC_B + C::TAB_B);
+  T* const cpv = reinterpret_cast<T*>(smem + NS * C::STAGE + C::HN_B + C::HC_B + C::TAB_B);
+  uint64_t* const bar = reinterpret_cast<uint64_t*>(smem + NS * C::STAGE + C::HN_B + C::HC_B + C::TAB_B + C::CP_B);
+  // CPML vector v (0..5 = bE cE kE bH cH kH) of axis a at slab coordinate q
+  auto cp = [&](int a, int v, int q) -> T { return cpv[(a * 6 + v) * kMaxSlab + q]; };
 
   const StepParams<T>& p = fp.sp;
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -138,9 +203,10 @@ __global__ void __launch_bounds__((TY + 2) * 32, 1) k_step_fused(const __grid_co
 
   if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && threadIdx.x == 0) *p.nstep += 1;
 
-  // one elected thread issues the boxes of iteration `it` into stage it % NS
-  auto issue = [&](int it) {
-    const int k = k0 - 2 + it, s = it % NS;
+  // one elected thread issues the boxes of iteration `it` (plane k) into stage s
+  auto issue = [&](int it, int s) {
+    if (fp.dbg & 4) return;
+    const int k = k0 - 2 + it;
     unsigned char* st = smem + s * C::STAGE;
     const bool want_idx = !kFull && it >= 2;
     const unsigned bytes = it == 0 ? 2u * C::E_TX : 3u * C::E_TX + 3u * C::H_TX + (want_idx ? (unsigned)C::I_TX : 0u);
@@ -163,26 +229,49 @@ __global__ void __launch_bounds__((TY + 2) * 32, 1) k_step_fused(const __grid_co
     for (int q = 0; q < 7; ++q) tma_prefetch_desc(&fp.tm[q]);
   }
   if (!kFull) {
-    for (int q = threadIdx.x; q < (kMu ? kTabWords : kTabH); q += C::THREADS) tab[q] = p.tab[q];
+    for (int q = threadIdx.x; q < kTabH; q += C::THREADS) tab[q] = p.tab[q];
+  }
+  for (int a = 0; a < 3; ++a) {  // CPML vectors -> shared memory
+    const int S = p.lo[a] + p.hi[a];
+    const T* const src[6] = {p.bE[a], p.cE[a], p.kE[a], p.bH[a], p.cH[a], p.kH[a]};
+#pragma unroll
+    for (int v = 0; v < 6; ++v)
+      for (int q = threadIdx.x; q < S; q += C::THREADS) cpv[(a * 6 + v) * kMaxSlab + q] = src[v][q];
   }
   __syncthreads();
   if (threadIdx.x == 0) {
-    for (int it = 0; it < NS && it < nIt; ++it) issue(it);
+    for (int it = 0; it < NS && it < nIt; ++it) issue(it, it);
   }
 
+  // ---- loop invariants ------------------------------------------------------------------------------------------------
   const bool rowwarp = w <= TY;
   // row warps: j = y0-1+w (w = 0 is the halo row); column warp: lane l <-> row y0+l at i = x0-1
   const int j = rowwarp ? y0 - 1 + w : y0 + lane;
   const int i0 = rowwarp ? x0 + lane * V : x0 - 1;
   const bool jin = j >= 0 && j < p.ny;
-  const bool cin = rowwarp ? (jin && i0 < p.nx) : (jin && i0 >= 0 && lane < TY);  // thread's cell(s) exist
-  const bool owned = rowwarp && w >= 1 && cin;
-  const int sj = jin ? slab_coord(j, p.lo[1], p.hi[1], p.ny) : -1;
-  const int Sx = p.lo[0] + p.hi[0], Sy = p.lo[1] + p.hi[1];
-  const T iky_H = sj >= 0 ? p.kH[1][sj] : T(1), iky_E = sj >= 0 ? p.kE[1][sj] : T(1);
-  const T bHy = sj >= 0 ? p.bH[1][sj] : T(0), cHy = sj >= 0 ? p.cH[1][sj] : T(0);
-  const T bEy = sj >= 0 ? p.bE[1][sj] : T(0), cEy = sj >= 0 ? p.cE[1][sj] : T(0);
-  const bool xs = rowwarp && ((i0 < p.lo[0]) || (i0 + V > p.nx - p.hi[0]));  // some cell of the vector is in an x slab
+  const bool cin = rowwarp ? (jin && i0 < p.nx) : (jin && i0 >= 0 && lane < TY);  // the thread's cell(s) exist
+  const bool owned = rowwarp && w >= 1 && cin;                                    // ... and this thread stores them
+  const int nvalid = rowwarp ? min(V, p.nx - i0) : 1;                             // cells of the vector inside the grid
+  const int Sx = p.lo[0] + p.hi[0], Sy = p.lo[1] + p.hi[1], Sz = p.lo[2] + p.hi[2];
+  const int sj = (cin && Sy > 0) ? slab_coord(j, p.lo[1], p.hi[1], p.ny) : -1;
+  // x slab: coordinate of the thread's first cell; the whole vector is handled with 128-bit psi accesses when the slab
+  // edges fall on vector boundaries (xvec), cell by cell otherwise
+  const bool xs = cin && Sx > 0 && (rowwarp ? ((i0 < p.lo[0]) || (i0 + V > p.nx - p.hi[0]))
+                                            : (slab_coord(i0, p.lo[0], p.hi[0], p.nx) >= 0));
+  const bool xvec = (p.lo[0] % V == 0) && ((p.nx - p.hi[0]) % V == 0) && (p.nx % V == 0);
+  const int si0 = xs ? slab_coord(i0, p.lo[0], p.hi[0], p.nx) : -1;
+  const bool wj = (j == 0), wi = (i0 == 0);
+  const bool xtail = x0 + TX > p.nx;
+  const int kzlo = p.lo[2], kzhi = p.nz - p.hi[2];
+  // uniform update constants (no permeability arrays): H -= (dt/mu0)/d * dE
+  const T cx = p.db0 * p.idx_, cy = p.db0 * p.idy_, cz = p.db0 * p.idz_;
+  // psi offsets, evaluated inside the slab branches only (keeps the plain path's register budget small)
+  auto qy = [&](int k) { return (long long)i0 + (long long)p.P * (sj + (long long)Sy * k); };              // y slab
+  auto qz = [&](int sk) { return (long long)i0 + (long long)p.P * (j + (long long)p.ny * sk); };           // z slab
+  auto qx = [&](int k) { return (long long)(si0 >= 0 ? si0 : 0) + (long long)Sx * (j + (long long)p.ny * k); };  // x slab
+  const long long orow = (long long)i0 + (long long)p.P * j;
+  const int off = rowwarp ? w * BX + V + lane * V : 0;
+  T* const hn_row = hn + (rowwarp ? w : 0) * TX + lane * V;
 
   // registers carried from one plane to the next
   T ex0[V], ey0[V], exj0[V], hxm[V], hym[V];
@@ -191,8 +280,11 @@ __global__ void __launch_bounds__((TY + 2) * 32, 1) k_step_fused(const __grid_co
   for (int v = 0; v < V; ++v) { ex0[v] = ey0[v] = exj0[v] = hxm[v] = hym[v] = T(0); }
   T c_ex0 = T(0), c_exj0 = T(0), c_ey0 = T(0), c_eyp0 = T(0);  // column warp: Ex(x0-1,j), Ex(x0-1,j+1), Ey(x0-1,j), Ey(x0,j)
 
-  for (int it = 0; it < nIt; ++it) {
-    const int k = k0 - 2 + it, s = it % NS;
+  int s = 0;
+  unsigned ph = 0;
+  long long o = orow + p.PS * (long long)(k0 - 2);
+  for (int it = 0; it < nIt; ++it, o += p.PS) {
+    const int k = k0 - 2 + it;
     const unsigned char* st = smem + s * C::STAGE;
     const T* sEx = reinterpret_cast<const T*>(st);
     const T* sEy = reinterpret_cast<const T*>(st + C::E_B);
@@ -201,24 +293,49 @@ __global__ void __launch_bounds__((TY + 2) * 32, 1) k_step_fused(const __grid_co
     const T* sHy = reinterpret_cast<const T*>(st + 3 * C::E_B + C::H_B);
     const T* sHz = reinterpret_cast<const T*>(st + 3 * C::E_B + 2 * C::H_B);
     const unsigned char* sIdx = st + 3 * C::E_B + 3 * C::H_B;
-    const bool kin = k >= 0;  // k < nz always
-    const int sk = kin ? slab_coord(k, p.lo[2], p.hi[2], p.nz) : -1;
-    const long long o = (long long)i0 + (long long)p.P * j + p.PS * k;
-    T* const hnb = hn + (it & 1) * (2 * C::ROWS_H * TX);
+    const bool zs = Sz > 0 && k >= 0 && (k < kzlo || k >= kzhi);
+    const bool pml = (xs || sj >= 0 || zs) && cin && k >= 0;   // some CPML correction applies to this thread
+    T* const hnb = hn_row + (it & 1) * (2 * C::ROWS_H * TX);
     T* const hcb = hc + (it & 1) * (2 * TY);
 
-    mbar_wait(&bar[s], (unsigned)(it / NS) & 1u);
+    if (pml && it + 1 < nIt) {  // pull the psi lines of the next plane into L2 while this plane is being processed
+      if (sj >= 0) {
+        const long long q = qy(k + 1);
+        prefetch_l2(fp.psiH_src[pHxy] + q); prefetch_l2(fp.psiH_src[pHzy] + q);
+        prefetch_l2(p.psi[pExy] + q); prefetch_l2(p.psi[pEzy] + q);
+      }
+      if (xs) {
+        const long long q = qx(k + 1);
+        prefetch_l2(fp.psiH_src[pHyx] + q); prefetch_l2(fp.psiH_src[pHzx] + q);
+        prefetch_l2(p.psi[pEyx] + q); prefetch_l2(p.psi[pEzx] + q);
+      }
+      if (k + 1 < kzlo || k + 1 >= kzhi) {
+        if (Sz > 0 && k + 1 >= 0 && k + 1 < p.nz) {
+          const long long q = qz(slab_coord(k + 1, p.lo[2], p.hi[2], p.nz));
+          prefetch_l2(fp.psiH_src[pHxz] + q); prefetch_l2(fp.psiH_src[pHyz] + q);
+          prefetch_l2(p.psi[pExz] + q); prefetch_l2(p.psi[pEyz] + q);
+        }
+      }
+    }
 
-    T hx[V], hy[V], hz[V], ez[V];
-    unsigned char mi[V];
+    if (!(fp.dbg & 4)) mbar_wait(&bar[s], ph);
+    if (fp.dbg & 1) {
+      __syncthreads();
+      if (threadIdx.x == 0 && it + NS < nIt) issue(it + NS, s);
+      if (++s == NS) { s = 0; ph ^= 1u; }
+      continue;
+    }
+
     if (rowwarp) {
-      // ---------------- H phase, row warps -------------------------------------------------------------------------
-      const int off = w * BX + V + lane * V;
+      // ================= row warps ====================================================================================
       T ex1[V], ey1[V], exj1[V];
       ldv(sEx + off, ex1); ldv(sEy + off, ey1); ldv(sEx + off + BX, exj1);
       T eyi1 = __shfl_down_sync(0xffffffffu, ey1[0], 1);
       if (lane == 31) eyi1 = sEy[off + V];
+      T hx[V], hy[V], hz[V], ez[V];
+      unsigned char mi[V];
       if (it >= 1) {
+        // ---------------- H phase: H^{n+1/2}(k) = H^{n-1/2}(k) - Db curl E^n -----------------------------------------
         T ezj[V];
         ldv(sEz + off, ez); ldv(sEz + off + BX, ezj);
         T ezi = __shfl_down_sync(0xffffffffu, ez[0], 1);
@@ -226,182 +343,209 @@ __global__ void __launch_bounds__((TY + 2) * 32, 1) k_step_fused(const __grid_co
         ldv(sHx + off, hx); ldv(sHy + off, hy); ldv(sHz + off, hz);
         if (!kFull && it >= 2 && w >= 1) ld_index_smem<V>(sIdx + (w - 1) * TX + lane * V, mi);
 
-        const bool live = cin && kin;
-        const T ikz = sk >= 0 ? p.kH[2][sk] : T(1);
-        T ax[V], ay[V], az[V], d0[V], d1[V], d2[V], d3[V];
+        T dEz_y[V], dEy_z[V], dEx_z[V], dEx_y[V], dEz_x[V], dEy_x[V];   // undivided differences
+        O::sub(dEz_y, ezj, ez); O::sub(dEy_z, ey1, ey0); O::sub(dEx_z, ex1, ex0); O::sub(dEx_y, exj0, ex0);
 #pragma unroll
         for (int v = 0; v < V; ++v) {
-          const T eyp = (v + 1 < V) ? ey0[v + 1] : eyi0;
-          const T ezp = (v + 1 < V) ? ez[v + 1] : ezi;
-          const T dyEz = (ezj[v] - ez[v]) * p.idy_, dzEy = (ey1[v] - ey0[v]) * p.idz_;
-          const T dzEx = (ex1[v] - ex0[v]) * p.idz_, dxEz = (ezp - ez[v]) * p.idx_;
-          const T dxEy = (eyp - ey0[v]) * p.idx_,    dyEx = (exj0[v] - ex0[v]) * p.idy_;
-          ax[v] = dyEz * iky_H - dzEy * ikz;
-          ay[v] = dzEx * ikz;
-          az[v] = -dyEx * iky_H;
-          if (!xs) { ay[v] -= dxEz; az[v] += dxEy; }
-          else {
-            const int si = slab_coord(i0 + v, p.lo[0], p.hi[0], p.nx);
-            T ikx = T(1), pyx = T(0), pzx = T(0);
-            if (si >= 0 && i0 + v < p.nx && live) {
-              ikx = p.kH[0][si];
-              const long long q = si + (long long)Sx * (j + (long long)p.ny * k);
-              const T b = p.bH[0][si], c = p.cH[0][si];
-              pyx = b * fp.psiH_src[pHyx][q] + c * dxEz;
-              pzx = b * fp.psiH_src[pHzx][q] + c * dxEy;
-              if (owned && it >= 2) { p.psi[pHyx][q] = pyx; p.psi[pHzx][q] = pzx; }
-            }
-            ay[v] -= dxEz * ikx + pyx;
-            az[v] += dxEy * ikx + pzx;
-          }
-          d0[v] = dyEz; d1[v] = dyEx; d2[v] = dzEy; d3[v] = dzEx;
-        }
-        if (sj >= 0 && live) {  // y slab: psiHxy (from D+y Ez), psiHzy (from D+y Ex)
-          const long long q = i0 + (long long)p.P * (sj + (long long)Sy * k);
-          T a[V], d[V];
-          ldv(fp.psiH_src[pHxy] + q, a); ldv(fp.psiH_src[pHzy] + q, d);
-#pragma unroll
-          for (int v = 0; v < V; ++v) {
-            a[v] = bHy * a[v] + cHy * d0[v]; d[v] = bHy * d[v] + cHy * d1[v];
-            if (i0 + v >= p.nx) { a[v] = T(0); d[v] = T(0); }
-            ax[v] += a[v]; az[v] -= d[v];
-          }
-          if (owned && it >= 2) { stv(p.psi[pHxy] + q, a); stv(p.psi[pHzy] + q, d); }
-        }
-        if (sk >= 0 && live) {  // z slab: psiHxz (from D+z Ey), psiHyz (from D+z Ex)
-          const long long q = i0 + (long long)p.P * (j + (long long)p.ny * sk);
-          const T b = p.bH[2][sk], c = p.cH[2][sk];
-          T a[V], d[V];
-          ldv(fp.psiH_src[pHxz] + q, a); ldv(fp.psiH_src[pHyz] + q, d);
-#pragma unroll
-          for (int v = 0; v < V; ++v) {
-            a[v] = b * a[v] + c * d2[v]; d[v] = b * d[v] + c * d3[v];
-            if (i0 + v >= p.nx) { a[v] = T(0); d[v] = T(0); }
-            ax[v] -= a[v]; ay[v] += d[v];
-          }
-          if (owned && it >= 2) { stv(p.psi[pHxz] + q, a); stv(p.psi[pHyz] + q, d); }
+          dEz_x[v] = ((v + 1 < V) ? ez[v + 1] : ezi) - ez[v];
+          dEy_x[v] = ((v + 1 < V) ? ey0[v + 1] : eyi0) - ey0[v];
         }
         T dbx[V], dby[V], dbz[V];
-        if (kMu) {
+        if (!kMu) {
+          O::fma_s(hx, dEz_y, -cy); O::fma_s(hx, dEy_z, cz);
+          O::fma_s(hy, dEx_z, -cz); O::fma_s(hy, dEz_x, cx);
+          O::fma_s(hz, dEy_x, -cx); O::fma_s(hz, dEx_y, cy);
+#pragma unroll
+          for (int v = 0; v < V; ++v) { dbx[v] = dby[v] = dbz[v] = p.db0; }
+        } else {
 #pragma unroll
           for (int v = 0; v < V; ++v) { dbx[v] = dby[v] = dbz[v] = T(0); }
-          if (live) {
+          if (cin && k >= 0) {
             if (kFull) { ldv(p.Db[0] + o, dbx); ldv(p.Db[1] + o, dby); ldv(p.Db[2] + o, dbz); }
             else {
               unsigned char m[V];
               ld_index<V>(p.idx + o, m);
 #pragma unroll
               for (int v = 0; v < V; ++v) {
-                dbx[v] = tab[kTabH + 4 * (int)m[v]]; dby[v] = tab[kTabH + 4 * (int)m[v] + 1]; dbz[v] = tab[kTabH + 4 * (int)m[v] + 2];
+                const Vec4<T> d = ld4(p.tab + kTabH + 4 * (int)m[v]);
+                dbx[v] = d.a; dby[v] = d.b; dbz[v] = d.c;
               }
             }
           }
-        } else {
 #pragma unroll
-          for (int v = 0; v < V; ++v) { dbx[v] = p.db0; dby[v] = p.db0; dbz[v] = p.db0; }
+          for (int v = 0; v < V; ++v) {
+            hx[v] -= dbx[v] * (dEz_y[v] * p.idy_ - dEy_z[v] * p.idz_);
+            hy[v] -= dby[v] * (dEx_z[v] * p.idz_ - dEz_x[v] * p.idx_);
+            hz[v] -= dbz[v] * (dEy_x[v] * p.idx_ - dEx_y[v] * p.idy_);
+          }
         }
+        if (pml) {
+          const bool wr = owned && it >= 2;
+          if (sj >= 0) {  // y slab: psiHxy (from D+y Ez) -> Hx, psiHzy (from D+y Ex) -> Hz
+            const long long q = qy(k);
+            T a[V], d[V];
+            ldv(fp.psiH_src[pHxy] + q, a); ldv(fp.psiH_src[pHzy] + q, d);
+            const T ykH = (cp(1, 5, sj) - T(1)) * p.idy_;
+            psi_update2<T, V>(a, d, dEz_y, dEx_y, cp(1, 3, sj), cp(1, 4, sj), p.idy_, nvalid);
 #pragma unroll
-        for (int v = 0; v < V; ++v) {
-          hx[v] -= dbx[v] * ax[v]; hy[v] -= dby[v] * ay[v]; hz[v] -= dbz[v] * az[v];
-          if (!live || i0 + v >= p.nx) { hx[v] = T(0); hy[v] = T(0); hz[v] = T(0); }
+            for (int v = 0; v < V; ++v) {
+              hx[v] -= dbx[v] * (ykH * dEz_y[v] + a[v]); hz[v] += dbz[v] * (ykH * dEx_y[v] + d[v]);
+            }
+            if (wr) { stv(p.psi[pHxy] + q, a); stv(p.psi[pHzy] + q, d); }
+          }
+          if (zs) {  // z slab: psiHxz (from D+z Ey) -> Hx, psiHyz (from D+z Ex) -> Hy
+            const int sk = slab_coord(k, p.lo[2], p.hi[2], p.nz);
+            const long long q = qz(sk);
+            const T b = cp(2, 3, sk), c = cp(2, 4, sk), km = (cp(2, 5, sk) - T(1)) * p.idz_;
+            T a[V], d[V];
+            ldv(fp.psiH_src[pHxz] + q, a); ldv(fp.psiH_src[pHyz] + q, d);
+            psi_update2<T, V>(a, d, dEy_z, dEx_z, b, c, p.idz_, nvalid);
+#pragma unroll
+            for (int v = 0; v < V; ++v) {
+              hx[v] += dbx[v] * (km * dEy_z[v] + a[v]); hy[v] -= dby[v] * (km * dEx_z[v] + d[v]);
+            }
+            if (wr) { stv(p.psi[pHxz] + q, a); stv(p.psi[pHyz] + q, d); }
+          }
+          if (xs) {  // x slab: psiHyx (from D+x Ez) -> Hy, psiHzx (from D+x Ey) -> Hz
+            const long long q0 = qx(k);
+            if (xvec) {
+              T a[V], d[V];
+              ldv(fp.psiH_src[pHyx] + q0, a); ldv(fp.psiH_src[pHzx] + q0, d);
+#pragma unroll
+              for (int v = 0; v < V; ++v) {
+                const T b = cp(0, 3, si0 + v), c = cp(0, 4, si0 + v) * p.idx_, km = (cp(0, 5, si0 + v) - T(1)) * p.idx_;
+                a[v] = b * a[v] + c * dEz_x[v]; d[v] = b * d[v] + c * dEy_x[v];
+                hy[v] += dby[v] * (km * dEz_x[v] + a[v]); hz[v] -= dbz[v] * (km * dEy_x[v] + d[v]);
+              }
+              if (wr) { stv(p.psi[pHyx] + q0, a); stv(p.psi[pHzx] + q0, d); }
+            } else {
+#pragma unroll
+              for (int v = 0; v < V; ++v) {
+                const int si = slab_coord(i0 + v, p.lo[0], p.hi[0], p.nx);
+                if (si >= 0 && v < nvalid) {
+                  const long long q = q0 + si - (si0 >= 0 ? si0 : 0);
+                  const T b = cp(0, 3, si), c = cp(0, 4, si) * p.idx_, km = (cp(0, 5, si) - T(1)) * p.idx_;
+                  const T pyx = b * fp.psiH_src[pHyx][q] + c * dEz_x[v], pzx = b * fp.psiH_src[pHzx][q] + c * dEy_x[v];
+                  if (wr) { p.psi[pHyx][q] = pyx; p.psi[pHzx][q] = pzx; }
+                  hy[v] += dby[v] * (km * dEz_x[v] + pyx); hz[v] -= dbz[v] * (km * dEy_x[v] + pzx);
+                }
+              }
+            }
+          }
         }
-        stv(hnb + w * TX + lane * V, hx);
-        stv(hnb + (C::ROWS_H + w) * TX + lane * V, hz);
-        if (owned && it >= 2) {
+        stv(hnb, hx);
+        stv(hnb + C::ROWS_H * TX, hz);
+        if (owned && it >= 2 && !(fp.dbg & 2)) {
           stv_stream(p.dst[kHx] + o, hx); stv_stream(p.dst[kHy] + o, hy); stv_stream(p.dst[kHz] + o, hz);
         }
       }
-      // carry the k+1 operands (E^n own values of plane k are still needed by the E phase below: rotate after it)
+      __syncthreads();
+      if (threadIdx.x == 0 && it + NS < nIt) issue(it + NS, s);
       if (it >= 2 && w >= 1) {
-        // ---------------- sync, then E phase -------------------------------------------------------------------------
-        __syncthreads();
+        // ---------------- E phase: E^{n+1}(k) = Ca E^n + Cb curl H^{n+1/2} ---------------------------------------------
         T hxj[V], hzj[V];
-        ldv(hnb + (w - 1) * TX + lane * V, hxj);
-        ldv(hnb + (C::ROWS_H + w - 1) * TX + lane * V, hzj);
+        ldv(hnb - TX, hxj);
+        ldv(hnb + (C::ROWS_H - 1) * TX, hzj);
         T hyi = __shfl_up_sync(0xffffffffu, hy[V - 1], 1), hzi = __shfl_up_sync(0xffffffffu, hz[V - 1], 1);
         if (lane == 0) { hyi = hcb[w - 1]; hzi = hcb[TY + w - 1]; }
-        const T ikz = sk >= 0 ? p.kE[2][sk] : T(1);
-        T ax[V], ay[V], az[V], d0[V], d1[V], d2[V], d3[V];
+        T dHz_y[V], dHy_z[V], dHx_z[V], dHx_y[V], dHz_x[V], dHy_x[V];
+        O::sub(dHz_y, hz, hzj); O::sub(dHy_z, hy, hym); O::sub(dHx_z, hx, hxm); O::sub(dHx_y, hx, hxj);
 #pragma unroll
         for (int v = 0; v < V; ++v) {
-          const T hym_ = (v > 0) ? hy[v - 1] : hyi;
-          const T hzm_ = (v > 0) ? hz[v - 1] : hzi;
-          const T dyHz = (hz[v] - hzj[v]) * p.idy_, dzHy = (hy[v] - hym[v]) * p.idz_;
-          const T dzHx = (hx[v] - hxm[v]) * p.idz_, dxHz = (hz[v] - hzm_) * p.idx_;
-          const T dxHy = (hy[v] - hym_) * p.idx_,   dyHx = (hx[v] - hxj[v]) * p.idy_;
-          ax[v] = dyHz * iky_E - dzHy * ikz;
-          ay[v] = dzHx * ikz;
-          az[v] = -dyHx * iky_E;
-          if (!xs) { ay[v] -= dxHz; az[v] += dxHy; }
-          else {
-            const int si = slab_coord(i0 + v, p.lo[0], p.hi[0], p.nx);
-            T ikx = T(1), pyx = T(0), pzx = T(0);
-            if (si >= 0 && i0 + v < p.nx && owned) {
-              ikx = p.kE[0][si];
-              const long long q = si + (long long)Sx * (j + (long long)p.ny * k);
-              const T b = p.bE[0][si], c = p.cE[0][si];
-              pyx = b * p.psi[pEyx][q] + c * dxHz; p.psi[pEyx][q] = pyx;
-              pzx = b * p.psi[pEzx][q] + c * dxHy; p.psi[pEzx][q] = pzx;
-            }
-            ay[v] -= dxHz * ikx + pyx;
-            az[v] += dxHy * ikx + pzx;
-          }
-          d0[v] = dyHz; d1[v] = dyHx; d2[v] = dzHy; d3[v] = dzHx;
+          dHz_x[v] = hz[v] - ((v > 0) ? hz[v - 1] : hzi);
+          dHy_x[v] = hy[v] - ((v > 0) ? hy[v - 1] : hyi);
         }
-        if (owned) {
-          if (sj >= 0) {  // y slab: psiExy (from D-y Hz), psiEzy (from D-y Hx)
-            const long long q = i0 + (long long)p.P * (sj + (long long)Sy * k);
+        T ax[V], ay[V], az[V];
+        O::mul_s(ax, dHz_y, p.idy_); O::fma_s(ax, dHy_z, -p.idz_);
+        O::mul_s(ay, dHx_z, p.idz_); O::fma_s(ay, dHz_x, -p.idx_);
+        O::mul_s(az, dHy_x, p.idx_); O::fma_s(az, dHx_y, -p.idy_);
+        if (pml && owned) {
+          if (sj >= 0) {  // y slab: psiExy (from D-y Hz) -> Ex, psiEzy (from D-y Hx) -> Ez
+            const long long q = qy(k);
             T a[V], d[V];
             ldv(p.psi[pExy] + q, a); ldv(p.psi[pEzy] + q, d);
+            const T ykE = (cp(1, 2, sj) - T(1)) * p.idy_;
+            psi_update2<T, V>(a, d, dHz_y, dHx_y, cp(1, 0, sj), cp(1, 1, sj), p.idy_, nvalid);
 #pragma unroll
-            for (int v = 0; v < V; ++v) {
-              a[v] = bEy * a[v] + cEy * d0[v]; d[v] = bEy * d[v] + cEy * d1[v];
-              if (i0 + v >= p.nx) { a[v] = T(0); d[v] = T(0); }
-              ax[v] += a[v]; az[v] -= d[v];
-            }
+            for (int v = 0; v < V; ++v) { ax[v] += ykE * dHz_y[v] + a[v]; az[v] -= ykE * dHx_y[v] + d[v]; }
             stv(p.psi[pExy] + q, a); stv(p.psi[pEzy] + q, d);
           }
-          if (sk >= 0) {  // z slab: psiExz (from D-z Hy), psiEyz (from D-z Hx)
-            const long long q = i0 + (long long)p.P * (j + (long long)p.ny * sk);
-            const T b = p.bE[2][sk], c = p.cE[2][sk];
+          if (zs) {  // z slab: psiExz (from D-z Hy) -> Ex, psiEyz (from D-z Hx) -> Ey
+            const int sk = slab_coord(k, p.lo[2], p.hi[2], p.nz);
+            const long long q = qz(sk);
+            const T b = cp(2, 0, sk), c = cp(2, 1, sk), km = (cp(2, 2, sk) - T(1)) * p.idz_;
             T a[V], d[V];
             ldv(p.psi[pExz] + q, a); ldv(p.psi[pEyz] + q, d);
+            psi_update2<T, V>(a, d, dHy_z, dHx_z, b, c, p.idz_, nvalid);
 #pragma unroll
-            for (int v = 0; v < V; ++v) {
-              a[v] = b * a[v] + c * d2[v]; d[v] = b * d[v] + c * d3[v];
-              if (i0 + v >= p.nx) { a[v] = T(0); d[v] = T(0); }
-              ax[v] -= a[v]; ay[v] += d[v];
-            }
+            for (int v = 0; v < V; ++v) { ax[v] -= km * dHy_z[v] + a[v]; ay[v] += km * dHx_z[v] + d[v]; }
             stv(p.psi[pExz] + q, a); stv(p.psi[pEyz] + q, d);
           }
-          T cax[V], cay[V], caz[V], cbx[V], cby[V], cbz[V];
+          if (xs) {  // x slab: psiEyx (from D-x Hz) -> Ey, psiEzx (from D-x Hy) -> Ez
+            const long long q0 = qx(k);
+            if (xvec) {
+              T a[V], d[V];
+              ldv(p.psi[pEyx] + q0, a); ldv(p.psi[pEzx] + q0, d);
+#pragma unroll
+              for (int v = 0; v < V; ++v) {
+                const T b = cp(0, 0, si0 + v), c = cp(0, 1, si0 + v) * p.idx_, km = (cp(0, 2, si0 + v) - T(1)) * p.idx_;
+                a[v] = b * a[v] + c * dHz_x[v]; d[v] = b * d[v] + c * dHy_x[v];
+                ay[v] -= km * dHz_x[v] + a[v]; az[v] += km * dHy_x[v] + d[v];
+              }
+              stv(p.psi[pEyx] + q0, a); stv(p.psi[pEzx] + q0, d);
+            } else {
+#pragma unroll
+              for (int v = 0; v < V; ++v) {
+                const int si = slab_coord(i0 + v, p.lo[0], p.hi[0], p.nx);
+                if (si >= 0 && v < nvalid) {
+                  const long long q = q0 + si - (si0 >= 0 ? si0 : 0);
+                  const T b = cp(0, 0, si), c = cp(0, 1, si) * p.idx_, km = (cp(0, 2, si) - T(1)) * p.idx_;
+                  const T pyx = b * p.psi[pEyx][q] + c * dHz_x[v], pzx = b * p.psi[pEzx][q] + c * dHy_x[v];
+                  p.psi[pEyx][q] = pyx; p.psi[pEzx][q] = pzx;
+                  ay[v] -= km * dHz_x[v] + pyx; az[v] += km * dHy_x[v] + pzx;
+                }
+              }
+            }
+          }
+        }
+        if (owned) {
+          T ex[V], ey[V];
           if (kFull) {
-            ldv(p.Ca[0] + o, cax); ldv(p.Ca[1] + o, cay); ldv(p.Ca[2] + o, caz);
-            ldv(p.Cb[0] + o, cbx); ldv(p.Cb[1] + o, cby); ldv(p.Cb[2] + o, cbz);
+            T ca[V], cb[V];
+            ldv(p.Ca[0] + o, ca); ldv(p.Cb[0] + o, cb);
+#pragma unroll
+            for (int v = 0; v < V; ++v) ex[v] = fma(cb[v], ax[v], ca[v] * ex0[v]);
+            ldv(p.Ca[1] + o, ca); ldv(p.Cb[1] + o, cb);
+#pragma unroll
+            for (int v = 0; v < V; ++v) ey[v] = fma(cb[v], ay[v], ca[v] * ey0[v]);
+            ldv(p.Ca[2] + o, ca); ldv(p.Cb[2] + o, cb);
+#pragma unroll
+            for (int v = 0; v < V; ++v) ez[v] = fma(cb[v], az[v], ca[v] * ez[v]);
           } else {
 #pragma unroll
             for (int v = 0; v < V; ++v) {
               const Vec4<T> a = lds4(tab + 8 * (int)mi[v]), b = lds4(tab + 8 * (int)mi[v] + 4);
-              cax[v] = a.a; cay[v] = a.b; caz[v] = a.c; cbx[v] = a.d; cby[v] = b.a; cbz[v] = b.b;
+              ex[v] = fma(a.d, ax[v], a.a * ex0[v]);
+              ey[v] = fma(b.a, ay[v], a.b * ey0[v]);
+              ez[v] = fma(b.b, az[v], a.c * ez[v]);
             }
           }
-          const bool wj = (j == 0), wk = (k == 0);
-          T ex[V], ey[V];
+          // PEC walls: low-face tangential E stays zero (R1)
+          if (k == 0) {
 #pragma unroll
-          for (int v = 0; v < V; ++v) {
-            const bool wi = (i0 + v == 0), pad = (i0 + v >= p.nx);
-            ex[v] = cax[v] * ex0[v] + cbx[v] * ax[v];
-            ey[v] = cay[v] * ey0[v] + cby[v] * ay[v];
-            ez[v] = caz[v] * ez[v] + cbz[v] * az[v];
-            if (wj || wk || pad) ex[v] = T(0);
-            if (wi || wk || pad) ey[v] = T(0);
-            if (wi || wj || pad) ez[v] = T(0);
+            for (int v = 0; v < V; ++v) { ex[v] = T(0); ey[v] = T(0); }
           }
-          stv_stream(p.dst[kEx] + o, ex); stv_stream(p.dst[kEy] + o, ey); stv_stream(p.dst[kEz] + o, ez);
+          if (wj) {
+#pragma unroll
+            for (int v = 0; v < V; ++v) { ex[v] = T(0); ez[v] = T(0); }
+          }
+          if (wi) { ey[0] = T(0); ez[0] = T(0); }
+          if (xtail) {  // pad columns i >= nx stay zero: they are the high-face PEC wall (R1)
+#pragma unroll
+            for (int v = 0; v < V; ++v) if (v >= nvalid) { ex[v] = T(0); ey[v] = T(0); ez[v] = T(0); }
+          }
+          if (!(fp.dbg & 2)) { stv_stream(p.dst[kEx] + o, ex); stv_stream(p.dst[kEy] + o, ey); stv_stream(p.dst[kEz] + o, ez); }
         }
-      } else {
-        __syncthreads();
-        if (threadIdx.x == 0 && it + NS < nIt) issue(it + NS);
       }
 #pragma unroll
       for (int v = 0; v < V; ++v) { ex0[v] = ex1[v]; ey0[v] = ey1[v]; exj0[v] = exj1[v]; }
@@ -411,40 +555,48 @@ __global__ void __launch_bounds__((TY + 2) * 32, 1) k_step_fused(const __grid_co
         for (int v = 0; v < V; ++v) { hxm[v] = hx[v]; hym[v] = hy[v]; }
       }
     } else {
-      // ---------------- H phase, halo column warp: Hy, Hz at (x0-1, y0+lane, k) ---------------------------------------
+      // ================= halo column warp: Hy, Hz at (x0-1, y0+lane, k) ================================================
       const int r = (lane < TY ? lane : 0) + 1;
       const T c_ex1 = sEx[r * BX + V - 1], c_exj1 = sEx[(r + 1) * BX + V - 1];
       const T c_ey1 = sEy[r * BX + V - 1], c_eyp1 = sEy[r * BX + V];
       if (it >= 1) {
-        T hyc = T(0), hzc = T(0);
-        if (cin && kin) {
-          const T ezc = sEz[r * BX + V - 1], ezp = sEz[r * BX + V];
-          hyc = sHy[r * BX + V - 1]; hzc = sHz[r * BX + V - 1];
-          const T dzEx = (c_ex1 - c_ex0) * p.idz_, dxEz = (ezp - ezc) * p.idx_;
-          const T dxEy = (c_eyp0 - c_ey0) * p.idx_, dyEx = (c_exj0 - c_ex0) * p.idy_;
-          const int si = slab_coord(i0, p.lo[0], p.hi[0], p.nx);
-          T ay = dzEx * (sk >= 0 ? p.kH[2][sk] : T(1));
-          T az = -dyEx * iky_H;
-          if (si >= 0) {
-            const long long q = si + (long long)Sx * (j + (long long)p.ny * k);
-            const T b = p.bH[0][si], c = p.cH[0][si], ikx = p.kH[0][si];
-            ay -= dxEz * ikx + (b * fp.psiH_src[pHyx][q] + c * dxEz);
-            az += dxEy * ikx + (b * fp.psiH_src[pHzx][q] + c * dxEy);
-          } else { ay -= dxEz; az += dxEy; }
-          if (sj >= 0) az -= bHy * fp.psiH_src[pHzy][i0 + (long long)p.P * (sj + (long long)Sy * k)] + cHy * dyEx;
-          if (sk >= 0) ay += p.bH[2][sk] * fp.psiH_src[pHyz][i0 + (long long)p.P * (j + (long long)p.ny * sk)] + p.cH[2][sk] * dzEx;
-          T dby = p.db0, dbz = p.db0;
-          if (kMu) {
+        const T ezc = sEz[r * BX + V - 1], ezp = sEz[r * BX + V];
+        T hyc = sHy[r * BX + V - 1], hzc = sHz[r * BX + V - 1];
+        const T dEx_z = c_ex1 - c_ex0, dEz_x = ezp - ezc, dEy_x = c_eyp0 - c_ey0, dEx_y = c_exj0 - c_ex0;
+        T dby = p.db0, dbz = p.db0;
+        if (kMu) {
+          dby = dbz = T(0);
+          if (cin && k >= 0) {
             if (kFull) { dby = p.Db[1][o]; dbz = p.Db[2][o]; }
-            else { const int m = p.idx[o]; dby = tab[kTabH + 4 * m + 1]; dbz = tab[kTabH + 4 * m + 2]; }
+            else { const int m = p.idx[o]; dby = p.tab[kTabH + 4 * m + 1]; dbz = p.tab[kTabH + 4 * m + 2]; }
           }
-          hyc -= dby * ay; hzc -= dbz * az;
+        }
+        hyc -= dby * (dEx_z * p.idz_ - dEz_x * p.idx_);
+        hzc -= dbz * (dEy_x * p.idx_ - dEx_y * p.idy_);
+        if (pml) {
+          if (xs) {
+            const long long q = qx(k);
+            const T b = cp(0, 3, si0), c = cp(0, 4, si0), km1 = cp(0, 5, si0) - T(1);
+            const T dz_ = dEz_x * p.idx_, dy_ = dEy_x * p.idx_;
+            hyc += dby * (km1 * dz_ + b * fp.psiH_src[pHyx][q] + c * dz_);
+            hzc -= dbz * (km1 * dy_ + b * fp.psiH_src[pHzx][q] + c * dy_);
+          }
+          if (sj >= 0) {
+            const T dx_ = dEx_y * p.idy_;
+            hzc += dbz * ((cp(1, 5, sj) - T(1)) * dx_ + cp(1, 3, sj) * fp.psiH_src[pHzy][qy(k)] + cp(1, 4, sj) * dx_);
+          }
+          if (zs) {
+            const int sk = slab_coord(k, p.lo[2], p.hi[2], p.nz);
+            const T dx_ = dEx_z * p.idz_;
+            hyc -= dby * ((cp(2, 5, sk) - T(1)) * dx_ + cp(2, 3, sk) * fp.psiH_src[pHyz][qz(sk)] + cp(2, 4, sk) * dx_);
+          }
         }
         if (lane < TY) { hcb[lane] = hyc; hcb[TY + lane] = hzc; }
       }
       __syncthreads();
       c_ex0 = c_ex1; c_exj0 = c_exj1; c_ey0 = c_ey1; c_eyp0 = c_eyp1;
     }
+    if (++s == NS) { s = 0; ph ^= 1u; }
   }
 }
 

@@ -18,6 +18,7 @@ enum { kEx = 0, kEy, kEz, kHx, kHy, kHz };
 enum { pHxy = 0, pHzy, pHxz, pHyz, pHyx, pHzx, pExy, pEzy, pExz, pEyz, pEyx, pEzx };
 
 constexpr int kMaxTable = 256;
+constexpr int kMaxSlab = 64;   // fused kernel: CPML cells per axis (lo + hi) whose coefficient vectors fit its shared memory
 // material table (indexed mode), one 32-byte (fp32) / 64-byte (fp64) record per entry so that a look-up is two
 // (four) 128-bit loads:  tab[8*m + 0..5] = Cax Cay Caz Cbx Cby Cbz, then tab[kTabH + 4*m + 0..2] = Dbx Dby Dbz.
 constexpr int kTabH = 8 * kMaxTable;
