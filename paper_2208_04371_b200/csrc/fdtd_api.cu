@@ -777,7 +777,9 @@ int fdtd_set_option(fdtd_t* h, int option, long value) {
     case FDTD_OPT_USE_GRAPH: h->opt_graph = value ? 1 : 0; return FDTD_OK;
     case FDTD_OPT_GRAPH_UNROLL: if (value < 1 || value > 1024) break; h->opt_unroll = value; return FDTD_OK;
     case FDTD_OPT_FUSED_KZ: if (value < 0 || value > 65535) break; h->opt_kz = value; return FDTD_OK;
-    case 99: h->opt_dbg = value; return FDTD_OK;  // tuning experiments (results are wrong when set)
+#ifdef FDTD_TUNING
+    case 99: h->opt_dbg = value; return FDTD_OK;  // bandwidth experiments of tuning builds (results are wrong when set)
+#endif
   }
   return h->fail(FDTD_EINVAL, "fdtd_set_option: unknown option %d or bad value %ld", option, value);
 }

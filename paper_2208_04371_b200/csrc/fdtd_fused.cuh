@@ -38,7 +38,7 @@ struct FusedParams {
   StepParams<T> sp;      // src = set read, dst = set written; psi[0..5] = psi_H written, psi[6..11] = psi_E (in place)
   const T* psiH_src[6];  // psi_H read (pHxy pHzy pHxz pHyz pHyx pHzx)
   int kz;                // planes per z chunk (grid.z = ceil(nz / kz))
-  int dbg;               // tuning experiments only (0 in production): 1 = loads only, 2 = no global stores
+  int dbg;               // read by -DFDTD_TUNING builds only (bandwidth experiments); ignored otherwise
 };
 
 constexpr int round128(int v) { return (v + 127) / 128 * 128; }
@@ -196,6 +196,11 @@ __global__ void __launch_bounds__((TY + 2) * 32, FDTD_FUSED_MINB) k_step_fused(c
   auto cp = [&](int a, int v, int q) -> T { return cpv[(a * 6 + v) * kMaxSlab + q]; };
 
   const StepParams<T>& p = fp.sp;
+#ifdef FDTD_TUNING
+  const int dbg = fp.dbg;   // tuning builds only: 1 = loads only, 2 = no global stores, 4 = no loads (results are wrong)
+#else
+  constexpr int dbg = 0;
+#endif
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
   const int k0 = blockIdx.z * fp.kz, k1 = min(k0 + fp.kz, p.nz);
@@ -205,7 +210,7 @@ __global__ void __launch_bounds__((TY + 2) * 32, FDTD_FUSED_MINB) k_step_fused(c
 
   // one elected thread issues the boxes of iteration `it` (plane k) into stage s
   auto issue = [&](int it, int s) {
-    if (fp.dbg & 4) return;
+    if (dbg & 4) return;
     const int k = k0 - 2 + it;
     unsigned char* st = smem + s * C::STAGE;
     const bool want_idx = !kFull && it >= 2;
@@ -318,8 +323,8 @@ __global__ void __launch_bounds__((TY + 2) * 32, FDTD_FUSED_MINB) k_step_fused(c
       }
     }
 
-    if (!(fp.dbg & 4)) mbar_wait(&bar[s], ph);
-    if (fp.dbg & 1) {
+    if (!(dbg & 4)) mbar_wait(&bar[s], ph);
+    if (dbg & 1) {
       __syncthreads();
       if (threadIdx.x == 0 && it + NS < nIt) issue(it + NS, s);
       if (++s == NS) { s = 0; ph ^= 1u; }
@@ -435,7 +440,7 @@ __global__ void __launch_bounds__((TY + 2) * 32, FDTD_FUSED_MINB) k_step_fused(c
         }
         stv(hnb, hx);
         stv(hnb + C::ROWS_H * TX, hz);
-        if (owned && it >= 2 && !(fp.dbg & 2)) {
+        if (owned && it >= 2 && !(dbg & 2)) {
           stv_stream(p.dst[kHx] + o, hx); stv_stream(p.dst[kHy] + o, hy); stv_stream(p.dst[kHz] + o, hz);
         }
       }
@@ -544,7 +549,7 @@ __global__ void __launch_bounds__((TY + 2) * 32, FDTD_FUSED_MINB) k_step_fused(c
 #pragma unroll
             for (int v = 0; v < V; ++v) if (v >= nvalid) { ex[v] = T(0); ey[v] = T(0); ez[v] = T(0); }
           }
-          if (!(fp.dbg & 2)) { stv_stream(p.dst[kEx] + o, ex); stv_stream(p.dst[kEy] + o, ey); stv_stream(p.dst[kEz] + o, ez); }
+          if (!(dbg & 2)) { stv_stream(p.dst[kEx] + o, ex); stv_stream(p.dst[kEy] + o, ey); stv_stream(p.dst[kEz] + o, ez); }
         }
       }
 #pragma unroll

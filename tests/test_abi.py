@@ -94,14 +94,18 @@ def test_setup_checks_and_lifecycle_without_gpu():
 
 
 def test_workspace_size_is_the_documented_layout():
-    """fp32 indexed: six padded field arrays + one padded byte array dominate; psi only on the slabs."""
+    """fp32 indexed: padded field arrays + one padded byte array dominate; psi only on the slabs.
+    At this size the step is the fused kernel: two field sets (ping-pong) and a second copy of the six psi_H families;
+    forcing the two-pass step (FDTD_OPT_STEP_IMPL = 1) gives the single-set layout."""
     nx, ny, nz = 1536, 768, 768
-    h = B.fdtd_create(nx, ny, nz, 5e-9, 5e-9, 5e-9, 9e-18)
-    B.fdtd_set_boundary(h, [16] * 6)
     P = (nx + 1 + 31) // 32 * 32
     padded = P * (ny + 1) * (nz + 2)
-    psi = 4 * (4 * 32 * ny * nz + 4 * P * 32 * nz + 4 * P * ny * 32)
-    expect = 6 * 4 * padded + padded + psi
-    got = B.fdtd_workspace_bytes(h)
-    B.fdtd_destroy(h)
-    assert expect <= got <= expect * 1.2 + (1 << 20)
+    fam = 4 * (2 * 32 * ny * nz + 2 * P * 32 * nz + 2 * P * ny * 32)      # one family group: 2 psi arrays per axis
+    for impl, nsets, ngroups in ((1, 1, 2), (0, 2, 3)):
+        h = B.fdtd_create(nx, ny, nz, 5e-9, 5e-9, 5e-9, 9e-18)
+        B.fdtd_set_boundary(h, [16] * 6)
+        B.fdtd_set_option(h, B.FDTD_OPT_STEP_IMPL, impl)
+        expect = nsets * 6 * 4 * padded + padded + ngroups * fam
+        got = B.fdtd_workspace_bytes(h)
+        B.fdtd_destroy(h)
+        assert expect <= got <= expect * 1.01 + (1 << 20), (impl, expect, got)
