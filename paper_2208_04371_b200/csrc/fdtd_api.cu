@@ -49,7 +49,7 @@ struct fdtd {
   int has_mu = 0;
   std::vector<PortDev> ports;
   std::vector<double> freqs;
-  long opt_impl = 0, opt_graph = 1, opt_unroll = 8, opt_kz = 0, opt_dbg = 0;
+  long opt_impl = 0, opt_graph = 1, opt_unroll = 8, opt_kz = 0;
   bool committed = false;
   long nstep = 0;
   long launches = 0;
@@ -511,9 +511,8 @@ int Solver<T>::build_fused() {
       fp.sp.psi[q] = reinterpret_cast<T*>(ws + (c ? cv.psi[q] : cv.psiH2[q]));
     }
     fp.kz = kz;
-    fp.dbg = (int)opt_dbg;
     for (int f = 0; f < 6; ++f) {
-      if (!make(&fp.tm[f], ws + (c ? cv.field2[f] : cv.field[f]), fdt, sizeof(T), C::BX, f < 3 ? C::ROWS_E : C::ROWS_H))
+      if (!make(&fp.tm[f], ws + (c ? cv.field2[f] : cv.field[f]), fdt, sizeof(T), C::xw(f), C::nr(f)))
         return fail(FDTD_ECUDA, "fdtd_commit: cuTensorMapEncodeTiled failed for field %d", f);
     }
     if (mat_mode == FDTD_MAT_INDEXED) {
@@ -777,9 +776,6 @@ int fdtd_set_option(fdtd_t* h, int option, long value) {
     case FDTD_OPT_USE_GRAPH: h->opt_graph = value ? 1 : 0; return FDTD_OK;
     case FDTD_OPT_GRAPH_UNROLL: if (value < 1 || value > 1024) break; h->opt_unroll = value; return FDTD_OK;
     case FDTD_OPT_FUSED_KZ: if (value < 0 || value > 65535) break; h->opt_kz = value; return FDTD_OK;
-#ifdef FDTD_TUNING
-    case 99: h->opt_dbg = value; return FDTD_OK;  // bandwidth experiments of tuning builds (results are wrong when set)
-#endif
   }
   return h->fail(FDTD_EINVAL, "fdtd_set_option: unknown option %d or bad value %ld", option, value);
 }

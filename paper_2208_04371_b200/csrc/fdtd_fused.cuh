@@ -9,17 +9,19 @@
 //     planes.  For plane k it needs E^n on planes k, k+1 and H^{n-1/2} on plane k, on the tile plus a one-cell halo:
 //     E^{n+1}(c) needs H^{n+1/2}(c), H^{n+1/2}(c - e_a), which need E^n(c), E^n(c + e_b), E^n(c - e_a + e_b).
 //   * TMA (cp.async.bulk.tensor.3d) brings, per plane, seven boxes into shared memory: Ex, Ey of plane k+1, Ez and
-//     Hx, Hy, Hz of plane k (each (TX + 2 vectors) x (TY + 2 | TY + 1) with the halo, zero-filled outside the array)
-//     and the uint8 index tile.  NS stages ring, one mbarrier per stage, one elected thread issues; the boxes of plane
-//     k + NS are requested as soon as plane k has been read, so NS - 1 planes are in flight per SM with no register
-//     cost.  This is what keeps HBM busy with one resident block per SM.
-//   * H phase: warp w = 1..TY owns tile row w-1; warp 0 recomputes the halo row j = y0-1 (its Hx, Hz are the j-1
-//     operands of the first owned row), warp TY+1 recomputes Hy, Hz of the halo column i = x0-1.  Plane k operands that
-//     were loaded as "k+1" one iteration earlier are carried in registers, so an iteration reads only its own stage.
-//     New Hx, Hz rows go to shared memory (for the row above), the halo column to a small array, Hy and the k-1 plane
-//     of Hx, Hy stay in registers; the x-1 operands come from warp shuffles.
-//   * one __syncthreads, then the E phase for the owned cells: coefficients from the shared-memory table (or the
-//     full arrays), CPML, walls, store.
+//     Hx, Hy, Hz of plane k and the uint8 index tile.  Every field has its own box: only the halo it really needs
+//     (Hx none in x, Ex/Hy/Hz one vector on the low side, Ey/Ez both sides; Hy no halo row, Ex/Ez two, the rest one),
+//     zero-filled outside the array.  NS stages ring with a full and an empty mbarrier per stage.
+//   * warp roles, no block-wide barrier anywhere in the plane loop:
+//       warp 0         producer: an elected lane re-arms a stage as soon as every consumer warp has released it; the
+//                      warp also recomputes Hy, Hz of the halo column i = x0-1 (lane l <-> row y0+l) into shared memory
+//       warp 1         halo row j = y0-1: recomputes its Hx, Hz (the j-1 operands of the first owned row)
+//       warp 2..TY+1   one owned tile row each: H phase, then E phase
+//     New Hx, Hz rows go to a ring of NS shared-memory buffers; row r signals an mbarrier per (buffer, row) and row r+1
+//     waits on it before its E phase (point-to-point, so warps drift freely and latencies overlap).  Hy and the k-1
+//     plane of Hx, Hy stay in registers; the x-1 operands come from warp shuffles (lane 0: the halo column).
+//     A stage is released after the E phase has read the neighbour row, which is also what makes the ring of H buffers
+//     safe to overwrite NS planes later.
 //   * results go to the OTHER field set (ping-pong): a neighbouring block may still need E^n / H^{n-1/2} of this tile
 //     for its halo, so updating in place would be a race.  psi_H is double buffered for the same reason (the halo
 //     recomputation reads the old value); psi_E is touched by the owner only and stays in place.
@@ -38,24 +40,31 @@ struct FusedParams {
   StepParams<T> sp;      // src = set read, dst = set written; psi[0..5] = psi_H written, psi[6..11] = psi_E (in place)
   const T* psiH_src[6];  // psi_H read (pHxy pHzy pHxz pHyz pHyx pHzx)
   int kz;                // planes per z chunk (grid.z = ceil(nz / kz))
-  int dbg;               // read by -DFDTD_TUNING builds only (bandwidth experiments); ignored otherwise
 };
 
-constexpr int round128(int v) { return (v + 127) / 128 * 128; }
+__host__ __device__ constexpr int round128(int v) { return (v + 127) / 128 * 128; }
 
 template <typename T, int TY_, int NS_>
 struct FusedCfg {
-  static constexpr int V = VecOf<T>::V, TX = 32 * V, BX = TX + 2 * V, TY = TY_, NS = NS_;
-  static constexpr int ROWS_E = TY + 2, ROWS_H = TY + 1;
-  static constexpr int E_TX = ROWS_E * BX * (int)sizeof(T), H_TX = ROWS_H * BX * (int)sizeof(T), I_TX = TY * TX;
-  static constexpr int E_B = round128(E_TX), H_B = round128(H_TX), I_B = round128(I_TX);
-  static constexpr int STAGE = 3 * E_B + 3 * H_B + I_B;
-  static constexpr int HN_B = 2 * 2 * ROWS_H * TX * (int)sizeof(T);   // [buffer][Hx|Hz][row][x]
-  static constexpr int HC_B = round128(2 * 2 * TY * (int)sizeof(T));  // [buffer][Hy|Hz][row] at i = x0-1
-  static constexpr int TAB_B = kTabH * (int)sizeof(T);               // E records only; Db records are read from global
-  static constexpr int CP_B = 3 * 6 * kMaxSlab * (int)sizeof(T);      // CPML vectors [axis][bE cE kE bH cH kH][slab coordinate]
-  static constexpr int BAR_B = 128;
-  static constexpr int SMEM = NS * STAGE + HN_B + HC_B + TAB_B + CP_B + BAR_B;
+  static constexpr int V = VecOf<T>::V, TX = 32 * V, TY = TY_, NS = NS_;
+  // box of field f (Ex Ey Ez Hx Hy Hz): low-side x halo (elements), row width, first row relative to y0, rows
+  __host__ __device__ static constexpr int xl(int f) { return f == kHx ? 0 : V; }
+  __host__ __device__ static constexpr int xw(int f) { return f == kHx ? TX : ((f == kEy || f == kEz) ? TX + 2 * V : TX + V); }
+  __host__ __device__ static constexpr int r0(int f) { return f == kHy ? 0 : -1; }
+  __host__ __device__ static constexpr int nr(int f) { return (f == kEx || f == kEz) ? TY + 2 : (f == kHy ? TY : TY + 1); }
+  __host__ __device__ static constexpr int tx_bytes(int f) { return nr(f) * xw(f) * (int)sizeof(T); }
+  __host__ __device__ static constexpr int off(int f) { return f == 0 ? 0 : off(f - 1) + round128(tx_bytes(f - 1)); }
+  static constexpr int I_TX = TY * TX, I_OFF = off(6);
+  static constexpr int STAGE = I_OFF + round128(I_TX);
+  static constexpr int HN_SLOT = 2 * TY * TX * (int)sizeof(T);          // [Hx|Hz][row 0..TY-1 = j - (y0-1)][x]
+  static constexpr int HC_SLOT = round128(2 * TY * (int)sizeof(T));     // [Hy|Hz][row] at i = x0-1
+  static constexpr int TAB_B = kTabH * (int)sizeof(T);                  // E records only; Db records are read from global
+  static constexpr int CP_B = 3 * 6 * kMaxSlab * (int)sizeof(T);        // CPML vectors [axis][bE cE kE bH cH kH][slab coordinate]
+  static constexpr int NBAR = 2 * NS + NS * TY + NS;                    // full, empty, row-ready, column-ready
+  static constexpr int BAR_B = round128(NBAR * 8);
+  static constexpr int O_HN = NS * STAGE, O_HC = O_HN + NS * HN_SLOT, O_TAB = O_HC + NS * HC_SLOT, O_CP = O_TAB + TAB_B,
+                       O_BAR = O_CP + CP_B;
+  static constexpr int SMEM = O_BAR + BAR_B;
   static constexpr int THREADS = (TY + 2) * 32;
 };
 
@@ -67,6 +76,9 @@ __device__ __forceinline__ void mbar_init(uint64_t* b, unsigned count) {
 __device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 __device__ __forceinline__ void mbar_expect_tx(uint64_t* b, unsigned bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* b) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
 }
 __device__ __forceinline__ bool mbar_try_wait(uint64_t* b, unsigned parity) {
   unsigned ok;
@@ -177,30 +189,26 @@ __device__ __forceinline__ void psi_update2(T (&a)[V], T (&d)[V], const T (&da)[
   }
 }
 
-#ifndef FDTD_FUSED_MINB
-#define FDTD_FUSED_MINB 1
-#endif
 template <typename T, int MODE, int TY, int NS>
-__global__ void __launch_bounds__((TY + 2) * 32, FDTD_FUSED_MINB) k_step_fused(const __grid_constant__ FusedParams<T> fp) {
+__global__ void __launch_bounds__((TY + 2) * 32, 1) k_step_fused(const __grid_constant__ FusedParams<T> fp) {
   using C = FusedCfg<T, TY, NS>;
   using O = VOps<T, C::V>;
-  constexpr int V = C::V, TX = C::TX, BX = C::BX;
+  constexpr int V = C::V, TX = C::TX;
+  constexpr int WEx = C::xw(kEx), WEy = C::xw(kEy), WEz = C::xw(kEz), WHy = C::xw(kHy), WHz = C::xw(kHz);
   constexpr bool kFull = (MODE & kModeFull) != 0, kMu = (MODE & kModeMu) != 0;
   extern __shared__ __align__(1024) unsigned char smem[];
-  T* const hn = reinterpret_cast<T*>(smem + NS * C::STAGE);
-  T* const hc = reinterpret_cast<T*>(smem + NS * C::STAGE + C::HN_B);
-  T* const tab = reinterpret_cast<T*>(smem + NS * C::STAGE + C::HN_B + C::HC_B);
-  T* const cpv = reinterpret_cast<T*>(smem + NS * C::STAGE + C::HN_B + C::HC_B + C::TAB_B);
-  uint64_t* const bar = reinterpret_cast<uint64_t*>(smem + NS * C::STAGE + C::HN_B + C::HC_B + C::TAB_B + C::CP_B);
+  T* const hn = reinterpret_cast<T*>(smem + C::O_HN);
+  T* const hc = reinterpret_cast<T*>(smem + C::O_HC);
+  T* const tab = reinterpret_cast<T*>(smem + C::O_TAB);
+  T* const cpv = reinterpret_cast<T*>(smem + C::O_CP);
+  uint64_t* const full = reinterpret_cast<uint64_t*>(smem + C::O_BAR);  // [NS] TMA bytes of the stage have landed
+  uint64_t* const empty = full + NS;                                     // [NS] every consumer warp is done with the stage
+  uint64_t* const rowrdy = full + 2 * NS;                                // [NS][TY] new Hx, Hz of row r are in hn[slot]
+  uint64_t* const colrdy = full + 2 * NS + NS * TY;                      // [NS] halo column Hy, Hz are in hc[slot]
   // CPML vector v (0..5 = bE cE kE bH cH kH) of axis a at slab coordinate q
   auto cp = [&](int a, int v, int q) -> T { return cpv[(a * 6 + v) * kMaxSlab + q]; };
 
   const StepParams<T>& p = fp.sp;
-#ifdef FDTD_TUNING
-  const int dbg = fp.dbg;   // tuning builds only: 1 = loads only, 2 = no global stores, 4 = no loads (results are wrong)
-#else
-  constexpr int dbg = 0;
-#endif
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
   const int k0 = blockIdx.z * fp.kz, k1 = min(k0 + fp.kz, p.nz);
@@ -210,25 +218,32 @@ __global__ void __launch_bounds__((TY + 2) * 32, FDTD_FUSED_MINB) k_step_fused(c
 
   // one elected thread issues the boxes of iteration `it` (plane k) into stage s
   auto issue = [&](int it, int s) {
-    if (dbg & 4) return;
     const int k = k0 - 2 + it;
     unsigned char* st = smem + s * C::STAGE;
     const bool want_idx = !kFull && it >= 2;
-    const unsigned bytes = it == 0 ? 2u * C::E_TX : 3u * C::E_TX + 3u * C::H_TX + (want_idx ? (unsigned)C::I_TX : 0u);
-    mbar_expect_tx(&bar[s], bytes);
-    tma_load_3d(st, &fp.tm[kEx], &bar[s], x0 - V, y0 - 1, k + 2);               // plane k+1 (array plane index + 1)
-    tma_load_3d(st + C::E_B, &fp.tm[kEy], &bar[s], x0 - V, y0 - 1, k + 2);
+    const unsigned bytes = it == 0 ? (unsigned)(C::tx_bytes(kEx) + C::tx_bytes(kEy))
+                                   : (unsigned)(C::tx_bytes(kEx) + C::tx_bytes(kEy) + C::tx_bytes(kEz) + C::tx_bytes(kHx) +
+                                                C::tx_bytes(kHy) + C::tx_bytes(kHz)) + (want_idx ? (unsigned)C::I_TX : 0u);
+    mbar_expect_tx(&full[s], bytes);
+    // Ex, Ey: plane k+1 (array plane index + 1); the rest: plane k
+    tma_load_3d(st + C::off(kEx), &fp.tm[kEx], &full[s], x0 - C::xl(kEx), y0 + C::r0(kEx), k + 2);
+    tma_load_3d(st + C::off(kEy), &fp.tm[kEy], &full[s], x0 - C::xl(kEy), y0 + C::r0(kEy), k + 2);
     if (it >= 1) {
-      tma_load_3d(st + 2 * C::E_B, &fp.tm[kEz], &bar[s], x0 - V, y0 - 1, k + 1);  // plane k
-      tma_load_3d(st + 3 * C::E_B, &fp.tm[kHx], &bar[s], x0 - V, y0 - 1, k + 1);
-      tma_load_3d(st + 3 * C::E_B + C::H_B, &fp.tm[kHy], &bar[s], x0 - V, y0 - 1, k + 1);
-      tma_load_3d(st + 3 * C::E_B + 2 * C::H_B, &fp.tm[kHz], &bar[s], x0 - V, y0 - 1, k + 1);
-      if (want_idx) tma_load_3d(st + 3 * C::E_B + 3 * C::H_B, &fp.tm[6], &bar[s], x0, y0, k + 1);
+      tma_load_3d(st + C::off(kEz), &fp.tm[kEz], &full[s], x0 - C::xl(kEz), y0 + C::r0(kEz), k + 1);
+      tma_load_3d(st + C::off(kHx), &fp.tm[kHx], &full[s], x0 - C::xl(kHx), y0 + C::r0(kHx), k + 1);
+      tma_load_3d(st + C::off(kHy), &fp.tm[kHy], &full[s], x0 - C::xl(kHy), y0 + C::r0(kHy), k + 1);
+      tma_load_3d(st + C::off(kHz), &fp.tm[kHz], &full[s], x0 - C::xl(kHz), y0 + C::r0(kHz), k + 1);
+      if (want_idx) tma_load_3d(st + C::I_OFF, &fp.tm[6], &full[s], x0, y0, k + 1);
     }
   };
 
   if (threadIdx.x == 0) {
-    for (int s = 0; s < NS; ++s) mbar_init(&bar[s], 1);
+    for (int s = 0; s < NS; ++s) {
+      mbar_init(&full[s], 1);
+      mbar_init(&empty[s], TY + 1);   // warps 1..TY+1
+      mbar_init(&colrdy[s], 1);
+      for (int r = 0; r < TY; ++r) mbar_init(&rowrdy[s * TY + r], 1);
+    }
     mbar_fence_init();
 #pragma unroll
     for (int q = 0; q < 7; ++q) tma_prefetch_desc(&fp.tm[q]);
@@ -249,13 +264,14 @@ __global__ void __launch_bounds__((TY + 2) * 32, FDTD_FUSED_MINB) k_step_fused(c
   }
 
   // ---- loop invariants ------------------------------------------------------------------------------------------------
-  const bool rowwarp = w <= TY;
-  // row warps: j = y0-1+w (w = 0 is the halo row); column warp: lane l <-> row y0+l at i = x0-1
-  const int j = rowwarp ? y0 - 1 + w : y0 + lane;
+  const bool rowwarp = w >= 1;
+  const int r = w - 1;  // row warps: tile row index relative to the halo row, j = y0-1+r
+  // row warps: j = y0-1+r (r = 0 is the halo row); column warp: lane l <-> row y0+l at i = x0-1
+  const int j = rowwarp ? y0 - 1 + r : y0 + lane;
   const int i0 = rowwarp ? x0 + lane * V : x0 - 1;
   const bool jin = j >= 0 && j < p.ny;
   const bool cin = rowwarp ? (jin && i0 < p.nx) : (jin && i0 >= 0 && lane < TY);  // the thread's cell(s) exist
-  const bool owned = rowwarp && w >= 1 && cin;                                    // ... and this thread stores them
+  const bool owned = rowwarp && r >= 1 && cin;                                    // ... and this thread stores them
   const int nvalid = rowwarp ? min(V, p.nx - i0) : 1;                             // cells of the vector inside the grid
   const int Sx = p.lo[0] + p.hi[0], Sy = p.lo[1] + p.hi[1], Sz = p.lo[2] + p.hi[2];
   const int sj = (cin && Sy > 0) ? slab_coord(j, p.lo[1], p.hi[1], p.ny) : -1;
@@ -275,298 +291,31 @@ __global__ void __launch_bounds__((TY + 2) * 32, FDTD_FUSED_MINB) k_step_fused(c
   auto qz = [&](int sk) { return (long long)i0 + (long long)p.P * (j + (long long)p.ny * sk); };           // z slab
   auto qx = [&](int k) { return (long long)(si0 >= 0 ? si0 : 0) + (long long)Sx * (j + (long long)p.ny * k); };  // x slab
   const long long orow = (long long)i0 + (long long)p.P * j;
-  const int off = rowwarp ? w * BX + V + lane * V : 0;
-  T* const hn_row = hn + (rowwarp ? w : 0) * TX + lane * V;
-
-  // registers carried from one plane to the next
-  T ex0[V], ey0[V], exj0[V], hxm[V], hym[V];
-  T eyi0 = T(0);
-#pragma unroll
-  for (int v = 0; v < V; ++v) { ex0[v] = ey0[v] = exj0[v] = hxm[v] = hym[v] = T(0); }
-  T c_ex0 = T(0), c_exj0 = T(0), c_ey0 = T(0), c_eyp0 = T(0);  // column warp: Ex(x0-1,j), Ex(x0-1,j+1), Ey(x0-1,j), Ey(x0,j)
 
   int s = 0;
   unsigned ph = 0;
   long long o = orow + p.PS * (long long)(k0 - 2);
-  for (int it = 0; it < nIt; ++it, o += p.PS) {
-    const int k = k0 - 2 + it;
-    const unsigned char* st = smem + s * C::STAGE;
-    const T* sEx = reinterpret_cast<const T*>(st);
-    const T* sEy = reinterpret_cast<const T*>(st + C::E_B);
-    const T* sEz = reinterpret_cast<const T*>(st + 2 * C::E_B);
-    const T* sHx = reinterpret_cast<const T*>(st + 3 * C::E_B);
-    const T* sHy = reinterpret_cast<const T*>(st + 3 * C::E_B + C::H_B);
-    const T* sHz = reinterpret_cast<const T*>(st + 3 * C::E_B + 2 * C::H_B);
-    const unsigned char* sIdx = st + 3 * C::E_B + 3 * C::H_B;
-    const bool zs = Sz > 0 && k >= 0 && (k < kzlo || k >= kzhi);
-    const bool pml = (xs || sj >= 0 || zs) && cin && k >= 0;   // some CPML correction applies to this thread
-    T* const hnb = hn_row + (it & 1) * (2 * C::ROWS_H * TX);
-    T* const hcb = hc + (it & 1) * (2 * TY);
 
-    if (pml && it + 1 < nIt) {  // pull the psi lines of the next plane into L2 while this plane is being processed
-      if (sj >= 0) {
-        const long long q = qy(k + 1);
-        prefetch_l2(fp.psiH_src[pHxy] + q); prefetch_l2(fp.psiH_src[pHzy] + q);
-        prefetch_l2(p.psi[pExy] + q); prefetch_l2(p.psi[pEzy] + q);
-      }
-      if (xs) {
-        const long long q = qx(k + 1);
-        prefetch_l2(fp.psiH_src[pHyx] + q); prefetch_l2(fp.psiH_src[pHzx] + q);
-        prefetch_l2(p.psi[pEyx] + q); prefetch_l2(p.psi[pEzx] + q);
-      }
-      if (k + 1 < kzlo || k + 1 >= kzhi) {
-        if (Sz > 0 && k + 1 >= 0 && k + 1 < p.nz) {
-          const long long q = qz(slab_coord(k + 1, p.lo[2], p.hi[2], p.nz));
-          prefetch_l2(fp.psiH_src[pHxz] + q); prefetch_l2(fp.psiH_src[pHyz] + q);
-          prefetch_l2(p.psi[pExz] + q); prefetch_l2(p.psi[pEyz] + q);
-        }
-      }
-    }
-
-    if (!(dbg & 4)) mbar_wait(&bar[s], ph);
-    if (dbg & 1) {
-      __syncthreads();
-      if (threadIdx.x == 0 && it + NS < nIt) issue(it + NS, s);
-      if (++s == NS) { s = 0; ph ^= 1u; }
-      continue;
-    }
-
-    if (rowwarp) {
-      // ================= row warps ====================================================================================
-      T ex1[V], ey1[V], exj1[V];
-      ldv(sEx + off, ex1); ldv(sEy + off, ey1); ldv(sEx + off + BX, exj1);
-      T eyi1 = __shfl_down_sync(0xffffffffu, ey1[0], 1);
-      if (lane == 31) eyi1 = sEy[off + V];
-      T hx[V], hy[V], hz[V], ez[V];
-      unsigned char mi[V];
+  if (!rowwarp) {
+    // ================= warp 0: halo column Hy, Hz at (x0-1, y0+lane, k), and the TMA producer ==========================
+    T c_ex0 = T(0), c_exj0 = T(0), c_ey0 = T(0), c_eyp0 = T(0);  // plane k: Ex(x0-1,j), Ex(x0-1,j+1), Ey(x0-1,j), Ey(x0,j)
+    const int rr = lane < TY ? lane : 0;
+    for (int it = 0; it < nIt; ++it, o += p.PS) {
+      const int k = k0 - 2 + it;
+      const unsigned char* st = smem + s * C::STAGE;
+      const T* sEx = reinterpret_cast<const T*>(st + C::off(kEx));
+      const T* sEy = reinterpret_cast<const T*>(st + C::off(kEy));
+      const T* sEz = reinterpret_cast<const T*>(st + C::off(kEz));
+      const T* sHy = reinterpret_cast<const T*>(st + C::off(kHy));
+      const T* sHz = reinterpret_cast<const T*>(st + C::off(kHz));
+      const bool zs = Sz > 0 && k >= 0 && (k < kzlo || k >= kzhi);
+      const bool pml = (xs || sj >= 0 || zs) && cin && k >= 0;
+      mbar_wait(&full[s], ph);
+      const T c_ex1 = sEx[(rr + 1) * WEx + V - 1], c_exj1 = sEx[(rr + 2) * WEx + V - 1];
+      const T c_ey1 = sEy[(rr + 1) * WEy + V - 1], c_eyp1 = sEy[(rr + 1) * WEy + V];
       if (it >= 1) {
-        // ---------------- H phase: H^{n+1/2}(k) = H^{n-1/2}(k) - Db curl E^n -----------------------------------------
-        T ezj[V];
-        ldv(sEz + off, ez); ldv(sEz + off + BX, ezj);
-        T ezi = __shfl_down_sync(0xffffffffu, ez[0], 1);
-        if (lane == 31) ezi = sEz[off + V];
-        ldv(sHx + off, hx); ldv(sHy + off, hy); ldv(sHz + off, hz);
-        if (!kFull && it >= 2 && w >= 1) ld_index_smem<V>(sIdx + (w - 1) * TX + lane * V, mi);
-
-        T dEz_y[V], dEy_z[V], dEx_z[V], dEx_y[V], dEz_x[V], dEy_x[V];   // undivided differences
-        O::sub(dEz_y, ezj, ez); O::sub(dEy_z, ey1, ey0); O::sub(dEx_z, ex1, ex0); O::sub(dEx_y, exj0, ex0);
-#pragma unroll
-        for (int v = 0; v < V; ++v) {
-          dEz_x[v] = ((v + 1 < V) ? ez[v + 1] : ezi) - ez[v];
-          dEy_x[v] = ((v + 1 < V) ? ey0[v + 1] : eyi0) - ey0[v];
-        }
-        T dbx[V], dby[V], dbz[V];
-        if (!kMu) {
-          O::fma_s(hx, dEz_y, -cy); O::fma_s(hx, dEy_z, cz);
-          O::fma_s(hy, dEx_z, -cz); O::fma_s(hy, dEz_x, cx);
-          O::fma_s(hz, dEy_x, -cx); O::fma_s(hz, dEx_y, cy);
-#pragma unroll
-          for (int v = 0; v < V; ++v) { dbx[v] = dby[v] = dbz[v] = p.db0; }
-        } else {
-#pragma unroll
-          for (int v = 0; v < V; ++v) { dbx[v] = dby[v] = dbz[v] = T(0); }
-          if (cin && k >= 0) {
-            if (kFull) { ldv(p.Db[0] + o, dbx); ldv(p.Db[1] + o, dby); ldv(p.Db[2] + o, dbz); }
-            else {
-              unsigned char m[V];
-              ld_index<V>(p.idx + o, m);
-#pragma unroll
-              for (int v = 0; v < V; ++v) {
-                const Vec4<T> d = ld4(p.tab + kTabH + 4 * (int)m[v]);
-                dbx[v] = d.a; dby[v] = d.b; dbz[v] = d.c;
-              }
-            }
-          }
-#pragma unroll
-          for (int v = 0; v < V; ++v) {
-            hx[v] -= dbx[v] * (dEz_y[v] * p.idy_ - dEy_z[v] * p.idz_);
-            hy[v] -= dby[v] * (dEx_z[v] * p.idz_ - dEz_x[v] * p.idx_);
-            hz[v] -= dbz[v] * (dEy_x[v] * p.idx_ - dEx_y[v] * p.idy_);
-          }
-        }
-        if (pml) {
-          const bool wr = owned && it >= 2;
-          if (sj >= 0) {  // y slab: psiHxy (from D+y Ez) -> Hx, psiHzy (from D+y Ex) -> Hz
-            const long long q = qy(k);
-            T a[V], d[V];
-            ldv(fp.psiH_src[pHxy] + q, a); ldv(fp.psiH_src[pHzy] + q, d);
-            const T ykH = (cp(1, 5, sj) - T(1)) * p.idy_;
-            psi_update2<T, V>(a, d, dEz_y, dEx_y, cp(1, 3, sj), cp(1, 4, sj), p.idy_, nvalid);
-#pragma unroll
-            for (int v = 0; v < V; ++v) {
-              hx[v] -= dbx[v] * (ykH * dEz_y[v] + a[v]); hz[v] += dbz[v] * (ykH * dEx_y[v] + d[v]);
-            }
-            if (wr) { stv(p.psi[pHxy] + q, a); stv(p.psi[pHzy] + q, d); }
-          }
-          if (zs) {  // z slab: psiHxz (from D+z Ey) -> Hx, psiHyz (from D+z Ex) -> Hy
-            const int sk = slab_coord(k, p.lo[2], p.hi[2], p.nz);
-            const long long q = qz(sk);
-            const T b = cp(2, 3, sk), c = cp(2, 4, sk), km = (cp(2, 5, sk) - T(1)) * p.idz_;
-            T a[V], d[V];
-            ldv(fp.psiH_src[pHxz] + q, a); ldv(fp.psiH_src[pHyz] + q, d);
-            psi_update2<T, V>(a, d, dEy_z, dEx_z, b, c, p.idz_, nvalid);
-#pragma unroll
-            for (int v = 0; v < V; ++v) {
-              hx[v] += dbx[v] * (km * dEy_z[v] + a[v]); hy[v] -= dby[v] * (km * dEx_z[v] + d[v]);
-            }
-            if (wr) { stv(p.psi[pHxz] + q, a); stv(p.psi[pHyz] + q, d); }
-          }
-          if (xs) {  // x slab: psiHyx (from D+x Ez) -> Hy, psiHzx (from D+x Ey) -> Hz
-            const long long q0 = qx(k);
-            if (xvec) {
-              T a[V], d[V];
-              ldv(fp.psiH_src[pHyx] + q0, a); ldv(fp.psiH_src[pHzx] + q0, d);
-#pragma unroll
-              for (int v = 0; v < V; ++v) {
-                const T b = cp(0, 3, si0 + v), c = cp(0, 4, si0 + v) * p.idx_, km = (cp(0, 5, si0 + v) - T(1)) * p.idx_;
-                a[v] = b * a[v] + c * dEz_x[v]; d[v] = b * d[v] + c * dEy_x[v];
-                hy[v] += dby[v] * (km * dEz_x[v] + a[v]); hz[v] -= dbz[v] * (km * dEy_x[v] + d[v]);
-              }
-              if (wr) { stv(p.psi[pHyx] + q0, a); stv(p.psi[pHzx] + q0, d); }
-            } else {
-#pragma unroll
-              for (int v = 0; v < V; ++v) {
-                const int si = slab_coord(i0 + v, p.lo[0], p.hi[0], p.nx);
-                if (si >= 0 && v < nvalid) {
-                  const long long q = q0 + si - (si0 >= 0 ? si0 : 0);
-                  const T b = cp(0, 3, si), c = cp(0, 4, si) * p.idx_, km = (cp(0, 5, si) - T(1)) * p.idx_;
-                  const T pyx = b * fp.psiH_src[pHyx][q] + c * dEz_x[v], pzx = b * fp.psiH_src[pHzx][q] + c * dEy_x[v];
-                  if (wr) { p.psi[pHyx][q] = pyx; p.psi[pHzx][q] = pzx; }
-                  hy[v] += dby[v] * (km * dEz_x[v] + pyx); hz[v] -= dbz[v] * (km * dEy_x[v] + pzx);
-                }
-              }
-            }
-          }
-        }
-        stv(hnb, hx);
-        stv(hnb + C::ROWS_H * TX, hz);
-        if (owned && it >= 2 && !(dbg & 2)) {
-          stv_stream(p.dst[kHx] + o, hx); stv_stream(p.dst[kHy] + o, hy); stv_stream(p.dst[kHz] + o, hz);
-        }
-      }
-      __syncthreads();
-      if (threadIdx.x == 0 && it + NS < nIt) issue(it + NS, s);
-      if (it >= 2 && w >= 1) {
-        // ---------------- E phase: E^{n+1}(k) = Ca E^n + Cb curl H^{n+1/2} ---------------------------------------------
-        T hxj[V], hzj[V];
-        ldv(hnb - TX, hxj);
-        ldv(hnb + (C::ROWS_H - 1) * TX, hzj);
-        T hyi = __shfl_up_sync(0xffffffffu, hy[V - 1], 1), hzi = __shfl_up_sync(0xffffffffu, hz[V - 1], 1);
-        if (lane == 0) { hyi = hcb[w - 1]; hzi = hcb[TY + w - 1]; }
-        T dHz_y[V], dHy_z[V], dHx_z[V], dHx_y[V], dHz_x[V], dHy_x[V];
-        O::sub(dHz_y, hz, hzj); O::sub(dHy_z, hy, hym); O::sub(dHx_z, hx, hxm); O::sub(dHx_y, hx, hxj);
-#pragma unroll
-        for (int v = 0; v < V; ++v) {
-          dHz_x[v] = hz[v] - ((v > 0) ? hz[v - 1] : hzi);
-          dHy_x[v] = hy[v] - ((v > 0) ? hy[v - 1] : hyi);
-        }
-        T ax[V], ay[V], az[V];
-        O::mul_s(ax, dHz_y, p.idy_); O::fma_s(ax, dHy_z, -p.idz_);
-        O::mul_s(ay, dHx_z, p.idz_); O::fma_s(ay, dHz_x, -p.idx_);
-        O::mul_s(az, dHy_x, p.idx_); O::fma_s(az, dHx_y, -p.idy_);
-        if (pml && owned) {
-          if (sj >= 0) {  // y slab: psiExy (from D-y Hz) -> Ex, psiEzy (from D-y Hx) -> Ez
-            const long long q = qy(k);
-            T a[V], d[V];
-            ldv(p.psi[pExy] + q, a); ldv(p.psi[pEzy] + q, d);
-            const T ykE = (cp(1, 2, sj) - T(1)) * p.idy_;
-            psi_update2<T, V>(a, d, dHz_y, dHx_y, cp(1, 0, sj), cp(1, 1, sj), p.idy_, nvalid);
-#pragma unroll
-            for (int v = 0; v < V; ++v) { ax[v] += ykE * dHz_y[v] + a[v]; az[v] -= ykE * dHx_y[v] + d[v]; }
-            stv(p.psi[pExy] + q, a); stv(p.psi[pEzy] + q, d);
-          }
-          if (zs) {  // z slab: psiExz (from D-z Hy) -> Ex, psiEyz (from D-z Hx) -> Ey
-            const int sk = slab_coord(k, p.lo[2], p.hi[2], p.nz);
-            const long long q = qz(sk);
-            const T b = cp(2, 0, sk), c = cp(2, 1, sk), km = (cp(2, 2, sk) - T(1)) * p.idz_;
-            T a[V], d[V];
-            ldv(p.psi[pExz] + q, a); ldv(p.psi[pEyz] + q, d);
-            psi_update2<T, V>(a, d, dHy_z, dHx_z, b, c, p.idz_, nvalid);
-#pragma unroll
-            for (int v = 0; v < V; ++v) { ax[v] -= km * dHy_z[v] + a[v]; ay[v] += km * dHx_z[v] + d[v]; }
-            stv(p.psi[pExz] + q, a); stv(p.psi[pEyz] + q, d);
-          }
-          if (xs) {  // x slab: psiEyx (from D-x Hz) -> Ey, psiEzx (from D-x Hy) -> Ez
-            const long long q0 = qx(k);
-            if (xvec) {
-              T a[V], d[V];
-              ldv(p.psi[pEyx] + q0, a); ldv(p.psi[pEzx] + q0, d);
-#pragma unroll
-              for (int v = 0; v < V; ++v) {
-                const T b = cp(0, 0, si0 + v), c = cp(0, 1, si0 + v) * p.idx_, km = (cp(0, 2, si0 + v) - T(1)) * p.idx_;
-                a[v] = b * a[v] + c * dHz_x[v]; d[v] = b * d[v] + c * dHy_x[v];
-                ay[v] -= km * dHz_x[v] + a[v]; az[v] += km * dHy_x[v] + d[v];
-              }
-              stv(p.psi[pEyx] + q0, a); stv(p.psi[pEzx] + q0, d);
-            } else {
-#pragma unroll
-              for (int v = 0; v < V; ++v) {
-                const int si = slab_coord(i0 + v, p.lo[0], p.hi[0], p.nx);
-                if (si >= 0 && v < nvalid) {
-                  const long long q = q0 + si - (si0 >= 0 ? si0 : 0);
-                  const T b = cp(0, 0, si), c = cp(0, 1, si) * p.idx_, km = (cp(0, 2, si) - T(1)) * p.idx_;
-                  const T pyx = b * p.psi[pEyx][q] + c * dHz_x[v], pzx = b * p.psi[pEzx][q] + c * dHy_x[v];
-                  p.psi[pEyx][q] = pyx; p.psi[pEzx][q] = pzx;
-                  ay[v] -= km * dHz_x[v] + pyx; az[v] += km * dHy_x[v] + pzx;
-                }
-              }
-            }
-          }
-        }
-        if (owned) {
-          T ex[V], ey[V];
-          if (kFull) {
-            T ca[V], cb[V];
-            ldv(p.Ca[0] + o, ca); ldv(p.Cb[0] + o, cb);
-#pragma unroll
-            for (int v = 0; v < V; ++v) ex[v] = fma(cb[v], ax[v], ca[v] * ex0[v]);
-            ldv(p.Ca[1] + o, ca); ldv(p.Cb[1] + o, cb);
-#pragma unroll
-            for (int v = 0; v < V; ++v) ey[v] = fma(cb[v], ay[v], ca[v] * ey0[v]);
-            ldv(p.Ca[2] + o, ca); ldv(p.Cb[2] + o, cb);
-#pragma unroll
-            for (int v = 0; v < V; ++v) ez[v] = fma(cb[v], az[v], ca[v] * ez[v]);
-          } else {
-#pragma unroll
-            for (int v = 0; v < V; ++v) {
-              const Vec4<T> a = lds4(tab + 8 * (int)mi[v]), b = lds4(tab + 8 * (int)mi[v] + 4);
-              ex[v] = fma(a.d, ax[v], a.a * ex0[v]);
-              ey[v] = fma(b.a, ay[v], a.b * ey0[v]);
-              ez[v] = fma(b.b, az[v], a.c * ez[v]);
-            }
-          }
-          // PEC walls: low-face tangential E stays zero (R1)
-          if (k == 0) {
-#pragma unroll
-            for (int v = 0; v < V; ++v) { ex[v] = T(0); ey[v] = T(0); }
-          }
-          if (wj) {
-#pragma unroll
-            for (int v = 0; v < V; ++v) { ex[v] = T(0); ez[v] = T(0); }
-          }
-          if (wi) { ey[0] = T(0); ez[0] = T(0); }
-          if (xtail) {  // pad columns i >= nx stay zero: they are the high-face PEC wall (R1)
-#pragma unroll
-            for (int v = 0; v < V; ++v) if (v >= nvalid) { ex[v] = T(0); ey[v] = T(0); ez[v] = T(0); }
-          }
-          if (!(dbg & 2)) { stv_stream(p.dst[kEx] + o, ex); stv_stream(p.dst[kEy] + o, ey); stv_stream(p.dst[kEz] + o, ez); }
-        }
-      }
-#pragma unroll
-      for (int v = 0; v < V; ++v) { ex0[v] = ex1[v]; ey0[v] = ey1[v]; exj0[v] = exj1[v]; }
-      eyi0 = eyi1;
-      if (it >= 1) {
-#pragma unroll
-        for (int v = 0; v < V; ++v) { hxm[v] = hx[v]; hym[v] = hy[v]; }
-      }
-    } else {
-      // ================= halo column warp: Hy, Hz at (x0-1, y0+lane, k) ================================================
-      const int r = (lane < TY ? lane : 0) + 1;
-      const T c_ex1 = sEx[r * BX + V - 1], c_exj1 = sEx[(r + 1) * BX + V - 1];
-      const T c_ey1 = sEy[r * BX + V - 1], c_eyp1 = sEy[r * BX + V];
-      if (it >= 1) {
-        const T ezc = sEz[r * BX + V - 1], ezp = sEz[r * BX + V];
-        T hyc = sHy[r * BX + V - 1], hzc = sHz[r * BX + V - 1];
+        const T ezc = sEz[(rr + 1) * WEz + V - 1], ezp = sEz[(rr + 1) * WEz + V];
+        T hyc = sHy[rr * WHy + V - 1], hzc = sHz[(rr + 1) * WHz + V - 1];
         const T dEx_z = c_ex1 - c_ex0, dEz_x = ezp - ezc, dEy_x = c_eyp0 - c_ey0, dEx_y = c_exj0 - c_ex0;
         T dby = p.db0, dbz = p.db0;
         if (kMu) {
@@ -596,10 +345,305 @@ __global__ void __launch_bounds__((TY + 2) * 32, FDTD_FUSED_MINB) k_step_fused(c
             hyc -= dby * ((cp(2, 5, sk) - T(1)) * dx_ + cp(2, 3, sk) * fp.psiH_src[pHyz][qz(sk)] + cp(2, 4, sk) * dx_);
           }
         }
+        T* const hcb = hc + s * (C::HC_SLOT / (int)sizeof(T));
         if (lane < TY) { hcb[lane] = hyc; hcb[TY + lane] = hzc; }
       }
-      __syncthreads();
       c_ex0 = c_ex1; c_exj0 = c_exj1; c_ey0 = c_ey1; c_eyp0 = c_eyp1;
+      __syncwarp();
+      if (lane == 0) {
+        mbar_arrive(&colrdy[s]);
+        // re-arm the stage of the previous plane once every consumer warp has released it
+        if (it >= 1 && it - 1 + NS < nIt) {
+          const int ps = s == 0 ? NS - 1 : s - 1;
+          mbar_wait(&empty[ps], s == 0 ? ph ^ 1u : ph);
+          issue(it - 1 + NS, ps);
+        }
+      }
+      if (++s == NS) { s = 0; ph ^= 1u; }
+    }
+    return;
+  }
+
+  // ================= warps 1..TY+1: row j = y0-1+r ======================================================================
+  const int oEx = r * WEx + V + lane * V, oEy = r * WEy + V + lane * V, oEz = r * WEz + V + lane * V;
+  const int oHx = r * TX + lane * V, oHy = (r >= 1 ? r - 1 : 0) * WHy + V + lane * V, oHz = r * WHz + V + lane * V;
+  const int oHn = r * TX + lane * V;   // own row in the H ring (rows 0..TY-1 are written; row TY has no reader)
+  // registers carried from one plane to the next
+  T ex0[V], ey0[V], exj0[V], hxm[V], hym[V];
+  T eyi0 = T(0);
+#pragma unroll
+  for (int v = 0; v < V; ++v) { ex0[v] = ey0[v] = exj0[v] = hxm[v] = hym[v] = T(0); }
+
+  for (int it = 0; it < nIt; ++it, o += p.PS) {
+    const int k = k0 - 2 + it;
+    const unsigned char* st = smem + s * C::STAGE;
+    const T* sEx = reinterpret_cast<const T*>(st + C::off(kEx));
+    const T* sEy = reinterpret_cast<const T*>(st + C::off(kEy));
+    const T* sEz = reinterpret_cast<const T*>(st + C::off(kEz));
+    const T* sHx = reinterpret_cast<const T*>(st + C::off(kHx));
+    const T* sHy = reinterpret_cast<const T*>(st + C::off(kHy));
+    const T* sHz = reinterpret_cast<const T*>(st + C::off(kHz));
+    const unsigned char* sIdx = st + C::I_OFF;
+    const bool zs = Sz > 0 && k >= 0 && (k < kzlo || k >= kzhi);
+    const bool pml = (xs || sj >= 0 || zs) && cin && k >= 0;   // some CPML correction applies to this thread
+    T* const hnb = hn + s * (C::HN_SLOT / (int)sizeof(T));
+
+    if (pml && it + 1 < nIt) {  // pull the psi lines of the next plane into L2 while this plane is being processed
+      if (sj >= 0) {
+        const long long q = qy(k + 1);
+        prefetch_l2(fp.psiH_src[pHxy] + q); prefetch_l2(fp.psiH_src[pHzy] + q);
+        prefetch_l2(p.psi[pExy] + q); prefetch_l2(p.psi[pEzy] + q);
+      }
+      if (xs) {
+        const long long q = qx(k + 1);
+        prefetch_l2(fp.psiH_src[pHyx] + q); prefetch_l2(fp.psiH_src[pHzx] + q);
+        prefetch_l2(p.psi[pEyx] + q); prefetch_l2(p.psi[pEzx] + q);
+      }
+      if (k + 1 < kzlo || k + 1 >= kzhi) {
+        if (Sz > 0 && k + 1 >= 0 && k + 1 < p.nz) {
+          const long long q = qz(slab_coord(k + 1, p.lo[2], p.hi[2], p.nz));
+          prefetch_l2(fp.psiH_src[pHxz] + q); prefetch_l2(fp.psiH_src[pHyz] + q);
+          prefetch_l2(p.psi[pExz] + q); prefetch_l2(p.psi[pEyz] + q);
+        }
+      }
+    }
+
+    mbar_wait(&full[s], ph);
+    T ex1[V], ey1[V], exj1[V];
+    ldv(sEx + oEx, ex1); ldv(sEy + oEy, ey1); ldv(sEx + oEx + WEx, exj1);
+    T eyi1 = __shfl_down_sync(0xffffffffu, ey1[0], 1);
+    if (lane == 31) eyi1 = sEy[oEy + V];
+    T hx[V], hy[V], hz[V], ez[V];
+    if (it >= 1) {
+      // ---------------- H phase: H^{n+1/2}(k) = H^{n-1/2}(k) - Db curl E^n -------------------------------------------
+      T ezj[V];
+      ldv(sEz + oEz, ez); ldv(sEz + oEz + WEz, ezj);
+      T ezi = __shfl_down_sync(0xffffffffu, ez[0], 1);
+      if (lane == 31) ezi = sEz[oEz + V];
+      ldv(sHx + oHx, hx); ldv(sHy + oHy, hy); ldv(sHz + oHz, hz);
+
+      T dEz_y[V], dEy_z[V], dEx_z[V], dEx_y[V], dEz_x[V], dEy_x[V];   // undivided differences
+      O::sub(dEz_y, ezj, ez); O::sub(dEy_z, ey1, ey0); O::sub(dEx_z, ex1, ex0); O::sub(dEx_y, exj0, ex0);
+#pragma unroll
+      for (int v = 0; v < V; ++v) {
+        dEz_x[v] = ((v + 1 < V) ? ez[v + 1] : ezi) - ez[v];
+        dEy_x[v] = ((v + 1 < V) ? ey0[v + 1] : eyi0) - ey0[v];
+      }
+      T dbx[V], dby[V], dbz[V];
+      if (!kMu) {
+        O::fma_s(hx, dEz_y, -cy); O::fma_s(hx, dEy_z, cz);
+        O::fma_s(hy, dEx_z, -cz); O::fma_s(hy, dEz_x, cx);
+        O::fma_s(hz, dEy_x, -cx); O::fma_s(hz, dEx_y, cy);
+#pragma unroll
+        for (int v = 0; v < V; ++v) { dbx[v] = dby[v] = dbz[v] = p.db0; }
+      } else {
+#pragma unroll
+        for (int v = 0; v < V; ++v) { dbx[v] = dby[v] = dbz[v] = T(0); }
+        if (cin && k >= 0) {
+          if (kFull) { ldv(p.Db[0] + o, dbx); ldv(p.Db[1] + o, dby); ldv(p.Db[2] + o, dbz); }
+          else {
+            unsigned char m[V];
+            ld_index<V>(p.idx + o, m);
+#pragma unroll
+            for (int v = 0; v < V; ++v) {
+              const Vec4<T> d = ld4(p.tab + kTabH + 4 * (int)m[v]);
+              dbx[v] = d.a; dby[v] = d.b; dbz[v] = d.c;
+            }
+          }
+        }
+#pragma unroll
+        for (int v = 0; v < V; ++v) {
+          hx[v] -= dbx[v] * (dEz_y[v] * p.idy_ - dEy_z[v] * p.idz_);
+          hy[v] -= dby[v] * (dEx_z[v] * p.idz_ - dEz_x[v] * p.idx_);
+          hz[v] -= dbz[v] * (dEy_x[v] * p.idx_ - dEx_y[v] * p.idy_);
+        }
+      }
+      if (pml) {
+        const bool wr = owned && it >= 2;
+        if (sj >= 0) {  // y slab: psiHxy (from D+y Ez) -> Hx, psiHzy (from D+y Ex) -> Hz
+          const long long q = qy(k);
+          T a[V], d[V];
+          ldv(fp.psiH_src[pHxy] + q, a); ldv(fp.psiH_src[pHzy] + q, d);
+          const T ykH = (cp(1, 5, sj) - T(1)) * p.idy_;
+          psi_update2<T, V>(a, d, dEz_y, dEx_y, cp(1, 3, sj), cp(1, 4, sj), p.idy_, nvalid);
+#pragma unroll
+          for (int v = 0; v < V; ++v) {
+            hx[v] -= dbx[v] * (ykH * dEz_y[v] + a[v]); hz[v] += dbz[v] * (ykH * dEx_y[v] + d[v]);
+          }
+          if (wr) { stv(p.psi[pHxy] + q, a); stv(p.psi[pHzy] + q, d); }
+        }
+        if (zs) {  // z slab: psiHxz (from D+z Ey) -> Hx, psiHyz (from D+z Ex) -> Hy
+          const int sk = slab_coord(k, p.lo[2], p.hi[2], p.nz);
+          const long long q = qz(sk);
+          const T b = cp(2, 3, sk), c = cp(2, 4, sk), km = (cp(2, 5, sk) - T(1)) * p.idz_;
+          T a[V], d[V];
+          ldv(fp.psiH_src[pHxz] + q, a); ldv(fp.psiH_src[pHyz] + q, d);
+          psi_update2<T, V>(a, d, dEy_z, dEx_z, b, c, p.idz_, nvalid);
+#pragma unroll
+          for (int v = 0; v < V; ++v) {
+            hx[v] += dbx[v] * (km * dEy_z[v] + a[v]); hy[v] -= dby[v] * (km * dEx_z[v] + d[v]);
+          }
+          if (wr) { stv(p.psi[pHxz] + q, a); stv(p.psi[pHyz] + q, d); }
+        }
+        if (xs) {  // x slab: psiHyx (from D+x Ez) -> Hy, psiHzx (from D+x Ey) -> Hz
+          const long long q0 = qx(k);
+          if (xvec) {
+            T a[V], d[V];
+            ldv(fp.psiH_src[pHyx] + q0, a); ldv(fp.psiH_src[pHzx] + q0, d);
+#pragma unroll
+            for (int v = 0; v < V; ++v) {
+              const T b = cp(0, 3, si0 + v), c = cp(0, 4, si0 + v) * p.idx_, km = (cp(0, 5, si0 + v) - T(1)) * p.idx_;
+              a[v] = b * a[v] + c * dEz_x[v]; d[v] = b * d[v] + c * dEy_x[v];
+              hy[v] += dby[v] * (km * dEz_x[v] + a[v]); hz[v] -= dbz[v] * (km * dEy_x[v] + d[v]);
+            }
+            if (wr) { stv(p.psi[pHyx] + q0, a); stv(p.psi[pHzx] + q0, d); }
+          } else {
+#pragma unroll
+            for (int v = 0; v < V; ++v) {
+              const int si = slab_coord(i0 + v, p.lo[0], p.hi[0], p.nx);
+              if (si >= 0 && v < nvalid) {
+                const long long q = q0 + si - (si0 >= 0 ? si0 : 0);
+                const T b = cp(0, 3, si), c = cp(0, 4, si) * p.idx_, km = (cp(0, 5, si) - T(1)) * p.idx_;
+                const T pyx = b * fp.psiH_src[pHyx][q] + c * dEz_x[v], pzx = b * fp.psiH_src[pHzx][q] + c * dEy_x[v];
+                if (wr) { p.psi[pHyx][q] = pyx; p.psi[pHzx][q] = pzx; }
+                hy[v] += dby[v] * (km * dEz_x[v] + pyx); hz[v] -= dbz[v] * (km * dEy_x[v] + pzx);
+              }
+            }
+          }
+        }
+      }
+      if (r < TY) { stv(hnb + oHn, hx); stv(hnb + TY * TX + oHn, hz); }
+      if (owned && it >= 2) {
+        stv_stream(p.dst[kHx] + o, hx); stv_stream(p.dst[kHy] + o, hy); stv_stream(p.dst[kHz] + o, hz);
+      }
+    }
+    __syncwarp();
+    if (lane == 0 && r < TY) mbar_arrive(&rowrdy[s * TY + r]);   // every iteration, so that the phase parity is it / NS
+    if (it >= 2 && r >= 1) {
+      // ---------------- E phase: E^{n+1}(k) = Ca E^n + Cb curl H^{n+1/2} ---------------------------------------------
+      unsigned char mi[V];
+      if (!kFull) ld_index_smem<V>(sIdx + (r - 1) * TX + lane * V, mi);
+      mbar_wait(&rowrdy[s * TY + r - 1], ph);
+      T hxj[V], hzj[V];
+      ldv(hnb + oHn - TX, hxj);
+      ldv(hnb + TY * TX + oHn - TX, hzj);
+      T hyi = __shfl_up_sync(0xffffffffu, hy[V - 1], 1), hzi = __shfl_up_sync(0xffffffffu, hz[V - 1], 1);
+      if (lane == 0) {
+        mbar_wait(&colrdy[s], ph);
+        const T* const hcb = hc + s * (C::HC_SLOT / (int)sizeof(T));
+        hyi = hcb[r - 1]; hzi = hcb[TY + r - 1];
+      }
+      // release the stage: nothing below reads it or the H ring (the loads above are ordered before the arrive)
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&empty[s]);
+      T dHz_y[V], dHy_z[V], dHx_z[V], dHx_y[V], dHz_x[V], dHy_x[V];
+      O::sub(dHz_y, hz, hzj); O::sub(dHy_z, hy, hym); O::sub(dHx_z, hx, hxm); O::sub(dHx_y, hx, hxj);
+#pragma unroll
+      for (int v = 0; v < V; ++v) {
+        dHz_x[v] = hz[v] - ((v > 0) ? hz[v - 1] : hzi);
+        dHy_x[v] = hy[v] - ((v > 0) ? hy[v - 1] : hyi);
+      }
+      T ax[V], ay[V], az[V];
+      O::mul_s(ax, dHz_y, p.idy_); O::fma_s(ax, dHy_z, -p.idz_);
+      O::mul_s(ay, dHx_z, p.idz_); O::fma_s(ay, dHz_x, -p.idx_);
+      O::mul_s(az, dHy_x, p.idx_); O::fma_s(az, dHx_y, -p.idy_);
+      if (pml && owned) {
+        if (sj >= 0) {  // y slab: psiExy (from D-y Hz) -> Ex, psiEzy (from D-y Hx) -> Ez
+          const long long q = qy(k);
+          T a[V], d[V];
+          ldv(p.psi[pExy] + q, a); ldv(p.psi[pEzy] + q, d);
+          const T ykE = (cp(1, 2, sj) - T(1)) * p.idy_;
+          psi_update2<T, V>(a, d, dHz_y, dHx_y, cp(1, 0, sj), cp(1, 1, sj), p.idy_, nvalid);
+#pragma unroll
+          for (int v = 0; v < V; ++v) { ax[v] += ykE * dHz_y[v] + a[v]; az[v] -= ykE * dHx_y[v] + d[v]; }
+          stv(p.psi[pExy] + q, a); stv(p.psi[pEzy] + q, d);
+        }
+        if (zs) {  // z slab: psiExz (from D-z Hy) -> Ex, psiEyz (from D-z Hx) -> Ey
+          const int sk = slab_coord(k, p.lo[2], p.hi[2], p.nz);
+          const long long q = qz(sk);
+          const T b = cp(2, 0, sk), c = cp(2, 1, sk), km = (cp(2, 2, sk) - T(1)) * p.idz_;
+          T a[V], d[V];
+          ldv(p.psi[pExz] + q, a); ldv(p.psi[pEyz] + q, d);
+          psi_update2<T, V>(a, d, dHy_z, dHx_z, b, c, p.idz_, nvalid);
+#pragma unroll
+          for (int v = 0; v < V; ++v) { ax[v] -= km * dHy_z[v] + a[v]; ay[v] += km * dHx_z[v] + d[v]; }
+          stv(p.psi[pExz] + q, a); stv(p.psi[pEyz] + q, d);
+        }
+        if (xs) {  // x slab: psiEyx (from D-x Hz) -> Ey, psiEzx (from D-x Hy) -> Ez
+          const long long q0 = qx(k);
+          if (xvec) {
+            T a[V], d[V];
+            ldv(p.psi[pEyx] + q0, a); ldv(p.psi[pEzx] + q0, d);
+#pragma unroll
+            for (int v = 0; v < V; ++v) {
+              const T b = cp(0, 0, si0 + v), c = cp(0, 1, si0 + v) * p.idx_, km = (cp(0, 2, si0 + v) - T(1)) * p.idx_;
+              a[v] = b * a[v] + c * dHz_x[v]; d[v] = b * d[v] + c * dHy_x[v];
+              ay[v] -= km * dHz_x[v] + a[v]; az[v] += km * dHy_x[v] + d[v];
+            }
+            stv(p.psi[pEyx] + q0, a); stv(p.psi[pEzx] + q0, d);
+          } else {
+#pragma unroll
+            for (int v = 0; v < V; ++v) {
+              const int si = slab_coord(i0 + v, p.lo[0], p.hi[0], p.nx);
+              if (si >= 0 && v < nvalid) {
+                const long long q = q0 + si - (si0 >= 0 ? si0 : 0);
+                const T b = cp(0, 0, si), c = cp(0, 1, si) * p.idx_, km = (cp(0, 2, si) - T(1)) * p.idx_;
+                const T pyx = b * p.psi[pEyx][q] + c * dHz_x[v], pzx = b * p.psi[pEzx][q] + c * dHy_x[v];
+                p.psi[pEyx][q] = pyx; p.psi[pEzx][q] = pzx;
+                ay[v] -= km * dHz_x[v] + pyx; az[v] += km * dHy_x[v] + pzx;
+              }
+            }
+          }
+        }
+      }
+      if (owned) {
+        T ex[V], ey[V];
+        if (kFull) {
+          T ca[V], cb[V];
+          ldv(p.Ca[0] + o, ca); ldv(p.Cb[0] + o, cb);
+#pragma unroll
+          for (int v = 0; v < V; ++v) ex[v] = fma(cb[v], ax[v], ca[v] * ex0[v]);
+          ldv(p.Ca[1] + o, ca); ldv(p.Cb[1] + o, cb);
+#pragma unroll
+          for (int v = 0; v < V; ++v) ey[v] = fma(cb[v], ay[v], ca[v] * ey0[v]);
+          ldv(p.Ca[2] + o, ca); ldv(p.Cb[2] + o, cb);
+#pragma unroll
+          for (int v = 0; v < V; ++v) ez[v] = fma(cb[v], az[v], ca[v] * ez[v]);
+        } else {
+#pragma unroll
+          for (int v = 0; v < V; ++v) {
+            const Vec4<T> a = lds4(tab + 8 * (int)mi[v]), b = lds4(tab + 8 * (int)mi[v] + 4);
+            ex[v] = fma(a.d, ax[v], a.a * ex0[v]);
+            ey[v] = fma(b.a, ay[v], a.b * ey0[v]);
+            ez[v] = fma(b.b, az[v], a.c * ez[v]);
+          }
+        }
+        // PEC walls: low-face tangential E stays zero (R1)
+        if (k == 0) {
+#pragma unroll
+          for (int v = 0; v < V; ++v) { ex[v] = T(0); ey[v] = T(0); }
+        }
+        if (wj) {
+#pragma unroll
+          for (int v = 0; v < V; ++v) { ex[v] = T(0); ez[v] = T(0); }
+        }
+        if (wi) { ey[0] = T(0); ez[0] = T(0); }
+        if (xtail) {  // pad columns i >= nx stay zero: they are the high-face PEC wall (R1)
+#pragma unroll
+          for (int v = 0; v < V; ++v) if (v >= nvalid) { ex[v] = T(0); ey[v] = T(0); ez[v] = T(0); }
+        }
+        stv_stream(p.dst[kEx] + o, ex); stv_stream(p.dst[kEy] + o, ey); stv_stream(p.dst[kEz] + o, ez);
+      }
+    } else {
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&empty[s]);
+    }
+#pragma unroll
+    for (int v = 0; v < V; ++v) { ex0[v] = ex1[v]; ey0[v] = ey1[v]; exj0[v] = exj1[v]; }
+    eyi0 = eyi1;
+    if (it >= 1) {
+#pragma unroll
+      for (int v = 0; v < V; ++v) { hxm[v] = hx[v]; hym[v] = hy[v]; }
     }
     if (++s == NS) { s = 0; ph ^= 1u; }
   }
