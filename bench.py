@@ -40,6 +40,14 @@ METRIC = "Mcell-updates/s per Yee E+H step"
 UNIT = "Mcell-updates/s"
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch, from the ncu captures summarised under profiles/
+NCU_TRAFFIC = {
+    ("c3", "k_step_fused", 32): (49.30e9, "profiles/r01_fused_v4.md (26.09 GB read + 23.21 GB written)"),
+    ("c3", "k_update_E", 32): (35.24e9, "profiles/r01_twopass.md"),
+    ("c3", "k_update_H", 32): (34.39e9, "profiles/r01_twopass.md"),
+}
+
+
 def workload(name, steps):
     import workloads as W
     if name == "c3":
@@ -266,8 +274,10 @@ def run_ours(args, rank, world, local_rank):
     peak, peak_src = measured_peak()
     achieved = ab / (kms * 1e-3) / 1e9
     step_bytes = algorithmic_bytes(w, impl, "H") + (algorithmic_bytes(w, impl, "E") if impl != "fused" else 0)
+    # DRAM bytes of one launch from the committed `ncu --set full` capture of this workload and kernel (profiles/), else null
+    traffic, traffic_src = NCU_TRAFFIC.get((args.workload, kname, w["precision"]), (None, None))
     roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": ab, "kernel_ms": kms,
                 "kernel_ms_all": {"H_or_fused": ms[0], "E": ms[1], "source": ms[2], "probe_dft": ms[3]},
                 "bytes_per_cell_update_step": step_bytes / n_cells,
