@@ -309,7 +309,7 @@ def run_ours(args, rank, world, local_rank):
             "dtype": "f32" if w["precision"] == 32 else "f64", "data": "synthetic",
             "config": {"workload": args.workload, "grid": [w["nx"], w["ny"], w["nz"]], "cells": n_cells,
                        "materials": m["mode"], "cpml_cells": w["pml"], "ports": len(w["ports"]), "dft_freqs": len(w["freqs"]),
-                       "step_impl": impl, "l2": "inputs larger than L2 (no flush needed)" if n_cells * 24 > 2.6e8 else
+                       "step_impl": impl, "fused_kz": s.fused_kz, "l2": "inputs larger than L2 (no flush needed)" if n_cells * 24 > 2.6e8 else
                        "grid fits in L2: launch-bound case, not a roofline case",
                        "parallelism": "replicas only" if world > 1 else "1 GPU", "library": os.path.basename(binding.library_path())},
             "clocks": ck, "e2e": e2e, "gpu_launches": launches, "roofline": roofline}

@@ -50,11 +50,12 @@ enum { FDTD_EX = 0, FDTD_EY, FDTD_EZ, FDTD_HX, FDTD_HY, FDTD_HZ };
 
 /* Options for fdtd_set_option (before commit). */
 enum {
-  FDTD_OPT_STEP_IMPL = 1,   /* 0 = auto (fused from 4 Mi cells up), 1 = two-pass (H kernel, E kernel, in place),
+  FDTD_OPT_STEP_IMPL = 1,   /* 0 = auto (two-pass below 4 Mi cells; above, whichever fdtd_commit measures faster),
+                               1 = two-pass (H kernel, E kernel, in place),
                                2 = fused E+H kernel (temporal blocking over the half steps; a second field set)         */
   FDTD_OPT_USE_GRAPH = 2,   /* 1 (default) = replay a captured CUDA graph per step; 0 = plain launches                  */
   FDTD_OPT_GRAPH_UNROLL = 3,/* steps per captured graph (default 8; rounded up to even for the fused step)              */
-  FDTD_OPT_FUSED_KZ = 4     /* planes per z chunk of the fused kernel (0 = auto)                                        */
+  FDTD_OPT_FUSED_KZ = 4     /* planes per z chunk of the fused kernel (0 = auto: measured at commit)                    */
 };
 
 /* A port (Fig. 1a): a soft E_z source on a box of the plane i = is (surface 'e'), a voltage box and
@@ -149,6 +150,10 @@ long fdtd_step_count(const fdtd_t*);
 long fdtd_launch_count(const fdtd_t*);
 /* Name of the step implementation in use after commit ("two_pass", "fused"), for reports. */
 const char* fdtd_impl_name(const fdtd_t*);
+/* z chunk length of the fused step in use after commit (0 for the two-pass step), for reports.  With
+ * FDTD_OPT_STEP_IMPL = 0 or FDTD_OPT_FUSED_KZ = 0, fdtd_commit times the candidates on the committed all-zero state
+ * (two-pass and fused with 12..48 planes per chunk) and keeps the fastest; the state is left exactly as committed. */
+int fdtd_fused_kz(const fdtd_t*);
 const char* fdtd_last_error(const fdtd_t*);
 void fdtd_destroy(fdtd_t*);
 

@@ -63,6 +63,7 @@ SYMBOLS = {
     "fdtd_step_count": (C.c_long, [_vp]),
     "fdtd_launch_count": (C.c_long, [_vp]),
     "fdtd_impl_name": (C.c_char_p, [_vp]),
+    "fdtd_fused_kz": (C.c_int, [_vp]),
     "fdtd_last_error": (C.c_char_p, [_vp]),
     "fdtd_destroy": (None, [_vp]),
 }
@@ -224,6 +225,10 @@ def fdtd_launch_count(h) -> int:
 
 def fdtd_impl_name(h) -> str:
     return lib().fdtd_impl_name(h).decode()
+
+
+def fdtd_fused_kz(h) -> int:
+    return int(lib().fdtd_fused_kz(h))
 
 
 def fdtd_last_error(h) -> str:

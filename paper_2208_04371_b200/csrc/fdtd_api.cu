@@ -88,6 +88,7 @@ struct fdtd {
   virtual int read_port_last(int port, double* V, double* I) = 0;
   virtual int reset() = 0;
   virtual const char* impl_name() const = 0;
+  virtual int fused_kz() const = 0;
 };
 
 namespace {
@@ -113,6 +114,7 @@ struct Solver : fdtd {
   bool fused = false;
   int cur = 0;
   int kz = 0;
+  double tuned_ms = 0.0;     // field-kernel time of the configuration autotune() kept
   FusedParams<T> fpar[2];
   cudaGraphExec_t gexec2 = nullptr;  // graph captured with cur == 1
   std::vector<T> h_tab;        // host staging of the material table (kept alive for the async upload)
@@ -182,7 +184,10 @@ struct Solver : fdtd {
   int read_port_last(int port, double* V, double* I) override;
   int reset() override;
   const char* impl_name() const override { return fused ? "fused" : "two_pass"; }
+  int fused_kz() const override { return fused ? kz : 0; }
   int build_fused();
+  int autotune();
+  double time_field_kernels(int reps);
   void launch_fused(cudaEvent_t* ev);
 
   int copy_field(int comp, void* user, bool to_user);
@@ -296,6 +301,7 @@ int Solver<T>::commit(void* w, size_t bytes, void* st) {
   cur = 0;
   if (fused) {
     pp2.Ez = field_origin(kEz, 1); pp2.Hy = field_origin(kHy, 1); pp2.Hz = field_origin(kHz, 1);
+    kz = opt_kz > 0 ? (int)opt_kz : 32;
     const int r = build_fused();
     if (r != FDTD_OK) return r;
   }
@@ -322,6 +328,10 @@ int Solver<T>::commit(void* w, size_t bytes, void* st) {
   }
   if ((e = cudaStreamSynchronize(stream)) != cudaSuccess) return cuda_fail(e, "fdtd_commit");
   if ((e = cudaGetLastError()) != cudaSuccess) return cuda_fail(e, "fdtd_commit");
+  if (fused && (opt_impl == 0 || opt_kz <= 0)) {
+    const int r = autotune();
+    if (r != FDTD_OK) return r;
+  }
   committed = true;
   nstep = 0;
   launches = 0;
@@ -491,9 +501,10 @@ int Solver<T>::build_fused() {
   // two chunks of each other in z: short chunks keep their 13 streams inside a narrow band of planes (measured on C3:
   // 9.0 ms/step at 128 planes, 8.2 ms at 24..32, 8.4 ms at 16 where the two priming planes per chunk start to cost).
   const long long tiles = (long long)((nx + C::TX - 1) / C::TX) * ((ny + C::TY - 1) / C::TY);
-  kz = opt_kz > 0 ? (int)opt_kz : 32;
-  if (opt_kz <= 0) while (kz > 8 && tiles * ((nz + kz - 1) / kz) < 2 * 148) kz /= 2;
+  // fdtd_commit then times the candidates on the committed (all-zero) state and keeps the fastest: autotune().
+  (void)tiles;
   if (kz > nz) kz = nz;
+  if (kz < 1) kz = 1;
 
   const cuuint64_t gdim[3] = {(cuuint64_t)pitch(), (cuuint64_t)(ny + 1), (cuuint64_t)(nz + 2)};
   const cuuint32_t estr[3] = {1, 1, 1};
@@ -524,6 +535,75 @@ int Solver<T>::build_fused() {
       fp.tm[6] = fp.tm[0];
     }
   }
+  return FDTD_OK;
+}
+
+// Device time (ms) of one launch of the field kernels of the current choice (fused / two-pass, kz), averaged over reps
+// launches after one warm-up.  Runs on the freshly committed state: all fields and psi are zero and the kernels add no
+// source, so the state stays zero; the device step counter is put back afterwards.
+template <typename T>
+double Solver<T>::time_field_kernels(int reps) {
+  cudaEvent_t a, b;
+  if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return -1.0;
+  auto once = [&]() {
+    if (fused) launch_fused(nullptr);
+    else switch (mode()) {
+      case 0: launch_two_pass<T, 0>(sp, stream, nullptr); break;
+      case 1: launch_two_pass<T, 1>(sp, stream, nullptr); break;
+      case 2: launch_two_pass<T, 2>(sp, stream, nullptr); break;
+      default: launch_two_pass<T, 3>(sp, stream, nullptr); break;
+    }
+  };
+  once();
+  cudaEventRecord(a, stream);
+  for (int q = 0; q < reps; ++q) once();
+  cudaEventRecord(b, stream);
+  float ms = -1.f;
+  if (cudaEventSynchronize(b) != cudaSuccess || cudaEventElapsedTime(&ms, a, b) != cudaSuccess) ms = -1.f;
+  cudaEventDestroy(a); cudaEventDestroy(b);
+  cur = 0;
+  return ms < 0.f ? -1.0 : (double)ms / reps;
+}
+
+// Choice of the step implementation and of the z chunk length, measured rather than modelled.  How well the fused kernel
+// does depends on how the (tile, chunk) blocks fill the SMs (mid-size grids give only a few waves of blocks) and on how far
+// apart in z the co-resident blocks drift; both are properties of this grid on this device.
+//   FDTD_OPT_STEP_IMPL 0 (auto): two-pass and fused with kz in {12, 16, 24, 32, 48} compete;
+//   FDTD_OPT_STEP_IMPL 2 with FDTD_OPT_FUSED_KZ 0: the kz candidates compete.
+template <typename T>
+int Solver<T>::autotune() {
+  const int reps = (long long)nx * ny * nz >= (64LL << 20) ? 2 : 4;
+  double best = -1.0;
+  int best_kz = kz;
+  bool best_fused = true;
+  if (opt_kz <= 0) {
+    const int cand[5] = {12, 16, 24, 32, 48};
+    for (int c = 0; c < 5; ++c) {
+      if (cand[c] > nz && c > 0) break;
+      kz = cand[c] > nz ? nz : cand[c];
+      fpar[0].kz = fpar[1].kz = kz;
+      const double t = time_field_kernels(reps);
+      if (t < 0) return fail(FDTD_ECUDA, "fdtd_commit: timing the fused kernel failed: %s", cudaGetErrorString(cudaGetLastError()));
+      if (best < 0 || t < best) { best = t; best_kz = kz; }
+    }
+  } else {
+    best = time_field_kernels(reps);
+    if (best < 0) return fail(FDTD_ECUDA, "fdtd_commit: timing the fused kernel failed: %s", cudaGetErrorString(cudaGetLastError()));
+  }
+  if (opt_impl == 0) {
+    fused = false;
+    const double t = time_field_kernels(reps);
+    if (t < 0) return fail(FDTD_ECUDA, "fdtd_commit: timing the two-pass kernels failed: %s", cudaGetErrorString(cudaGetLastError()));
+    if (t < best) { best = t; best_fused = false; }
+  }
+  fused = best_fused;
+  kz = best_kz;
+  fpar[0].kz = fpar[1].kz = kz;
+  cur = 0;
+  tuned_ms = best;
+  cudaError_t e = cudaMemsetAsync(sp.nstep, 0, sizeof(long long), stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+  if (e != cudaSuccess) return cuda_fail(e, "fdtd_commit: autotune");
   return FDTD_OK;
 }
 
@@ -800,6 +880,7 @@ int fdtd_reset(fdtd_t* h) { return h ? h->reset() : FDTD_EINVAL; }
 long fdtd_step_count(const fdtd_t* h) { return h ? h->nstep : -1; }
 long fdtd_launch_count(const fdtd_t* h) { return h ? h->launches : -1; }
 const char* fdtd_impl_name(const fdtd_t* h) { return h && h->committed ? h->impl_name() : ""; }
+int fdtd_fused_kz(const fdtd_t* h) { return h && h->committed ? h->fused_kz() : 0; }
 const char* fdtd_last_error(const fdtd_t* h) { return h ? h->err.c_str() : "null handle"; }
 void fdtd_destroy(fdtd_t* h) { delete h; }
 

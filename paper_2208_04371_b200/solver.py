@@ -104,6 +104,10 @@ class Solver:
     def impl_name(self):
         return B.fdtd_impl_name(self.h)
 
+    @property
+    def fused_kz(self):
+        return B.fdtd_fused_kz(self.h)
+
     def synchronize(self):
         self.stream.synchronize()
 
