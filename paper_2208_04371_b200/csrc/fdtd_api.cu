@@ -157,8 +157,12 @@ struct Solver : fdtd {
     }
     for (int q = 0; q < 12; ++q) c.psi[q] = take(psi_elems(psi_axis(q)) * sizeof(T));
     if (want_fused()) for (int q = 0; q < 6; ++q) c.psiH2[q] = take(psi_elems(psi_axis(q)) * sizeof(T));
-    for (int a = 0; a < 3; ++a)
-      for (int v = 0; v < 6; ++v) c.vec[a * 6 + v] = take((size_t)(S(a) > 0 ? S(a) : 1) * sizeof(T));
+    {  // 18 CPML vectors in one block, [axis][bE cE kE bH cH kH][stride]: the fused kernel copies it to shared memory whole
+      int stride = kMaxSlab;
+      for (int a = 0; a < 3; ++a) if (S(a) > stride) stride = (S(a) + 3) / 4 * 4;
+      const size_t base = take((size_t)18 * stride * sizeof(T));
+      for (int q = 0; q < 18; ++q) c.vec[q] = base + (size_t)q * stride * sizeof(T);
+    }
     c.ports = take((ports.size() + 1) * sizeof(PortDev));
     c.freqs = take((freqs.size() + 1) * sizeof(double));
     c.dftV = take((ports.size() * freqs.size() + 1) * 2 * sizeof(double));
@@ -524,6 +528,7 @@ int Solver<T>::build_fused() {
       fp.sp.psi[q] = reinterpret_cast<T*>(ws + (c ? cv.psi[q] : cv.psiH2[q]));
     }
     fp.kz = kz;
+    fp.cpack = reinterpret_cast<const T*>(ws + cv.vec[0]);   // stride kMaxSlab: build_fused runs only when slabs_fit()
     for (int f = 0; f < 6; ++f) {
       if (!make(&fp.tm[f], ws + (c ? cv.field2[f] : cv.field[f]), fdt, sizeof(T), C::xw(f), C::nr(f)))
         return fail(FDTD_ECUDA, "fdtd_commit: cuTensorMapEncodeTiled failed for field %d", f);

@@ -40,6 +40,7 @@ struct FusedParams {
   StepParams<T> sp;      // src = set read, dst = set written; psi[0..5] = psi_H written, psi[6..11] = psi_E (in place)
   const T* psiH_src[6];  // psi_H read (pHxy pHzy pHxz pHyz pHyx pHzx)
   int kz;                // planes per z chunk (grid.z = ceil(nz / kz))
+  const T* cpack;        // the 18 CPML vectors [axis][bE cE kE bH cH kH][kMaxSlab], contiguous
 };
 
 __host__ __device__ constexpr int round128(int v) { return (v + 127) / 128 * 128; }
@@ -245,23 +246,21 @@ __global__ void __launch_bounds__((TY + 2) * 32, 1) k_step_fused(const __grid_co
       for (int r = 0; r < TY; ++r) mbar_init(&rowrdy[s * TY + r], 1);
     }
     mbar_fence_init();
-#pragma unroll
-    for (int q = 0; q < 7; ++q) tma_prefetch_desc(&fp.tm[q]);
-  }
-  if (!kFull) {
-    for (int q = threadIdx.x; q < kTabH; q += C::THREADS) tab[q] = p.tab[q];
-  }
-  for (int a = 0; a < 3; ++a) {  // CPML vectors -> shared memory
-    const int S = p.lo[a] + p.hi[a];
-    const T* const src[6] = {p.bE[a], p.cE[a], p.kE[a], p.bH[a], p.cH[a], p.kH[a]};
-#pragma unroll
-    for (int v = 0; v < 6; ++v)
-      for (int q = threadIdx.x; q < S; q += C::THREADS) cpv[(a * 6 + v) * kMaxSlab + q] = src[v][q];
-  }
-  __syncthreads();
-  if (threadIdx.x == 0) {
+    // the first NS planes are requested before anything else so that their latency overlaps the table copies below
     for (int it = 0; it < NS && it < nIt; ++it) issue(it, it);
   }
+  {  // material table (E records) and CPML vectors -> shared memory, 128 bits per thread and round
+    constexpr int W4 = 16 / (int)sizeof(T);
+    if (!kFull) {
+      const float4* src = reinterpret_cast<const float4*>(p.tab);
+      float4* dst = reinterpret_cast<float4*>(tab);
+      for (int q = threadIdx.x; q < kTabH / W4; q += C::THREADS) dst[q] = __ldg(src + q);
+    }
+    const float4* src = reinterpret_cast<const float4*>(fp.cpack);
+    float4* dst = reinterpret_cast<float4*>(cpv);
+    for (int q = threadIdx.x; q < 18 * kMaxSlab / W4; q += C::THREADS) dst[q] = __ldg(src + q);
+  }
+  __syncthreads();
 
   // ---- loop invariants ------------------------------------------------------------------------------------------------
   const bool rowwarp = w >= 1;
