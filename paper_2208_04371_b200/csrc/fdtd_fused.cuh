@@ -222,9 +222,11 @@ __global__ void __launch_bounds__((TY + 2) * 32, 1) k_step_fused(const __grid_co
     const int k = k0 - 2 + it;
     unsigned char* st = smem + s * C::STAGE;
     const bool want_idx = !kFull && it >= 2;
+    // it = 1 (plane k0-1) exists only for its new Hx, Hy (the k-1 operands of plane k0): old Hz is not needed there
     const unsigned bytes = it == 0 ? (unsigned)(C::tx_bytes(kEx) + C::tx_bytes(kEy))
                                    : (unsigned)(C::tx_bytes(kEx) + C::tx_bytes(kEy) + C::tx_bytes(kEz) + C::tx_bytes(kHx) +
-                                                C::tx_bytes(kHy) + C::tx_bytes(kHz)) + (want_idx ? (unsigned)C::I_TX : 0u);
+                                                C::tx_bytes(kHy)) + (it >= 2 ? (unsigned)C::tx_bytes(kHz) : 0u) +
+                                         (want_idx ? (unsigned)C::I_TX : 0u);
     mbar_expect_tx(&full[s], bytes);
     // Ex, Ey: plane k+1 (array plane index + 1); the rest: plane k
     tma_load_3d(st + C::off(kEx), &fp.tm[kEx], &full[s], x0 - C::xl(kEx), y0 + C::r0(kEx), k + 2);
@@ -233,7 +235,7 @@ __global__ void __launch_bounds__((TY + 2) * 32, 1) k_step_fused(const __grid_co
       tma_load_3d(st + C::off(kEz), &fp.tm[kEz], &full[s], x0 - C::xl(kEz), y0 + C::r0(kEz), k + 1);
       tma_load_3d(st + C::off(kHx), &fp.tm[kHx], &full[s], x0 - C::xl(kHx), y0 + C::r0(kHx), k + 1);
       tma_load_3d(st + C::off(kHy), &fp.tm[kHy], &full[s], x0 - C::xl(kHy), y0 + C::r0(kHy), k + 1);
-      tma_load_3d(st + C::off(kHz), &fp.tm[kHz], &full[s], x0 - C::xl(kHz), y0 + C::r0(kHz), k + 1);
+      if (it >= 2) tma_load_3d(st + C::off(kHz), &fp.tm[kHz], &full[s], x0 - C::xl(kHz), y0 + C::r0(kHz), k + 1);
       if (want_idx) tma_load_3d(st + C::I_OFF, &fp.tm[6], &full[s], x0, y0, k + 1);
     }
   };

@@ -20,3 +20,35 @@ def s_star_column(j, V_inc, I_inc, V_tot):
     S = V_tot / V_inc[j][None, :] * np.sqrt(zr[j][None, :] / zr)
     S[j] = (V_tot[j] - V_inc[j]) / V_inc[j]
     return S
+
+
+def renormalize(S_star, Z_r, z_new=50.0):
+    """S* (power waves on the per-port reference impedances Z_r) -> S on z_new ohm at every port (Eq. 5-6,
+    PAPER.md:68-87, after Reveyrand; readings R29 in DESIGN.md).  S_star: [N, N, F], Z_r: [N, F] with Re Z_r > 0
+    (orient the current along the incident wave).  Returns [N, N, F].
+
+        B = (z_new - Z_r) / (z_new + conj Z_r)          (diagonal; the printed form is the identity, R29)
+        A = sqrt(z_new) / sqrt|Re Z_r| * (1 - conj B)   (diagonal, Eq. 6: G = 1/sqrt|Re Z_r|, G* = 1/sqrt(z_new))
+        S = A^-1 (S* - conj B) (I - B S*)^-1 conj A
+    Solved per frequency with one batched linear solve instead of explicit inverses.
+    """
+    S = np.moveaxis(np.asarray(S_star, dtype=np.complex128), 2, 0)          # [F, N, N]
+    Z = np.asarray(Z_r, dtype=np.complex128).T                              # [F, N]
+    n = Z.shape[1]
+    b = (z_new - Z) / (z_new + np.conj(Z))
+    a = np.sqrt(z_new) / np.sqrt(np.abs(Z.real)) * (1.0 - np.conj(b))
+    eye = np.eye(n)[None]
+    num = S - np.conj(b)[:, :, None] * eye                                   # S* - conj B
+    den = eye - b[:, :, None] * S                                            # I - B S*
+    # X = num den^-1  <=>  den^T X^T = num^T
+    X = np.swapaxes(np.linalg.solve(np.swapaxes(den, 1, 2), np.swapaxes(num, 1, 2)), 1, 2)
+    out = X * np.conj(a)[:, None, :] / a[:, :, None]                         # A^-1 X conj A
+    return np.moveaxis(out, 0, 2)
+
+
+def phase_delay(s, freqs):
+    """Eq. 8: tau = theta / (360 f), theta = phase of S*_ij in degrees unwrapped along frequency.
+    With this library's DFT kernel e^{-j 2 pi f t} a delayed signal has a falling phase, so tau is negative for a
+    physical delay; the paper's sign is that of its own time convention (R30)."""
+    th = np.degrees(np.unwrap(np.angle(np.asarray(s, dtype=np.complex128))))
+    return th / (360.0 * np.asarray(freqs, dtype=np.float64))

@@ -1,0 +1,55 @@
+"""The full N-port protocol: drive every port, inc + tot run each, S* by
+Eq. 1-2, S on 50 ohm by Eq. 5-6, phase delay by Eq. 8 -- GPU path (paper_2208_04371_b200.nport) against the same protocol
+written out here with the CPU oracle and its own post-processing (oracle/sparams.py, oracle/renorm.py)."""
+import numpy as np
+import pytest
+
+import workloads as W
+from oracle import renorm as orn
+from oracle import sparams as osp
+from oracle.yee import YeeOracle
+from paper_2208_04371_b200 import nport
+
+pytestmark = pytest.mark.gpu
+
+STEPS = 1500
+
+
+def _wl(run):
+    return W.interconnect_c2(run=run, div=4, steps=STEPS, npml=6, nf=24)
+
+
+def _oracle_protocol():
+    w_inc, w_tot = _wl("inc"), _wl("tot")
+    n, nf = len(w_inc["ports"]), len(w_inc["freqs"])
+    S = [[[0j] * nf for _ in range(n)] for _ in range(n)]
+    Z = [[0j] * nf for _ in range(n)]
+    for j in range(n):
+        runs = {}
+        for name, w in (("inc", w_inc), ("tot", w_tot)):
+            wj, d = W.drive_port(w, j)
+            o = YeeOracle.from_workload(wj)
+            o.step(STEPS)
+            runs[name] = [o.read_port_dft(p) for p in range(n)]
+        Vi = [runs["inc"][p][0] for p in range(n)]
+        Ii = [runs["inc"][p][1] for p in range(n)]
+        Vt = [runs["tot"][p][0] for p in range(n)]
+        col = osp.s_star_column(j, Vi, Ii, Vt)
+        for p in range(n):
+            S[p][j] = list(col[p])
+        Z[j] = [-d * v / i for v, i in zip(Vi[j], Ii[j])]
+    return np.array(S), np.array(Z), np.array(orn.renormalize(S, Z))
+
+
+def test_two_port_protocol_matches_the_oracle_protocol():
+    res = nport.extract(_wl, W.drive_port, steps=STEPS)
+    So, Zo, S50o = _oracle_protocol()
+    assert np.abs(res["S_star"] - So).max() <= 1e-3
+    assert np.abs(res["S"] - S50o).max() <= 1e-3
+    assert np.abs(res["Z_r"] - Zo).max() <= 1e-3 * np.abs(Zo).max()
+    assert (res["Z_r"].real > 0).all()                                   # oriented along the incident wave (R31)
+    # the structure is reciprocal: S*_12 = S*_21 (the stub sits between the ports; both columns come from different runs)
+    assert np.abs(res["S_star"][0, 1] - res["S_star"][1, 0]).max() <= 2e-2
+    tau_o = np.array(orn.phase_delay(list(So[1, 0]), list(res["freqs"])))
+    assert np.abs(res["tau"][1, 0] - tau_o).max() <= 1e-3 * np.abs(tau_o).max() + 1e-18
+    assert np.isnan(res["tau"][0, 0]).all()

@@ -345,6 +345,30 @@ def random_box(seed, nx=20, ny=14, nz=12, pml=(3, 4, 2, 3, 0, 3), indexed=True, 
                 freqs=np.linspace(0.2 * fmax, 2 * fmax, nf), steps=steps)
 
 
+def drive_port(w, j):
+    """Copy of workload w in which port j carries the (single) source instead of the port that has it now.
+
+    The waveform is kept; the source box becomes port j's voltage box, on a plane as far outside port j (towards the nearer
+    x end of the line) as the original source plane is outside its own port.  Returns (workload, direction): direction is
+    +1 when the incident wave crosses port j travelling towards +x, -1 otherwise (one inc/tot pair of
+    runs per driving port).  Input bookkeeping only: none of the method's arithmetic lives here."""
+    ports = [dict(q) for q in w["ports"]]
+    src = [q for q in ports if q["has_source"]]
+    assert len(src) == 1, "drive_port expects exactly one driving port"
+    s0 = src[0]
+    off = abs(s0["ip"] - s0["is"])
+    wave = {k: s0[k] for k in ("waveform", "amp", "t0", "sigma", "f0")}
+    for q in ports:
+        q.update(has_source=0, amp=0.0)
+    t = ports[j]
+    direction = 1 if t["ip"] < w["nx"] // 2 else -1
+    t.update(wave)
+    t.update({"has_source": 1, "is": t["ip"] - direction * off, "sj0": t["vj0"], "sj1": t["vj1"], "sk0": t["vk0"],
+              "sk1": t["vk1"]})
+    assert 0 <= t["is"] < w["nx"]
+    return dict(w, ports=ports), direction
+
+
 def get(name, **kw):
     return {"c0": cavity_c0, "c1": microstrip_c1, "c2": interconnect_c2, "c3": throughput_c3,
             "c4": interconnect_c4}[name](**kw)
