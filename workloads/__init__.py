@@ -164,6 +164,31 @@ def microstrip_c1(seed=2209, nx=192, steps=40000, precision=32, waveform=W_GAUSS
 
 
 # --------------------------------------------------------------------------------------------------
+# X1  the paper's microstrip verification case at paper size
+# --------------------------------------------------------------------------------------------------
+def microstrip_x1(nx=1000, steps=60000, precision=32, nf=79, f_hi=40e9, npml=10):
+    """Z0 = 25 ohm microstrip: eps_r = 3.8, h = 1 mm = 10 cells, w/h = 5.7 (57 cells), length 100 h = 1000 cells,
+    200 x 1000 x 50 cells of 0.1 mm (the paper's propagation axis y is x here), CFL number 0.9 (dt = 0.173 ps),
+    differentiated-Gaussian pulse sigma = 11.254 ps, t0 = 3 sigma (Eq. 3), 60 000 steps.  Not in the paper: the PML depth
+    (10 cells), the port planes (100 cells from either end), the strip thickness (a PEC sheet), the DFT band."""
+    ny, nz, d = 200, 50, 1e-4
+    dt = 0.9 * cfl_limit(d, d, d)
+    pt = Painter(nx, ny, nz)
+    pt.layers([0, 10, nz], [3.8, 1.0])
+    j0, j1 = 72, 129                                     # 57 cells wide, centred
+    pt.conductor(0, nx, j0, j1, 10, 10)                  # zero-thickness PEC sheet on the plane k = 10
+    sig = 11.254e-12
+    src = {"is": 60, "sj0": j0, "sj1": j1, "sk0": 0, "sk1": 10, "waveform": W_DGAUSS, "amp": 1.0,
+           "t0": 3 * sig, "sigma": sig, "f0": 0.0}
+    box = dict(vj0=j0, vj1=j1, vk0=0, vk1=10, lj0=j0 - 1, lj1=j1 + 1, lk0=9, lk1=11)
+    ports = [_port(ip=100, source=src, **box), _port(ip=nx - 100, **box)]
+    return dict(name="x1", nx=nx, ny=ny, nz=nz, dx=d, dy=d, dz=d, dt=dt, precision=precision,
+                pml=[npml, npml, npml, npml, 0, npml], cpml=[3.0, 1.0, 1.0, 0.0, 0.8, 2.4], materials=pt.indexed(),
+                ports=ports, freqs=np.linspace(f_hi / (nf + 1), f_hi, nf), steps=steps,
+                theory=dict(z0=25.0, eps_r=3.8, w_over_h=5.7, gamma=-0.333))
+
+
+# --------------------------------------------------------------------------------------------------
 # C2 / C4  CMOS-like multilayer interconnect (C4 = C2 with every extent x2, fp64, full uniaxial arrays)
 # --------------------------------------------------------------------------------------------------
 def _interconnect(seed, mult, div, run, full, precision, npml, nf, sig_dt, nports, steps):
