@@ -1,6 +1,6 @@
 """bench.py -- throughput of the Yee FDTD hot path on config C3 (BASELINE.json: "Mcell-updates/s per Yee E+H step").
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload c3|c3s|c2|c4]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload c3|c3s|c2|c4|x3]
 
 One "step" is one full leapfrog step of the whole hot path (psi_H, H, psi_E, E, walls, source,
 probes, running DFT) over the whole grid.  One cell-update = all six components of one cell advanced one step (R27);
@@ -58,6 +58,8 @@ def workload(name, steps):
         return W.interconnect_c2(steps=steps)
     if name == "c4":
         return W.interconnect_c4(steps=steps)
+    if name == "x3":  # the paper's CMOS-line grid shape, 200x120x800 cells of (20, 50, 5) nm
+        return W.cmos_line_x3(steps=steps)
     raise SystemExit(f"unknown workload {name}")
 
 

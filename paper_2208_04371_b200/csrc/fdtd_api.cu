@@ -21,6 +21,7 @@
 #include "fdtd_fused.cuh"
 #include "fdtd_kernels.cuh"
 #include "fdtd_params.h"
+#include "fdtd_persistent.cuh"
 
 using namespace fdtd_b200;
 
@@ -103,7 +104,7 @@ template <typename T>
 struct Solver : fdtd {
   // workspace carve (byte offsets), filled by layout()
   struct Carve {
-    size_t field[6], field2[6], idx, tab, coef[9], psi[12], psiH2[6], vec[18], ports, freqs, dftV, dftI, lastV, lastI, nstep, total;
+    size_t field[6], field2[6], idx, tab, coef[9], psi[12], psiH2[6], vec[18], ports, freqs, dftV, dftI, lastV, lastI, nstep, partial, pcount, total;
   };
   char* ws = nullptr;
   Carve cv{};
@@ -112,8 +113,11 @@ struct Solver : fdtd {
   PortParams<T> pp2{};
   // fused step: two field sets (ping-pong); fpar[c] reads set c and writes set 1-c; cur = set holding the current state
   bool fused = false;
+  bool persistent = false;   // small grids: many steps per cooperative launch (fdtd_persistent.cuh)
+  int persist_blocks = 0;
   int cur = 0;
   int kz = 0;
+  unsigned probe_blocks = 1; // blocks per port of k_probe_dft: about 1024 samples of the largest V box each
   double tuned_ms = 0.0;     // field-kernel time of the configuration autotune() kept
   FusedParams<T> fpar[2];
   cudaGraphExec_t gexec2 = nullptr;  // graph captured with cur == 1
@@ -170,6 +174,8 @@ struct Solver : fdtd {
     c.lastV = take((ports.size() + 1) * sizeof(double));
     c.lastI = take((ports.size() + 1) * sizeof(double));
     c.nstep = take(sizeof(long long));
+    c.partial = take((ports.size() + 1) * kProbeMaxBlocks * 2 * sizeof(double));
+    c.pcount = take((ports.size() + 1) * sizeof(int));
     c.total = off;
     return c;
   }
@@ -187,10 +193,12 @@ struct Solver : fdtd {
   int read_port_dft(int port, double* V, double* I) override;
   int read_port_last(int port, double* V, double* I) override;
   int reset() override;
-  const char* impl_name() const override { return fused ? "fused" : "two_pass"; }
+  const char* impl_name() const override { return fused ? "fused" : (persistent ? "persistent" : "two_pass"); }
   int fused_kz() const override { return fused ? kz : 0; }
   int build_fused();
   int autotune();
+  int setup_persistent();
+  int launch_persistent(const PortParams<T>& q, long n);
   double time_field_kernels(int reps);
   void launch_fused(cudaEvent_t* ev);
 
@@ -291,6 +299,8 @@ int Solver<T>::commit(void* w, size_t bytes, void* st) {
   pp.dftI = reinterpret_cast<double*>(ws + cv.dftI);
   pp.lastV = reinterpret_cast<double*>(ws + cv.lastV);
   pp.lastI = reinterpret_cast<double*>(ws + cv.lastI);
+  pp.partial = reinterpret_cast<double*>(ws + cv.partial);
+  pp.pcount = reinterpret_cast<int*>(ws + cv.pcount);
   pp.nstep = sp.nstep;
   pp.dt = dt; pp.dy = dy; pp.dz = dz;
   if (!ports.empty() &&
@@ -300,6 +310,15 @@ int Solver<T>::commit(void* w, size_t bytes, void* st) {
       (e = cudaMemcpyAsync(ws + cv.freqs, freqs.data(), freqs.size() * sizeof(double), cudaMemcpyHostToDevice, stream)) != cudaSuccess)
     return cuda_fail(e, "fdtd_commit: upload frequencies");
 
+  {
+    long long most = 1;
+    for (const PortDev& d : ports) {
+      const long long nv = (long long)(d.vj1 - d.vj0 + 1) * (d.vk1 - d.vk0);
+      if (nv > most) most = nv;
+    }
+    const long long nb = (most + 1023) / 1024;
+    probe_blocks = (unsigned)(nb < 1 ? 1 : (nb > kProbeMaxBlocks ? kProbeMaxBlocks : nb));
+  }
   pp2 = pp;
   fused = want_fused();
   cur = 0;
@@ -334,6 +353,10 @@ int Solver<T>::commit(void* w, size_t bytes, void* st) {
   if ((e = cudaGetLastError()) != cudaSuccess) return cuda_fail(e, "fdtd_commit");
   if (fused && (opt_impl == 0 || opt_kz <= 0)) {
     const int r = autotune();
+    if (r != FDTD_OK) return r;
+  }
+  if (!fused && (opt_impl == 0 || opt_impl == 3)) {
+    const int r = setup_persistent();
     if (r != FDTD_OK) return r;
   }
   committed = true;
@@ -612,6 +635,103 @@ int Solver<T>::autotune() {
   return FDTD_OK;
 }
 
+// ---- persistent multi-step kernel for small grids ---------------------------------------------------------------------
+template <typename T, int MODE>
+static cudaError_t persistent_launch(const StepParams<T>& sp, const PortParams<T>& q, int n, int blocks, cudaStream_t st) {
+  StepParams<T> a = sp;
+  PortParams<T> b = q;
+  void* args[3] = {&a, &b, &n};
+  return cudaLaunchCooperativeKernel(reinterpret_cast<void*>(k_steps_persistent<T, MODE>), dim3(blocks), dim3(kPersistThreads), args, 0, st);
+}
+template <typename T, int MODE>
+static cudaError_t persistent_occupancy(int* per_sm) {
+  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, k_steps_persistent<T, MODE>, kPersistThreads, 0);
+}
+
+template <typename T>
+int Solver<T>::launch_persistent(const PortParams<T>& q, long n) {
+  cudaError_t e = cudaSuccess;
+  while (n > 0 && e == cudaSuccess) {
+    const int m = (int)(n > (1L << 20) ? (1L << 20) : n);
+    switch (mode()) {
+      case 0: e = persistent_launch<T, 0>(sp, q, m, persist_blocks, stream); break;
+      case 1: e = persistent_launch<T, 1>(sp, q, m, persist_blocks, stream); break;
+      case 2: e = persistent_launch<T, 2>(sp, q, m, persist_blocks, stream); break;
+      default: e = persistent_launch<T, 3>(sp, q, m, persist_blocks, stream); break;
+    }
+    n -= m;
+  }
+  return e == cudaSuccess ? FDTD_OK : cuda_fail(e, "cooperative launch of the persistent step kernel");
+}
+
+// Small grids (two-pass regime): is one cooperative launch per batch of steps faster than a few launches per step?
+// FDTD_OPT_STEP_IMPL 3 forces it, 0 measures both on the committed zero state.  Neither side may disturb that state, so
+// the persistent kernel runs without ports and the two-pass side launches its field kernels plus the probe kernel once
+// per port kernel of a real step (probe + one per source; on zero fields the probe adds zeros to zero accumulators).
+template <typename T>
+int Solver<T>::setup_persistent() {
+  persistent = false;
+  int dev = 0, coop = 0, sms = 0, per_sm = 0;
+  int nsrc = 0;
+  for (const PortDev& d : ports) nsrc += d.has_source ? 1 : 0;
+  const long long nvec = (long long)((nx + VecOf<T>::V - 1) / VecOf<T>::V) * ny * nz;
+  bool ok = cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) == cudaSuccess && coop &&
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && nsrc <= kPersistMaxSrc &&
+            nvec < (1LL << 30);
+  if (ok) {
+    cudaError_t e;
+    switch (mode()) {
+      case 0: e = persistent_occupancy<T, 0>(&per_sm); break;
+      case 1: e = persistent_occupancy<T, 1>(&per_sm); break;
+      case 2: e = persistent_occupancy<T, 2>(&per_sm); break;
+      default: e = persistent_occupancy<T, 3>(&per_sm); break;
+    }
+    ok = e == cudaSuccess && per_sm >= 1;
+  }
+  if (!ok) {
+    cudaGetLastError();
+    if (opt_impl == 3) return fail(FDTD_ECUDA, "fdtd_commit: the persistent step needs cooperative launch, <= %d sources and < 2^30 cell vectors", kPersistMaxSrc);
+    return FDTD_OK;
+  }
+  long long want = (nvec + kPersistThreads - 1) / kPersistThreads;           // no more blocks than there is work
+  const long long cap = (long long)sms * (per_sm > 4 ? 4 : per_sm);
+  persist_blocks = (int)(want < cap ? (want < 1 ? 1 : want) : cap);
+  if (opt_impl == 3) { persistent = true; return FDTD_OK; }
+  // measure: 16 steps either way
+  const int reps = 16;
+  PortParams<T> none = pp;
+  none.nports = 0;
+  cudaEvent_t a, b, c;
+  if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess || cudaEventCreate(&c) != cudaSuccess)
+    return fail(FDTD_ECUDA, "fdtd_commit: timing failed");
+  auto two_pass_step = [&]() {
+    switch (mode()) {
+      case 0: launch_two_pass<T, 0>(sp, stream, nullptr); break;
+      case 1: launch_two_pass<T, 1>(sp, stream, nullptr); break;
+      case 2: launch_two_pass<T, 2>(sp, stream, nullptr); break;
+      default: launch_two_pass<T, 3>(sp, stream, nullptr); break;
+    }
+    if (!ports.empty())
+      for (int q = 0; q < 1 + nsrc; ++q) k_probe_dft<T><<<dim3(probe_blocks, (unsigned)ports.size(), 1), kProbeThreads, 0, stream>>>(pp);
+  };
+  two_pass_step();
+  int r = launch_persistent(none, 2);
+  cudaEventRecord(a, stream);
+  for (int q = 0; q < reps; ++q) two_pass_step();
+  cudaEventRecord(b, stream);
+  if (r == FDTD_OK) r = launch_persistent(none, reps);
+  cudaEventRecord(c, stream);
+  float ms2 = -1.f, msp = -1.f;
+  if (r != FDTD_OK || cudaEventSynchronize(c) != cudaSuccess || cudaEventElapsedTime(&ms2, a, b) != cudaSuccess ||
+      cudaEventElapsedTime(&msp, b, c) != cudaSuccess) msp = -1.f;
+  cudaEventDestroy(a); cudaEventDestroy(b); cudaEventDestroy(c);
+  cudaError_t e = cudaMemsetAsync(sp.nstep, 0, sizeof(long long), stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+  if (e != cudaSuccess || msp < 0.f) return cuda_fail(e, "fdtd_commit: timing the persistent step kernel");
+  persistent = msp < ms2;
+  return FDTD_OK;
+}
+
 template <typename T>
 void Solver<T>::launch_fused(cudaEvent_t* ev) {
   if (ev) cudaEventRecord(ev[0], stream);
@@ -641,12 +761,15 @@ void Solver<T>::enqueue_step(cudaEvent_t* ev) {
   }
   const PortParams<T>& q = cur ? pp2 : pp;   // the set that now holds E^{n+1}, H^{n+1/2}
   if (!ports.empty()) {
-    bool any_src = false;
-    for (const PortDev& d : ports) any_src = any_src || d.has_source;
-    if (any_src) { k_source<T><<<1, 256, 0, stream>>>(q); ++launches; }
+    for (size_t n = 0; n < ports.size(); ++n) {   // one launch per driving port, in port order
+      const PortDev& d = ports[n];
+      if (!d.has_source) continue;
+      const int ns = (d.sj1 - d.sj0 + 1) * (d.sk1 - d.sk0);
+      k_source<T><<<(ns + 255) / 256, 256, 0, stream>>>(q, (int)n);
+      ++launches;
+    }
     if (ev) cudaEventRecord(ev[3], stream);
-    const dim3 grid((unsigned)ports.size(), (unsigned)(freqs.empty() ? 1 : (freqs.size() + 63) / 64), 1);
-    k_probe_dft<T><<<grid, 128, 0, stream>>>(q);
+    k_probe_dft<T><<<dim3(probe_blocks, (unsigned)ports.size(), 1), kProbeThreads, 0, stream>>>(q);
     ++launches;
     if (ev) cudaEventRecord(ev[4], stream);
   } else if (ev) {
@@ -704,13 +827,20 @@ int Solver<T>::step(long n) {
   if (!committed) return fail(FDTD_ESTATE, "fdtd_step: call after fdtd_commit");
   if (n < 0) return fail(FDTD_EINVAL, "fdtd_step: n < 0");
   long left = n;
+  if (persistent && n > 0) {
+    const int r = launch_persistent(pp, n);
+    if (r != FDTD_OK) return r;
+    launches += 1;
+    nstep += n;
+    return FDTD_OK;
+  }
   graph_steps = (int)opt_unroll + ((fused && (opt_unroll & 1)) ? 1 : 0);
   if (opt_graph && stream != nullptr && left >= graph_steps) {
     cudaGraphExec_t* g = cur ? &gexec2 : &gexec;
     const int r = build_graph(g);
     if (r != FDTD_OK) return r;
     long nodes = fused ? 1 : 2;
-    if (!ports.empty()) { nodes += 1; for (const PortDev& q : ports) if (q.has_source) { nodes += 1; break; } }
+    if (!ports.empty()) { nodes += 1; for (const PortDev& q : ports) if (q.has_source) nodes += 1; }
     while (left >= graph_steps) {
       const cudaError_t e = cudaGraphLaunch(*g, stream);
       if (e != cudaSuccess) return cuda_fail(e, "graph launch");
@@ -859,7 +989,7 @@ int fdtd_set_option(fdtd_t* h, int option, long value) {
   if (!h) return FDTD_EINVAL;
   if (h->committed) return h->fail(FDTD_ESTATE, "fdtd_set_option: call before fdtd_commit");
   switch (option) {
-    case FDTD_OPT_STEP_IMPL: if (value < 0 || value > 2) break; h->opt_impl = value; return FDTD_OK;
+    case FDTD_OPT_STEP_IMPL: if (value < 0 || value > 3) break; h->opt_impl = value; return FDTD_OK;
     case FDTD_OPT_USE_GRAPH: h->opt_graph = value ? 1 : 0; return FDTD_OK;
     case FDTD_OPT_GRAPH_UNROLL: if (value < 1 || value > 1024) break; h->opt_unroll = value; return FDTD_OK;
     case FDTD_OPT_FUSED_KZ: if (value < 0 || value > 65535) break; h->opt_kz = value; return FDTD_OK;

@@ -65,14 +65,10 @@ enum { kModeIndexed = 0, kModeFull = 1, kModeMu = 2 };
 // ------------------------------------------------------------------------------------------------------------------
 // H pass.  R5 step 1:  psiH = bH psiH + cH D+E ;  Hx -= Dbx (D+y Ez / kHy + psiHxy - D+z Ey / kHz - psiHxz)  etc.
 // ------------------------------------------------------------------------------------------------------------------
+// the H update of the V consecutive cells starting at (i0, j, k); i0 < nx, j < ny
 template <typename T, int MODE>
-__global__ void __launch_bounds__(128) k_update_H(const StepParams<T> p) {
+__device__ __forceinline__ void update_H_vec(const StepParams<T>& p, int i0, int j, int k) {
   constexpr int V = VecOf<T>::V;
-  const int i0 = (blockIdx.x * blockDim.x + threadIdx.x) * V;
-  const int j = blockIdx.y * blockDim.y + threadIdx.y;
-  const int k = blockIdx.z;
-  if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && threadIdx.x == 0 && threadIdx.y == 0) *p.nstep += 1;
-  if (i0 >= p.nx || j >= p.ny) return;
   const long long o = i0 + (long long)p.P * j + p.PS * k;
 
   T ex[V], ey[V], ez[V], exk[V], eyk[V], exj[V], ezj[V], hx[V], hy[V], hz[V];
@@ -170,17 +166,25 @@ __global__ void __launch_bounds__(128) k_update_H(const StepParams<T> p) {
   stv(p.dst[kHx] + o, hx); stv(p.dst[kHy] + o, hy); stv(p.dst[kHz] + o, hz);
 }
 
-// ------------------------------------------------------------------------------------------------------------------
-// E pass.  R5 step 2:  psiE = bE psiE + cE D-H ;  Ex = Cax Ex + Cbx (D-y Hz / kEy + psiExy - D-z Hy / kEz - psiExz) ...
-// then the low-face wall rows are forced to zero (PEC walls; PAPER.md:46 for the ground).
-// ------------------------------------------------------------------------------------------------------------------
 template <typename T, int MODE>
-__global__ void __launch_bounds__(128) k_update_E(const StepParams<T> p) {
+__global__ void __launch_bounds__(128) k_update_H(const StepParams<T> p) {
   constexpr int V = VecOf<T>::V;
   const int i0 = (blockIdx.x * blockDim.x + threadIdx.x) * V;
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
   const int k = blockIdx.z;
+  if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && threadIdx.x == 0 && threadIdx.y == 0) *p.nstep += 1;
   if (i0 >= p.nx || j >= p.ny) return;
+  update_H_vec<T, MODE>(p, i0, j, k);
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// E pass.  R5 step 2:  psiE = bE psiE + cE D-H ;  Ex = Cax Ex + Cbx (D-y Hz / kEy + psiExy - D-z Hy / kEz - psiExz) ...
+// then the low-face wall rows are forced to zero (PEC walls; PAPER.md:46 for the ground).
+// ------------------------------------------------------------------------------------------------------------------
+// the E update of the V consecutive cells starting at (i0, j, k); i0 < nx, j < ny
+template <typename T, int MODE>
+__device__ __forceinline__ void update_E_vec(const StepParams<T>& p, int i0, int j, int k) {
+  constexpr int V = VecOf<T>::V;
   const long long o = i0 + (long long)p.P * j + p.PS * k;
 
   T hx[V], hy[V], hz[V], hxk[V], hyk[V], hxj[V], hzj[V], ex[V], ey[V], ez[V];
@@ -279,6 +283,16 @@ __global__ void __launch_bounds__(128) k_update_E(const StepParams<T> p) {
   stv(p.dst[kEx] + o, ex); stv(p.dst[kEy] + o, ey); stv(p.dst[kEz] + o, ez);
 }
 
+template <typename T, int MODE>
+__global__ void __launch_bounds__(128) k_update_E(const StepParams<T> p) {
+  constexpr int V = VecOf<T>::V;
+  const int i0 = (blockIdx.x * blockDim.x + threadIdx.x) * V;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z;
+  if (i0 >= p.nx || j >= p.ny) return;
+  update_E_vec<T, MODE>(p, i0, j, k);
+}
+
 // ------------------------------------------------------------------------------------------------------------------
 // Port work.  The device step counter was already incremented by the first kernel of the step.
 // ------------------------------------------------------------------------------------------------------------------
@@ -292,21 +306,18 @@ __device__ __forceinline__ double waveform_dev(int kind, double t, double t0, do
   return 0.0;
 }
 
-// one block; ports in order so that overlapping source boxes add up deterministically
+// one launch per driving port (in port order on the stream, so overlapping source boxes add up deterministically);
+// one thread per source sample
 template <typename T>
-__global__ void __launch_bounds__(256) k_source(const PortParams<T> p) {
+__global__ void __launch_bounds__(256) k_source(const PortParams<T> p, int n) {
+  const PortDev q = p.ports[n];
+  const int nj = q.sj1 - q.sj0 + 1, ns = nj * (q.sk1 - q.sk0);
+  const int s = blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= ns) return;
   const double t = (double)(*p.nstep) * p.dt;
-  for (int n = 0; n < p.nports; ++n) {
-    const PortDev q = p.ports[n];
-    if (!q.has_source) continue;
-    const T g = (T)(q.amp * waveform_dev(q.waveform, t, q.t0, q.sigma, q.f0));
-    const int nj = q.sj1 - q.sj0 + 1, ns = nj * (q.sk1 - q.sk0);
-    for (int s = threadIdx.x; s < ns; s += blockDim.x) {
-      const int j = q.sj0 + s % nj, k = q.sk0 + s / nj;
-      p.Ez[q.is + (long long)p.P * j + p.PS * k] += g;
-    }
-    __syncthreads();
-  }
+  const T g = (T)(q.amp * waveform_dev(q.waveform, t, q.t0, q.sigma, q.f0));
+  const int j = q.sj0 + s % nj, k = q.sk0 + s / nj;
+  p.Ez[q.is + (long long)p.P * j + p.PS * k] += g;
 }
 
 __device__ __forceinline__ double warp_sum(double v) {
@@ -315,22 +326,32 @@ __device__ __forceinline__ double warp_sum(double v) {
   return v;
 }
 
-// grid (nports, max(1, ceil(nf/64))), 128 threads.  Every block reduces V and I of its port (warp-shuffle partial
-// sums in fp64), then thread t accumulates frequency chunk*64 + t%64 of V (t < 64) or I (t >= 64).
+// Port probes and running DFT.  grid (nblk, nports), 256 threads.  Block b of a port reduces its slice of the V box and of
+// the I loop (warp-shuffle partial sums in fp64, a fixed sample -> thread -> block assignment) and writes one partial pair;
+// the block that arrives last at the port's counter adds the partials in block order (so V, I do not depend on which block
+// that is) and advances the DFT accumulators of every frequency:
+//   V = (dz / n_col) * sum Ez over the V box                                             (Eq. 4 line 1, R7)
+//   I = dz * sum_k (Hz[lj1,k] - Hz[lj0-1,k]) - dy * sum_j (Hy[j,lk1] - Hy[j,lk0-1])        (Eq. 4 line 2, R7)
+//   V^[m] += V e^{-j 2 pi f_m n dt} dt,  I^[m] += I e^{-j 2 pi f_m (n - 1/2) dt} dt        (R8)
+constexpr int kProbeThreads = 256;
+constexpr int kProbeMaxBlocks = 64;
 template <typename T>
-__global__ void __launch_bounds__(128) k_probe_dft(const PortParams<T> p) {
-  __shared__ double sh[2][4];
-  const PortDev q = p.ports[blockIdx.x];
+__global__ void __launch_bounds__(kProbeThreads) k_probe_dft(const PortParams<T> p) {
+  __shared__ double sh[2][kProbeThreads / 32];
+  __shared__ double res[2];
+  __shared__ int last;
+  const int port = blockIdx.y, nblk = gridDim.x;
+  const PortDev q = p.ports[port];
   const int nj = q.vj1 - q.vj0 + 1, nv = nj * (q.vk1 - q.vk0);
+  const int gtid = blockIdx.x * kProbeThreads + threadIdx.x, gstride = nblk * kProbeThreads;
   double sv = 0.0;
-  for (int s = threadIdx.x; s < nv; s += blockDim.x) {
+  for (int s = gtid; s < nv; s += gstride) {
     const int j = q.vj0 + s % nj, k = q.vk0 + s / nj;
     sv += (double)p.Ez[q.ip + (long long)p.P * j + p.PS * k];
   }
-  // I = dz * sum_k (Hz[lj1,k] - Hz[lj0-1,k]) - dy * sum_j (Hy[j,lk1] - Hy[j,lk0-1])
   const int nkl = q.lk1 - q.lk0 + 1, njl = q.lj1 - q.lj0 + 1;
   double si = 0.0;
-  for (int s = threadIdx.x; s < nkl + njl; s += blockDim.x) {
+  for (int s = gtid; s < nkl + njl; s += gstride) {
     if (s < nkl) {
       const int k = q.lk0 + s;
       si += p.dz * ((double)p.Hz[q.ip + (long long)p.P * q.lj1 + p.PS * k] -
@@ -345,18 +366,42 @@ __global__ void __launch_bounds__(128) k_probe_dft(const PortParams<T> p) {
   const int w = threadIdx.x >> 5;
   if ((threadIdx.x & 31) == 0) { sh[0][w] = sv; sh[1][w] = si; }
   __syncthreads();
-  const double V = p.dz / (double)nj * (sh[0][0] + sh[0][1] + sh[0][2] + sh[0][3]);
-  const double I = sh[1][0] + sh[1][1] + sh[1][2] + sh[1][3];
-  if (blockIdx.y == 0 && threadIdx.x == 0) { p.lastV[blockIdx.x] = V; p.lastI[blockIdx.x] = I; }
-  const int m = blockIdx.y * 64 + (threadIdx.x & 63);
-  if (m < p.nf) {
-    const bool isI = threadIdx.x >= 64;
-    const double n = (double)(*p.nstep);
+  if (threadIdx.x == 0) {
+    double a = 0.0, b = 0.0;
+#pragma unroll
+    for (int q2 = 0; q2 < kProbeThreads / 32; ++q2) { a += sh[0][q2]; b += sh[1][q2]; }
+    double V = a, I = b;
+    last = 1;
+    if (nblk > 1) {   // small port boxes take one block per port and skip the hand-over through global memory
+      double* part = p.partial + ((long long)port * kProbeMaxBlocks + blockIdx.x) * 2;
+      part[0] = a; part[1] = b;
+      __threadfence();
+      last = (atomicAdd(p.pcount + port, 1) == nblk - 1);
+      if (last) {
+        __threadfence();
+        V = 0.0; I = 0.0;
+        const volatile double* pp = p.partial + (long long)port * kProbeMaxBlocks * 2;
+        for (int b2 = 0; b2 < nblk; ++b2) { V += pp[2 * b2]; I += pp[2 * b2 + 1]; }
+        p.pcount[port] = 0;   // ready for the next step (the kernel boundary orders it)
+      }
+    }
+    if (last) {
+      V *= p.dz / (double)nj;
+      res[0] = V; res[1] = I;
+      p.lastV[port] = V; p.lastI[port] = I;
+    }
+  }
+  __syncthreads();
+  if (!last) return;
+  const double n = (double)(*p.nstep);
+  for (int m2 = threadIdx.x; m2 < 2 * p.nf; m2 += kProbeThreads) {
+    const bool isI = m2 >= p.nf;
+    const int m = isI ? m2 - p.nf : m2;
     const double t = (isI ? n - 0.5 : n) * p.dt;
     double s, c;
     sincos(2.0 * 3.14159265358979323846 * p.freqs[m] * t, &s, &c);
-    const double a = (isI ? I : V) * p.dt;
-    double* acc = (isI ? p.dftI : p.dftV) + ((long long)blockIdx.x * p.nf + m) * 2;
+    const double a = res[isI ? 1 : 0] * p.dt;
+    double* acc = (isI ? p.dftI : p.dftV) + ((long long)port * p.nf + m) * 2;
     acc[0] += a * c;
     acc[1] -= a * s;
   }

@@ -70,6 +70,8 @@ struct PortParams {
   double* dftI;
   double* lastV;  // [port]
   double* lastI;
+  double* partial;  // [port][kProbeMaxBlocks][V, I] per-block partial sums of k_probe_dft
+  int* pcount;      // [port] blocks of k_probe_dft that have delivered their partial; returns to 0 every step
   const long long* nstep;  // already incremented: E time = nstep*dt, H time = (nstep - 1/2)*dt
   double dt, dy, dz;
 };

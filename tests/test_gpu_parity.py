@@ -18,7 +18,7 @@ from .parity_util import TOL, assert_fields, run_pair
 
 pytestmark = pytest.mark.gpu
 
-IMPLS = [1, 2]  # FDTD_OPT_STEP_IMPL: 1 = two-pass kernels, 2 = fused E+H kernel (TMA-staged, ping-pong field sets)
+IMPLS = [1, 2, 3]  # FDTD_OPT_STEP_IMPL: 1 = two-pass kernels, 2 = fused E+H kernel (TMA-staged, ping-pong field sets), 3 = persistent
 
 
 @pytest.mark.parametrize("impl", IMPLS)
@@ -225,7 +225,8 @@ def test_error_codes_after_commit():
         s.set_materials_indexed(np.zeros(512, np.uint8), [[1.0, 1.0, -2.0]], [[0.0, 0.0, 0.0]])
     assert e.value.code == -1
     s.step(3)
-    assert s.step_count == 3 and s.launch_count == 6 and s.impl_name == "two_pass"
+    # a grid this small is in the two-pass regime; commit keeps whichever of its two drivers it measured faster
+    assert s.step_count == 3 and (s.launch_count, s.impl_name) in ((6, "two_pass"), (1, "persistent"))
 
 
 @pytest.mark.parametrize("prec", [FDTD_F64, FDTD_F32])

@@ -189,6 +189,33 @@ def microstrip_x1(nx=1000, steps=60000, precision=32, nf=79, f_hi=40e9, npml=10)
 
 
 # --------------------------------------------------------------------------------------------------
+# X3-shaped  grid and time scales of the paper's CMOS transmission line
+# --------------------------------------------------------------------------------------------------
+def cmos_line_x3(run="tot", steps=1400000, precision=32, nf=128, npml=10):
+    """200 x 120 x 800 cells of (20, 50, 5) nm = 4 x 6 x 4 um, CFL number 0.9 (dt = 0.0145 fs), Eq. 3 pulse with
+    sigma = 10.146 fs, 1.4 M steps in the paper; DFT over the band the paper calls resolved, 50 GHz - 95 THz.
+    The SHAPE of that workload only: Fig. 3 and the metal conductivities are not in the paper's text, so the
+    cross-section below (oxide, a 30 nm thick conducting strip, a block on it in the tot run) is a stand-in."""
+    nx, ny, nz = 200, 120, 800
+    dx, dy, dz = 20e-9, 50e-9, 5e-9
+    dt = 0.9 * cfl_limit(dx, dy, dz)
+    pt = Painter(nx, ny, nz)
+    pt.layers([0, 400, nz], [3.9, 1.0])
+    j0, j1, k0, k1 = 40, 80, 400, 406                   # 2 um wide, 30 nm thick
+    pt.conductor(0, nx, j0, j1, k0, k1, sigma=SIGMA_CU)
+    if run == "tot":
+        pt.conductor(90, 110, j0, j1, k1, k1 + 40, sigma=SIGMA_CU)
+    sig = 10.146e-15
+    src = {"is": 20, "sj0": j0, "sj1": j1, "sk0": 0, "sk1": k0, "waveform": W_DGAUSS, "amp": 1.0,
+           "t0": 3 * sig, "sigma": sig, "f0": 0.0}
+    box = dict(vj0=j0, vj1=j1, vk0=0, vk1=k0, lj0=j0 - 1, lj1=j1 + 1, lk0=k0 - 1, lk1=k1 + 1)
+    ports = [_port(ip=30, source=src, **box), _port(ip=nx - 30, **box)]
+    return dict(name="x3", nx=nx, ny=ny, nz=nz, dx=dx, dy=dy, dz=dz, dt=dt, precision=precision,
+                pml=[npml, npml, npml, npml, 0, npml], cpml=[3.0, 1.0, 1.0, 0.0, 0.8, 2.45], materials=pt.indexed(),
+                ports=ports, freqs=np.linspace(50e9, 95e12, nf), steps=steps, run=run)
+
+
+# --------------------------------------------------------------------------------------------------
 # C2 / C4  CMOS-like multilayer interconnect (C4 = C2 with every extent x2, fp64, full uniaxial arrays)
 # --------------------------------------------------------------------------------------------------
 def _interconnect(seed, mult, div, run, full, precision, npml, nf, sig_dt, nports, steps):
