@@ -42,7 +42,7 @@ UNIT = "Mcell-updates/s"
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch, from the ncu captures summarised under profiles/
 NCU_TRAFFIC = {
-    ("c3", "k_step_fused", 32): (49.30e9, "profiles/r01_fused_v4.md (26.09 GB read + 23.21 GB written)"),
+    ("c3", "k_step_fused", 32): (49.44e9, "profiles/r01_final.md (26.24 GB read + 23.20 GB written)"),
     ("c3", "k_update_E", 32): (35.24e9, "profiles/r01_twopass.md"),
     ("c3", "k_update_H", 32): (34.39e9, "profiles/r01_twopass.md"),
 }

@@ -62,3 +62,17 @@ def test_C4_full_grid_first_steps():
     assert_fields(rep, FDTD_F64)
     assert max(rep["dft_err"]) <= 1e-11
     s.destroy()
+
+
+def test_X3_shaped_full_grid_first_steps():
+    """the grid shape and time scale of the paper's CMOS line (200x120x800 cells of (20, 50, 5) nm,
+    dt = 0.0145 fs): strongly anisotropic cells, a ragged x tile (200 = 128 + 72), 16 400-sample
+    port boxes (multi-block probe reduction), DGAUSS source."""
+    w = W.cmos_line_x3(run="tot", steps=150)
+    assert (w["nx"], w["ny"], w["nz"]) == (200, 120, 800) and abs(w["dt"] - 0.0145e-15) < 0.00005e-15
+    for impl in (0, 2):
+        o, s, rep = run_pair(w, 150, options={FDTD_OPT_STEP_IMPL: impl}, checkpoints=[50, 150])
+        print(f"X3 full grid impl={s.impl_name} kz={s.fused_kz}: field_err={rep['field_err'].max():.3e} dft={rep['dft_err']}")
+        assert_fields(rep, FDTD_F32)
+        assert max(rep["dft_err"]) <= 1e-4
+        s.destroy()
