@@ -255,3 +255,28 @@ def test_fused_equals_two_pass_closely():
     for c in range(6):
         scale = max(np.abs(out[0][c]).max(), 1e-300)
         assert np.abs(out[0][c] - out[1][c]).max() / scale < 2e-6
+
+
+@pytest.mark.parametrize("impl", [2, 3])
+def test_repeated_runs_are_bitwise_identical(impl):
+    """The fused kernel synchronises its warps with mbarriers only (TMA ring, row-to-row and column hand-over) and the
+    persistent kernel with grid barriers: a missing edge in either protocol shows up as run-to-run differences.  Many
+    blocks per SM wave, several chunks, CPML on every face; three runs must agree bit for bit (compute-sanitizer is not
+    available on this pool)."""
+    from paper_2208_04371_b200 import FDTD_OPT_FUSED_KZ
+    w = W.throughput_c3(div=4, steps=60, npml=8, nf=8)          # 384x192x192: 3 x 14 x 16 blocks of the fused kernel
+    outs = []
+    for _ in range(3):
+        s = Solver.from_workload(w, options={FDTD_OPT_STEP_IMPL: impl, FDTD_OPT_FUSED_KZ: 12})
+        s.step(60)
+        outs.append([s.read_fields(c).clone() for c in range(6)] + [torch_dft(s)])
+        s.destroy()
+    for other in outs[1:]:
+        for a, b in zip(outs[0][:6], other[:6]):
+            assert bool((a == b).all())
+        assert np.array_equal(outs[0][6], other[6])
+
+
+def torch_dft(s):
+    v, i = s.read_port_dft(0)
+    return np.concatenate([v.view(np.float64), i.view(np.float64)])
