@@ -280,3 +280,20 @@ def test_repeated_runs_are_bitwise_identical(impl):
 def torch_dft(s):
     v, i = s.read_port_dft(0)
     return np.concatenate([v.view(np.float64), i.view(np.float64)])
+
+
+@pytest.mark.parametrize("impl", IMPLS)
+def test_two_overlapping_sources_and_thick_slabs(impl):
+    """Degenerate port set-ups: two driving ports whose source boxes overlap (the sum must not depend on the launch
+    order), different waveforms, a port without DFT work next to them; CPML slabs that are thicker than what they leave of
+    the grid in y (lo + hi = ny - 2)."""
+    w = W.random_box(31, nx=70, ny=18, nz=20, pml=(4, 5, 8, 8, 3, 4), steps=80, precision=FDTD_F32)
+    p0 = dict(w["ports"][0])
+    extra = dict(p0)
+    extra.update({"is": p0["is"], "sj0": p0["sj0"] - 1, "sj1": p0["sj1"], "sk0": p0["sk0"], "sk1": p0["sk1"] + 1,
+                  "waveform": 2, "f0": 3.0 / (80 * w["dt"]), "amp": -0.7, "ip": p0["ip"] + 3})
+    w = dict(w, ports=[p0, w["ports"][1], extra])
+    o, s, rep = run_pair(w, 80, options={FDTD_OPT_STEP_IMPL: impl}, checkpoints=[1, 40, 80])
+    assert_fields(rep, FDTD_F32)
+    assert max(rep["dft_err"]) <= 1e-5
+    s.destroy()
