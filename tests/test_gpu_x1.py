@@ -26,10 +26,16 @@ def test_x1_short_piece_matches_the_oracle():
     s.destroy()
 
 
-def test_x1_paper_size_against_eq7():
+def test_x1_paper_size_against_eq7(golden_dir):
+    from tests.test_oracle_pins import load_golden
+    g = load_golden(golden_dir)
     w = W.microstrip_x1()
-    assert (w["nx"], w["ny"], w["nz"], w["steps"]) == (1000, 200, 50, 60000)
-    assert abs(w["dt"] - 0.173e-12) < 0.0005e-12
+    cx, cy, cz = (int(v) for v in g["cells_microstrip"].split())           # the paper's propagation axis y is x here
+    assert (w["nx"], w["ny"], w["nz"], w["steps"]) == (cy, cx, cz, int(g["steps_microstrip"]))
+    assert abs(w["dt"] / float(g["dt_microstrip_s"]) - 1) < 2e-3
+    assert w["ports"][0]["sigma"] == float(g["sigma_microstrip_s"])
+    assert (w["theory"]["z0"], w["theory"]["eps_r"], w["theory"]["w_over_h"]) == (
+        float(g["z0_microstrip_ohm"]), float(g["epsr_microstrip"]), float(g["w_over_h_microstrip"]))
     r = x1_microstrip.run(w)
     th = r["theory"]
     f = r["freqs"]

@@ -32,13 +32,15 @@ def test_one_port_load():
         assert abs(out[0][0] - (ZL - 50) / (ZL + 50)) < 1e-15
 
 
-def test_eq7_matched_25_ohm_line():
-    gamma_printed = -0.333
-    G = (25.0 - 50.0) / (25.0 + 50.0)
+def test_eq7_matched_25_ohm_line(golden_dir):
+    from tests.test_oracle_pins import load_golden
+    g = load_golden(golden_dir)
+    gamma_printed, z0 = float(g["gamma_25_50"]), float(g["z0_microstrip_ohm"])
+    G = (z0 - 50.0) / (z0 + 50.0)
     assert abs(G - gamma_printed) < 5e-4
     for bl in (0.3, 1.7, 2.9, 5.1):
         k = cmath.exp(-1j * bl)                              # e^{-j beta l}: R30 (this library's DFT sign)
-        out = R.renormalize_one([[0, k], [k, 0]], [25 + 0j, 25 + 0j])
+        out = R.renormalize_one([[0, k], [k, 0]], [z0 + 0j, z0 + 0j])
         s11 = (1 - k * k) * G / (1 - k * k * G * G)          # Eq. 7, as printed
         s21 = (1 - G * G) * k / (1 - k * k * G * G)          # Eq. 7 with the numerator read as (1 - Gamma^2) kappa (R30)
         assert abs(out[0][0] - s11) < 1e-15 and abs(out[1][1] - s11) < 1e-15
