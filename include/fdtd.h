@@ -147,6 +147,26 @@ int fdtd_read_port_last(fdtd_t*, int port, double* V, double* I);
 /* Zero fields, psi, DFT accumulators and the step counter; materials, ports and tables stay. */
 int fdtd_reset(fdtd_t*);
 
+/* ---- domain decomposition along z ("decomposing the domain into a number of grids equal to the number
+ * of GPUs", guard-cell exchange every step) --------------------------------------------------------------
+ * A handle can be one z slab [z0, z1) of a larger grid.  fdtd_set_z_interfaces (before commit) declares which of its z
+ * faces are interfaces to a neighbouring slab instead of PEC walls: the halo planes -1 / nz of the padded arrays then
+ * hold the neighbour's planes z0-1 / z1, and Ex, Ey on plane 0 of a lo-open slab are ordinary cells.  Such a handle runs
+ * the fused step only and advances one step at a time:
+ *     fdtd_step_begin   H^{n+1/2} on every plane, E^{n+1} on every plane but plane 0 of a lo-open slab
+ *     caller            new Hx, Hy of my plane nz-1  ->  halo plane -1 of the upper neighbour
+ *     fdtd_step_end     E^{n+1} on plane 0 of a lo-open slab, then source, probes, DFT of this slab's ports
+ *     caller            new Ex, Ey of my plane 0     ->  halo plane nz of the lower neighbour
+ * CPML cells on z belong to the first (z-) and last (z+) slab only; a port must lie inside one slab (its I loop reads
+ * planes lk0-1 .. lk1).  fdtd_plane returns the device address and byte size of the padded plane k in [-1, nz] of a
+ * component in the field set that holds the current state (the new one after fdtd_step_begin); planes of slabs with
+ * equal nx, ny have equal size and layout, so an exchange is one contiguous device-to-device copy (NVLink peer copy,
+ * ncclSend/ncclRecv).  On a closed handle begin + end is one ordinary step.  Errors: FDTD_ESTATE out of order. */
+int fdtd_set_z_interfaces(fdtd_t*, int lo_open, int hi_open);
+int fdtd_step_begin(fdtd_t*);
+int fdtd_step_end(fdtd_t*);
+int fdtd_plane(fdtd_t*, int comp, int k, void** dev_ptr, size_t* bytes);
+
 long fdtd_step_count(const fdtd_t*);
 /* Number of kernel launches the library has enqueued since commit (graph nodes count individually). */
 long fdtd_launch_count(const fdtd_t*);

@@ -64,6 +64,10 @@ SYMBOLS = {
     "fdtd_launch_count": (C.c_long, [_vp]),
     "fdtd_impl_name": (C.c_char_p, [_vp]),
     "fdtd_fused_kz": (C.c_int, [_vp]),
+    "fdtd_set_z_interfaces": (C.c_int, [_vp, C.c_int, C.c_int]),
+    "fdtd_step_begin": (C.c_int, [_vp]),
+    "fdtd_step_end": (C.c_int, [_vp]),
+    "fdtd_plane": (C.c_int, [_vp, C.c_int, C.c_int, C.POINTER(C.c_void_p), C.POINTER(C.c_size_t)]),
     "fdtd_last_error": (C.c_char_p, [_vp]),
     "fdtd_destroy": (None, [_vp]),
 }
@@ -229,6 +233,25 @@ def fdtd_impl_name(h) -> str:
 
 def fdtd_fused_kz(h) -> int:
     return int(lib().fdtd_fused_kz(h))
+
+
+def fdtd_set_z_interfaces(h, lo_open, hi_open):
+    _check(h, lib().fdtd_set_z_interfaces(h, int(bool(lo_open)), int(bool(hi_open))))
+
+
+def fdtd_step_begin(h):
+    _check(h, lib().fdtd_step_begin(h))
+
+
+def fdtd_step_end(h):
+    _check(h, lib().fdtd_step_end(h))
+
+
+def fdtd_plane(h, comp, k):
+    """(device address, bytes) of the padded plane k in [-1, nz] of component comp in the current field set."""
+    p, n = C.c_void_p(), C.c_size_t()
+    _check(h, lib().fdtd_plane(h, int(comp), int(k), C.byref(p), C.byref(n)))
+    return int(p.value), int(n.value)
 
 
 def fdtd_last_error(h) -> str:

@@ -51,6 +51,8 @@ struct fdtd {
   std::vector<PortDev> ports;
   std::vector<double> freqs;
   long opt_impl = 0, opt_graph = 1, opt_unroll = 8, opt_kz = 0;
+  int z_lo_open = 0, z_hi_open = 0;   // this grid is a z slab of a larger one (fdtd_set_z_interfaces)
+  bool mid_step = false;              // between fdtd_step_begin and fdtd_step_end
   bool committed = false;
   long nstep = 0;
   long launches = 0;
@@ -82,6 +84,9 @@ struct fdtd {
   virtual int set_materials_indexed(const uint8_t* idx, int ne, const double* eps, const double* sig, const double* mu) = 0;
   virtual int set_materials_full(const void* const eps[3], const void* const sig[3], const void* const mu[3]) = 0;
   virtual int step(long n) = 0;
+  virtual int step_begin() = 0;
+  virtual int step_end() = 0;
+  virtual int plane_ptr(int comp, int k, void** ptr, size_t* bytes) = 0;
   virtual int profile_step(long n, double* ms) = 0;
   virtual int read_field(int comp, void* dst) = 0;
   virtual int write_field(int comp, const void* src) = 0;
@@ -132,7 +137,7 @@ struct Solver : fdtd {
   }
   // auto: the fused kernel pays off once the grid no longer fits in L2 (small grids are launch-bound)
   bool slabs_fit() const { return S(0) <= kMaxSlab && S(1) <= kMaxSlab && S(2) <= kMaxSlab; }
-  bool want_fused() const { return slabs_fit() && (opt_impl == 2 || (opt_impl == 0 && (long long)nx * ny * nz >= (4LL << 20))); }
+  bool want_fused() const { return slabs_fit() && (opt_impl == 2 || z_lo_open || z_hi_open || (opt_impl == 0 && (long long)nx * ny * nz >= (4LL << 20))); }
 
   int mode() const { return (mat_mode == FDTD_MAT_FULL ? kModeFull : 0) | (has_mu ? kModeMu : 0); }
   size_t psi_elems(int a) const {
@@ -187,6 +192,11 @@ struct Solver : fdtd {
   int set_materials_indexed(const uint8_t* idx, int ne, const double* eps, const double* sig, const double* mu) override;
   int set_materials_full(const void* const eps[3], const void* const sig[3], const void* const mu[3]) override;
   int step(long n) override;
+  int step_begin() override;
+  int step_end() override;
+  int plane_ptr(int comp, int k, void** ptr, size_t* bytes) override;
+  void enqueue_ports();
+  void enqueue_ports_ev(cudaEvent_t* ev);
   int profile_step(long n, double* ms) override;
   int read_field(int comp, void* dst) override { return copy_field(comp, dst, true); }
   int write_field(int comp, const void* src) override { return copy_field(comp, const_cast<void*>(src), false); }
@@ -197,6 +207,7 @@ struct Solver : fdtd {
   int fused_kz() const override { return fused ? kz : 0; }
   int build_fused();
   int autotune();
+  int autotune_kz_only() { const long keep = opt_impl; opt_impl = 2; const int r = autotune(); opt_impl = keep; return r; }
   int setup_persistent();
   int launch_persistent(const PortParams<T>& q, long n);
   double time_field_kernels(int reps);
@@ -286,6 +297,7 @@ int Solver<T>::commit(void* w, size_t bytes, void* st) {
   }
   for (int q = 0; q < 12; ++q) sp.psi[q] = reinterpret_cast<T*>(ws + cv.psi[q]);
   sp.nstep = reinterpret_cast<long long*>(ws + cv.nstep);
+  sp.z_lo_open = z_lo_open;
 
   // port parameters
   pp = PortParams<T>{};
@@ -319,6 +331,8 @@ int Solver<T>::commit(void* w, size_t bytes, void* st) {
     const long long nb = (most + 1023) / 1024;
     probe_blocks = (unsigned)(nb < 1 ? 1 : (nb > kProbeMaxBlocks ? kProbeMaxBlocks : nb));
   }
+  if ((z_lo_open || z_hi_open) && (!slabs_fit() || opt_impl == 1 || opt_impl == 3))
+    return fail(FDTD_EINVAL, "fdtd_commit: a z slab (fdtd_set_z_interfaces) runs the fused step only (CPML <= %d cells per axis)", kMaxSlab);
   pp2 = pp;
   fused = want_fused();
   cur = 0;
@@ -351,7 +365,9 @@ int Solver<T>::commit(void* w, size_t bytes, void* st) {
   }
   if ((e = cudaStreamSynchronize(stream)) != cudaSuccess) return cuda_fail(e, "fdtd_commit");
   if ((e = cudaGetLastError()) != cudaSuccess) return cuda_fail(e, "fdtd_commit");
-  if (fused && (opt_impl == 0 || opt_kz <= 0)) {
+  if (fused && (z_lo_open || z_hi_open)) {
+    if (opt_kz <= 0) { const int r = autotune_kz_only(); if (r != FDTD_OK) return r; }
+  } else if (fused && (opt_impl == 0 || opt_kz <= 0)) {
     const int r = autotune();
     if (r != FDTD_OK) return r;
   }
@@ -759,6 +775,14 @@ void Solver<T>::enqueue_step(cudaEvent_t* ev) {
     }
     launches += 2;
   }
+  enqueue_ports_ev(ev);
+}
+
+template <typename T>
+void Solver<T>::enqueue_ports() { enqueue_ports_ev(nullptr); }
+
+template <typename T>
+void Solver<T>::enqueue_ports_ev(cudaEvent_t* ev) {
   const PortParams<T>& q = cur ? pp2 : pp;   // the set that now holds E^{n+1}, H^{n+1/2}
   if (!ports.empty()) {
     for (size_t n = 0; n < ports.size(); ++n) {   // one launch per driving port, in port order
@@ -826,6 +850,9 @@ template <typename T>
 int Solver<T>::step(long n) {
   if (!committed) return fail(FDTD_ESTATE, "fdtd_step: call after fdtd_commit");
   if (n < 0) return fail(FDTD_EINVAL, "fdtd_step: n < 0");
+  if (mid_step) return fail(FDTD_ESTATE, "fdtd_step: fdtd_step_end is pending");
+  if ((z_lo_open || z_hi_open) && n > 0)
+    return fail(FDTD_ESTATE, "fdtd_step: a z slab advances with fdtd_step_begin / plane exchange / fdtd_step_end");
   long left = n;
   if (persistent && n > 0) {
     const int r = launch_persistent(pp, n);
@@ -852,6 +879,67 @@ int Solver<T>::step(long n) {
   const cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return cuda_fail(e, "fdtd_step");
   nstep += n;
+  return FDTD_OK;
+}
+
+// ---- z-slab stepping (one grid per GPU with guard-cell exchange) -----------------------
+// begin: the fused kernel: H^{n+1/2} on every plane (plane nz-1 uses the upper neighbour's E^n in halo plane nz), E^{n+1}
+//        on every plane except plane 0 of a lo-open slab.  The state moves to the other field set.
+// [caller: my new Hx, Hy of plane nz-1 -> halo plane -1 of the upper neighbour]
+// end:   E^{n+1} on plane 0 of a lo-open slab with the two-pass E kernel (same R5 arithmetic; old E from the previous
+//        set, new H of planes -1 and 0 from the new one), then source, probes, DFT.
+// [caller: my new Ex, Ey of plane 0 -> halo plane nz of the lower neighbour]
+template <typename T>
+int Solver<T>::step_begin() {
+  if (!committed) return fail(FDTD_ESTATE, "fdtd_step_begin: call after fdtd_commit");
+  if (!fused) return fail(FDTD_ESTATE, "fdtd_step_begin: the handle does not run the fused step");
+  if (mid_step) return fail(FDTD_ESTATE, "fdtd_step_begin: fdtd_step_end is pending");
+  launch_fused(nullptr);
+  launches += 1;
+  mid_step = true;
+  const cudaError_t e = cudaGetLastError();
+  return e == cudaSuccess ? FDTD_OK : cuda_fail(e, "fdtd_step_begin");
+}
+
+template <typename T, int MODE>
+static void launch_E_plane0(const StepParams<T>& q, cudaStream_t st) {
+  constexpr int V = VecOf<T>::V;
+  const int nvec = (q.nx + V - 1) / V;
+  int bx = 1;
+  while (bx < nvec && bx < 128) bx <<= 1;
+  const int by = 128 / bx;
+  k_update_E<T, MODE><<<dim3((nvec + bx - 1) / bx, (q.ny + by - 1) / by, 1), dim3(bx, by, 1), 0, st>>>(q);
+}
+
+template <typename T>
+int Solver<T>::step_end() {
+  if (!mid_step) return fail(FDTD_ESTATE, "fdtd_step_end: no fdtd_step_begin is pending");
+  if (z_lo_open) {
+    StepParams<T> q = fpar[cur ^ 1].sp;               // the launch that just ran: src = old set, dst = new (= current) set
+    for (int f = kHx; f <= kHz; ++f) q.src[f] = q.dst[f];   // H^{n+1/2} is read from the new set (halo plane -1 included)
+    switch (mode()) {
+      case 0: launch_E_plane0<T, 0>(q, stream); break;
+      case 1: launch_E_plane0<T, 1>(q, stream); break;
+      case 2: launch_E_plane0<T, 2>(q, stream); break;
+      default: launch_E_plane0<T, 3>(q, stream); break;
+    }
+    launches += 1;
+  }
+  enqueue_ports();
+  mid_step = false;
+  nstep += 1;
+  const cudaError_t e = cudaGetLastError();
+  return e == cudaSuccess ? FDTD_OK : cuda_fail(e, "fdtd_step_end");
+}
+
+// Device address and size of the padded plane k in [-1, nz] of component comp in the set that holds the current state
+// (after fdtd_step_begin: the new one).  The plane is contiguous: (ny + 1) rows of the x pitch.
+template <typename T>
+int Solver<T>::plane_ptr(int comp, int k, void** ptr, size_t* bytes) {
+  if (!committed) return fail(FDTD_ESTATE, "fdtd_plane: call after fdtd_commit");
+  if (comp < 0 || comp > 5 || k < -1 || k > nz || !ptr || !bytes) return fail(FDTD_EINVAL, "fdtd_plane: bad component, plane or null pointer");
+  *ptr = field_origin(comp, cur) + (long long)k * plane();
+  *bytes = (size_t)plane() * sizeof(T);
   return FDTD_OK;
 }
 
@@ -893,6 +981,7 @@ int Solver<T>::reset() {
   for (int q = 0; q < 6 && e == cudaSuccess && fused; ++q)
     if (psi_elems(psi_axis(q))) e = cudaMemsetAsync(ws + cv.psiH2[q], 0, psi_elems(psi_axis(q)) * sizeof(T), stream);
   cur = 0;
+  mid_step = false;
   if (e == cudaSuccess) e = cudaMemsetAsync(ws + cv.dftV, 0, cv.nstep + sizeof(long long) - cv.dftV, stream);
   if (e != cudaSuccess) return cuda_fail(e, "fdtd_reset");
   nstep = 0;
@@ -1006,6 +1095,16 @@ int fdtd_set_materials_full(fdtd_t* h, const void* const eps_r[3], const void* c
   return h ? h->set_materials_full(eps_r, sigma, mu_r) : FDTD_EINVAL;
 }
 int fdtd_step(fdtd_t* h, long n) { return h ? h->step(n) : FDTD_EINVAL; }
+int fdtd_step_begin(fdtd_t* h) { return h ? h->step_begin() : FDTD_EINVAL; }
+int fdtd_step_end(fdtd_t* h) { return h ? h->step_end() : FDTD_EINVAL; }
+int fdtd_plane(fdtd_t* h, int comp, int k, void** dev_ptr, size_t* bytes) { return h ? h->plane_ptr(comp, k, dev_ptr, bytes) : FDTD_EINVAL; }
+int fdtd_set_z_interfaces(fdtd_t* h, int lo_open, int hi_open) {
+  if (!h) return FDTD_EINVAL;
+  if (h->committed) return h->fail(FDTD_ESTATE, "fdtd_set_z_interfaces: call before fdtd_commit");
+  h->z_lo_open = lo_open ? 1 : 0;
+  h->z_hi_open = hi_open ? 1 : 0;
+  return FDTD_OK;
+}
 int fdtd_profile_step(fdtd_t* h, long n, double ms_avg[4]) { return h ? h->profile_step(n, ms_avg) : FDTD_EINVAL; }
 int fdtd_read_fields(fdtd_t* h, int comp, void* dst) { return h ? h->read_field(comp, dst) : FDTD_EINVAL; }
 int fdtd_write_fields(fdtd_t* h, int comp, const void* src) { return h ? h->write_field(comp, src) : FDTD_EINVAL; }

@@ -520,7 +520,7 @@ __global__ void __launch_bounds__((TY + 2) * 32, 1) k_step_fused(const __grid_co
     }
     __syncwarp();
     if (lane == 0 && r < TY) mbar_arrive(&rowrdy[s * TY + r]);   // every iteration, so that the phase parity is it / NS
-    if (it >= 2 && r >= 1) {
+    if (it >= 2 && r >= 1 && !(p.z_lo_open && k == 0)) {   // plane 0 of a lo-open z slab: E is updated by fdtd_step_end
       // ---------------- E phase: E^{n+1}(k) = Ca E^n + Cb curl H^{n+1/2} ---------------------------------------------
       unsigned char mi[V];
       if (!kFull) ld_index_smem<V>(sIdx + (r - 1) * TX + lane * V, mi);

@@ -269,7 +269,7 @@ __device__ __forceinline__ void update_E_vec(const StepParams<T>& p, int i0, int
       cax[v] = a.a; cay[v] = a.b; caz[v] = a.c; cbx[v] = a.d; cby[v] = b.a; cbz[v] = b.b;
     }
   }
-  const bool wj = (j == 0), wk = (k == 0);
+  const bool wj = (j == 0), wk = (k == 0) && !p.z_lo_open;
 #pragma unroll
   for (int v = 0; v < V; ++v) {
     const bool wi = (i0 + v == 0), pad = (i0 + v >= p.nx);

@@ -45,6 +45,7 @@ struct StepParams {
   const T* bH[3]; const T* cH[3]; const T* kH[3];   // at half-integer positions (H profile)
   T* psi[12];       // slab-only arrays: y-slab  i + P*(s + Sy*k);  z-slab  i + P*(j + ny*s);  x-slab  s + Sx*(j + ny*k)
   long long* nstep; // device step counter, incremented by the first kernel of every step
+  int z_lo_open;    // 1: this grid is a z slab of a larger one and plane 0 is not a wall (Ex, Ey there are ordinary cells)
 };
 
 struct PortDev {

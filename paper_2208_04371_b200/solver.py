@@ -45,6 +45,9 @@ class Solver:
     def set_option(self, option, value):
         B.fdtd_set_option(self.h, option, value)
 
+    def set_z_interfaces(self, lo_open, hi_open):
+        B.fdtd_set_z_interfaces(self.h, lo_open, hi_open)
+
     def workspace_bytes(self):
         return B.fdtd_workspace_bytes(self.h)
 
@@ -108,6 +111,21 @@ class Solver:
     def fused_kz(self):
         return B.fdtd_fused_kz(self.h)
 
+    # ---- z-slab stepping (include/fdtd.h "domain decomposition along z") ------------------------------------------
+    def step_begin(self):
+        B.fdtd_step_begin(self.h)
+
+    def step_end(self):
+        B.fdtd_step_end(self.h)
+
+    def plane(self, comp, k):
+        """The padded plane k in [-1, nz] of component comp in the current field set, as a uint8 view of the workspace
+        (contiguous; equal size and layout on every slab of equal nx, ny)."""
+        addr, nbytes = B.fdtd_plane(self.h, comp, k)
+        off = addr - self.workspace.data_ptr()
+        assert 0 <= off and off + nbytes <= self.workspace.numel()
+        return self.workspace[off:off + nbytes]
+
     def synchronize(self):
         self.stream.synchronize()
 
@@ -125,7 +143,7 @@ class Solver:
 
     # ---- a workload dict (workloads/__init__.py) -> a committed solver ------------------------------------------
     @classmethod
-    def from_workload(cls, w: dict, precision=None, options=None, device="cuda:0", materials_on_device=False):
+    def from_workload(cls, w: dict, precision=None, options=None, device="cuda:0", materials_on_device=False, z_open=None):
         prec = precision if precision is not None else w["precision"]
         s = cls(w["nx"], w["ny"], w["nz"], w["dx"], w["dy"], w["dz"], w["dt"], prec)
         if w.get("periodic_y"):
@@ -140,6 +158,8 @@ class Solver:
             s.set_dft(w["freqs"])
         for k, v in (options or {}).items():
             s.set_option(k, v)
+        if z_open is not None:
+            s.set_z_interfaces(*z_open)
         s.commit(device)
         np_dt = np.float64 if prec == B.FDTD_F64 else np.float32
         if m["mode"] == "indexed":
