@@ -389,6 +389,11 @@ __global__ void __launch_bounds__((TY + 2) * 32, 1) k_step_fused(const __grid_co
     const bool pml = (xs || sj >= 0 || zs) && cin && k >= 0;   // some CPML correction applies to this thread
     T* const hnb = hn + s * (C::HN_SLOT / (int)sizeof(T));
 
+    if (kFull && owned && it >= 1 && it + 1 < nIt) {  // full mode: the next plane's coefficient lines, one plane ahead, into L2
+      const long long on = o + p.PS;
+#pragma unroll
+      for (int c = 0; c < 3; ++c) { prefetch_l2(p.Ca[c] + on); prefetch_l2(p.Cb[c] + on); }
+    }
     if (pml && it + 1 < nIt) {  // pull the psi lines of the next plane into L2 while this plane is being processed
       if (sj >= 0) {
         const long long q = qy(k + 1);
