@@ -66,7 +66,10 @@ enum { kModeIndexed = 0, kModeFull = 1, kModeMu = 2 };
 // H pass.  R5 step 1:  psiH = bH psiH + cH D+E ;  Hx -= Dbx (D+y Ez / kHy + psiHxy - D+z Ey / kHz - psiHxz)  etc.
 // ------------------------------------------------------------------------------------------------------------------
 // the H update of the V consecutive cells starting at (i0, j, k); i0 < nx, j < ny
-template <typename T, int MODE>
+// XV: handle x-slab vectors with 128-bit psi / coefficient accesses when the slab edges fall on vector boundaries.  It
+// costs ~20 registers: worth it where most warps contain x-slab lanes and occupancy is not the limit (the persistent
+// small-grid kernel: C1 24.3 -> 15.1 us/step), not in the two-pass kernels (64 / 72 registers, 8 / 7 blocks per SM).
+template <typename T, int MODE, bool XV = false>
 __device__ __forceinline__ void update_H_vec(const StepParams<T>& p, int i0, int j, int k) {
   constexpr int V = VecOf<T>::V;
   const long long o = i0 + (long long)p.P * j + p.PS * k;
@@ -81,9 +84,12 @@ __device__ __forceinline__ void update_H_vec(const StepParams<T>& p, int i0, int
   const int sj = slab_coord(j, p.lo[1], p.hi[1], p.ny);
   const int sk = slab_coord(k, p.lo[2], p.hi[2], p.nz);
   const bool xs = (i0 < p.lo[0]) || (i0 + V > p.nx - p.hi[0]);
+  // slab edges on vector boundaries: a vector is then wholly inside or wholly outside the x slab (128-bit psi accesses)
+  const bool xvec = XV && (p.lo[0] % V == 0) && ((p.nx - p.hi[0]) % V == 0) && (p.nx % V == 0);
 
   T ax[V], ay[V], az[V];          // curl accumulators
   T d0[V], d1[V], d2[V], d3[V];  // raw derivatives kept for the y / z slab psi updates
+  T dxa[V], dxb[V];               // D+x Ez, D+x Ey for the vectorised x-slab update
   {
     const T iky = sj >= 0 ? p.kH[1][sj] : T(1), ikz = sk >= 0 ? p.kH[2][sk] : T(1);
 #pragma unroll
@@ -97,8 +103,9 @@ __device__ __forceinline__ void update_H_vec(const StepParams<T>& p, int i0, int
       ay[v] = dzEx * ikz;
       az[v] = -dyEx * iky;
       // x terms need the per-cell kappa: done in the x-slab branch or here with kappa = 1
+      dxa[v] = dxEz; dxb[v] = dxEy;
       if (!xs) { ay[v] -= dxEz; az[v] += dxEy; }
-      else {
+      else if (!xvec) {
         const int si = slab_coord(i0 + v, p.lo[0], p.hi[0], p.nx);
         T ikx = T(1);
         T pyx = T(0), pzx = T(0);
@@ -114,6 +121,20 @@ __device__ __forceinline__ void update_H_vec(const StepParams<T>& p, int i0, int
       }
       d0[v] = dyEz; d1[v] = dyEx; d2[v] = dzEy; d3[v] = dzEx;
     }
+  }
+  if (xs && xvec) {  // x slab, whole vector: psiHyx (from D+x Ez) -> Hy, psiHzx (from D+x Ey) -> Hz
+    const int si0 = slab_coord(i0, p.lo[0], p.hi[0], p.nx);
+    const long long q = si0 + (long long)(p.lo[0] + p.hi[0]) * (j + (long long)p.ny * k);
+    T a[V], d[V], b[V], c[V], ik[V];
+    ldv(p.psi[pHyx] + q, a); ldv(p.psi[pHzx] + q, d);
+    ldv(p.bH[0] + si0, b); ldv(p.cH[0] + si0, c); ldv(p.kH[0] + si0, ik);
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      a[v] = b[v] * a[v] + c[v] * dxa[v]; d[v] = b[v] * d[v] + c[v] * dxb[v];
+      ay[v] -= dxa[v] * ik[v] + a[v];
+      az[v] += dxb[v] * ik[v] + d[v];
+    }
+    stv(p.psi[pHyx] + q, a); stv(p.psi[pHzx] + q, d);
   }
   if (sj >= 0) {  // y slab: psiHxy (from D+y Ez), psiHzy (from D+y Ex)
     const long long q = i0 + (long long)p.P * (sj + (long long)(p.lo[1] + p.hi[1]) * k);
@@ -182,7 +203,7 @@ __global__ void __launch_bounds__(128) k_update_H(const StepParams<T> p) {
 // then the low-face wall rows are forced to zero (PEC walls; PAPER.md:46 for the ground).
 // ------------------------------------------------------------------------------------------------------------------
 // the E update of the V consecutive cells starting at (i0, j, k); i0 < nx, j < ny
-template <typename T, int MODE>
+template <typename T, int MODE, bool XV = false>
 __device__ __forceinline__ void update_E_vec(const StepParams<T>& p, int i0, int j, int k) {
   constexpr int V = VecOf<T>::V;
   const long long o = i0 + (long long)p.P * j + p.PS * k;
@@ -197,9 +218,11 @@ __device__ __forceinline__ void update_E_vec(const StepParams<T>& p, int i0, int
   const int sj = slab_coord(j, p.lo[1], p.hi[1], p.ny);
   const int sk = slab_coord(k, p.lo[2], p.hi[2], p.nz);
   const bool xs = (i0 < p.lo[0]) || (i0 + V > p.nx - p.hi[0]);
+  const bool xvec = XV && (p.lo[0] % V == 0) && ((p.nx - p.hi[0]) % V == 0) && (p.nx % V == 0);
 
   T ax[V], ay[V], az[V];
   T d0[V], d1[V], d2[V], d3[V];  // raw derivatives kept for the y / z slab psi updates
+  T dxa[V], dxb[V];               // D-x Hz, D-x Hy for the vectorised x-slab update
   {
     const T iky = sj >= 0 ? p.kE[1][sj] : T(1), ikz = sk >= 0 ? p.kE[2][sk] : T(1);
 #pragma unroll
@@ -212,8 +235,9 @@ __device__ __forceinline__ void update_E_vec(const StepParams<T>& p, int i0, int
       ax[v] = dyHz * iky - dzHy * ikz;
       ay[v] = dzHx * ikz;
       az[v] = -dyHx * iky;
+      dxa[v] = dxHz; dxb[v] = dxHy;
       if (!xs) { ay[v] -= dxHz; az[v] += dxHy; }
-      else {
+      else if (!xvec) {
         const int si = slab_coord(i0 + v, p.lo[0], p.hi[0], p.nx);
         T ikx = T(1), pyx = T(0), pzx = T(0);
         if (si >= 0 && i0 + v < p.nx) {
@@ -228,6 +252,20 @@ __device__ __forceinline__ void update_E_vec(const StepParams<T>& p, int i0, int
       }
       d0[v] = dyHz; d1[v] = dyHx; d2[v] = dzHy; d3[v] = dzHx;
     }
+  }
+  if (xs && xvec) {  // x slab, whole vector: psiEyx (from D-x Hz) -> Ey, psiEzx (from D-x Hy) -> Ez
+    const int si0 = slab_coord(i0, p.lo[0], p.hi[0], p.nx);
+    const long long q = si0 + (long long)(p.lo[0] + p.hi[0]) * (j + (long long)p.ny * k);
+    T a[V], d[V], b[V], c[V], ik[V];
+    ldv(p.psi[pEyx] + q, a); ldv(p.psi[pEzx] + q, d);
+    ldv(p.bE[0] + si0, b); ldv(p.cE[0] + si0, c); ldv(p.kE[0] + si0, ik);
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      a[v] = b[v] * a[v] + c[v] * dxa[v]; d[v] = b[v] * d[v] + c[v] * dxb[v];
+      ay[v] -= dxa[v] * ik[v] + a[v];
+      az[v] += dxb[v] * ik[v] + d[v];
+    }
+    stv(p.psi[pEyx] + q, a); stv(p.psi[pEzx] + q, d);
   }
   if (sj >= 0) {  // y slab: psiExy (from D-y Hz), psiEzy (from D-y Hx)
     const long long q = i0 + (long long)p.P * (sj + (long long)(p.lo[1] + p.hi[1]) * k);
