@@ -39,7 +39,9 @@ struct FusedParams {
   CUtensorMap tm[7];     // boxes of the set being read: Ex Ey Ez Hx Hy Hz, then the uint8 material index
   StepParams<T> sp;      // src = set read, dst = set written; psi[0..5] = psi_H written, psi[6..11] = psi_E (in place)
   const T* psiH_src[6];  // psi_H read (pHxy pHzy pHxz pHyz pHyx pHzx)
-  int kz;                // planes per z chunk (grid.z = ceil(nz / kz))
+  int kz;                // planes per z chunk
+  int ntx, nty, group;   // tiles in x, y; dispatch order: groups of `group` tiles, all z chunks of a group in ascending
+                         // order before the next group (1-D grid: block -> (group, chunk, tile of the group))
   const T* cpack;        // the 18 CPML vectors [axis][bE cE kE bH cH kH][kMaxSlab], contiguous
 };
 
@@ -211,11 +213,23 @@ __global__ void __launch_bounds__((TY + 2) * 32, 1) k_step_fused(const __grid_co
 
   const StepParams<T>& p = fp.sp;
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
-  const int k0 = blockIdx.z * fp.kz, k1 = min(k0 + fp.kz, p.nz);
+  // block -> (tile, chunk).  The hardware dispatches blocks in index order, so the co-resident blocks are `group`
+  // neighbouring tiles at (nearly) the same chunk: their streams stay within a narrow band of planes, halo rows/columns
+  // of neighbours hit in L2, and a tile's next chunk follows one wave after the previous one.
+  int tile, chunk;
+  {
+    const int tiles = fp.ntx * fp.nty, nchunk = (p.nz + fp.kz - 1) / fp.kz;
+    const int per_group = fp.group * nchunk, g = blockIdx.x / per_group;
+    const int gsize = min(fp.group, tiles - g * fp.group), rem = blockIdx.x - g * per_group;
+    chunk = rem / gsize;
+    tile = g * fp.group + (rem - chunk * gsize);
+  }
+  const int ty_ = tile / fp.ntx;
+  const int x0 = (tile - ty_ * fp.ntx) * TX, y0 = ty_ * TY;
+  const int k0 = chunk * fp.kz, k1 = min(k0 + fp.kz, p.nz);
   const int nIt = k1 - k0 + 2;  // it = 0: Ex, Ey of plane k0-1 only; it = 1: H of plane k0-1; it >= 2: plane k0 + it - 2
 
-  if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && threadIdx.x == 0) *p.nstep += 1;
+  if (blockIdx.x == 0 && threadIdx.x == 0) *p.nstep += 1;
 
   // one elected thread issues the boxes of iteration `it` (plane k) into stage s
   auto issue = [&](int it, int s) {
