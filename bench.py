@@ -42,7 +42,7 @@ UNIT = "Mcell-updates/s"
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch, from the ncu captures summarised under profiles/
 NCU_TRAFFIC = {
-    ("c3", "k_step_fused", 32): (49.44e9, "profiles/r01_final.md (26.24 GB read + 23.20 GB written)"),
+    ("c3", "k_step_fused", 32): (47.98e9, "profiles/r01_final.md, group dispatch (24.78 GB read + 23.21 GB written)"),
     ("c3", "k_update_E", 32): (35.24e9, "profiles/r01_twopass.md"),
     ("c3", "k_update_H", 32): (34.39e9, "profiles/r01_twopass.md"),
 }
