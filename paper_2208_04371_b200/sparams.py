@@ -52,3 +52,36 @@ def phase_delay(s, freqs):
     physical delay; the paper's sign is that of its own time convention (R30)."""
     th = np.degrees(np.unwrap(np.angle(np.asarray(s, dtype=np.complex128))))
     return th / (360.0 * np.asarray(freqs, dtype=np.float64))
+
+
+def abcd_from_s(S, z0=50.0):
+    """Two-port S (on the real reference z0 at both ports, [2, 2, F]) -> ABCD chain matrix [2, 2, F]
+    ("S* can also be converted to an ABCD matrix"; the standard two-port conversion, Pozar [3])."""
+    S = np.asarray(S, dtype=np.complex128)
+    s11, s12, s21, s22 = S[0, 0], S[0, 1], S[1, 0], S[1, 1]
+    A = ((1 + s11) * (1 - s22) + s12 * s21) / (2 * s21)
+    B = z0 * ((1 + s11) * (1 + s22) - s12 * s21) / (2 * s21)
+    Cc = ((1 - s11) * (1 - s22) - s12 * s21) / (2 * s21) / z0
+    D = ((1 - s11) * (1 + s22) + s12 * s21) / (2 * s21)
+    return np.array([[A, B], [Cc, D]])
+
+
+def telegrapher_from_abcd(abcd, length, freqs):
+    """Overall characteristic impedance and per-unit-length R, L, G, C of the "simplest Telegrapher's model" (PAPER.md:89,
+    128-134): a uniform line of the given length with the same ABCD matrix, A = cosh(gamma l), B = Z0 sinh(gamma l),
+    C = sinh(gamma l) / Z0:  Z0 = sqrt(B / C), gamma = acosh(A) / l (branch unwrapped along frequency, Re gamma >= 0),
+    R + j w L = gamma Z0,  G + j w C = gamma / Z0.  Returns a dict of arrays over frequency."""
+    A, Bm, Cm = abcd[0, 0], abcd[0, 1], abcd[1, 0]
+    f = np.asarray(freqs, dtype=np.float64)
+    z0 = np.sqrt(Bm / Cm)
+    z0 = np.where(z0.real < 0, -z0, z0)
+    gl = np.arccosh(A)                                   # principal value: Re >= 0, Im in [0, pi] (beta l folded)
+    gl = np.where(gl.real < 0, -gl, gl)
+    # unfold beta l: sinh(gamma l) = B / Z0 decides the sign of the imaginary part, then unwrap along frequency
+    sh = Bm / z0
+    im = np.where(np.sign(np.sinh(gl).imag) == np.sign(sh.imag), gl.imag, -gl.imag)
+    beta_l = np.unwrap(im)
+    gamma = (gl.real + 1j * beta_l) / length
+    w = 2 * np.pi * f
+    series, shunt = gamma * z0, gamma / z0
+    return {"Z0": z0, "gamma": gamma, "R": series.real, "L": series.imag / w, "G": shunt.real, "C": shunt.imag / w}

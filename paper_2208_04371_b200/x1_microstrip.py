@@ -45,10 +45,12 @@ def run(w, device="cuda:0", options=None):
     beta = theta / l
     v = 2 * np.pi * f / beta
     th = theory(w)
+    tl = sparams.telegrapher_from_abcd(sparams.abcd_from_s(S), l, f)   # S -> ABCD -> Z0, L, C (Fig. 1c)
     kappa = np.exp(-1j * 2 * np.pi * f * math.sqrt(th["eps_eff"]) / C0 * l)
     g = th["gamma"]
     return {"freqs": f, "l": l, "impl": impl, "Z_r": zr, "S_star21": s21, "S11": S[0, 0], "S21": S[1, 0],
             "eps_eff": (C0 / v) ** 2, "C": 1.0 / (zr.real * v), "L": zr.real / v,
+            "Z0_abcd": tl["Z0"], "C_abcd": tl["C"], "L_abcd": tl["L"], "beta_l": theta,
             "S11_th": (1 - kappa ** 2) * g / (1 - kappa ** 2 * g ** 2), "S21_th": (1 - g ** 2) * kappa / (1 - kappa ** 2 * g ** 2),
             "C_th": math.sqrt(th["eps_eff"]) / (th["z0"] * C0), "L_th": th["z0"] * math.sqrt(th["eps_eff"]) / C0, "theory": th}
 

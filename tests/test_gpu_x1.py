@@ -50,6 +50,13 @@ def test_x1_paper_size_against_eq7(golden_dir):
     # Eq. 7: per-unit-length C and L
     assert np.abs(r["C"][band] / r["C_th"] - 1).max() < 0.03
     assert np.abs(r["L"][band] / r["L_th"] - 1).max() < 0.08 and abs(r["L"][0] / r["L_th"] - 1) < 0.01
+    # the same through the ABCD matrix and the Telegrapher's model (the route of the paper's Fig. 1c)
+    # away from the half-wavelength points beta l = m pi, where B and C of the ABCD matrix both vanish and Z0 = sqrt(B/C)
+    # is ill-conditioned (every other frequency of this 0.5 GHz grid is close to one: there Z0 comes out 10 % high)
+    ok = band & (np.abs(np.sin(r["beta_l"])) > 0.7)
+    assert ok.sum() >= 6
+    assert np.abs(r["Z0_abcd"][ok].real / 25.0 - 1).max() < 0.04
+    assert np.abs(r["C_abcd"][ok] / r["C_th"] - 1).max() < 0.03 and np.abs(r["L_abcd"][ok] / r["L_th"] - 1).max() < 0.08
     # Eq. 7: S on 50 ohm.  Envelope of the ripple: max|S11| = 2|G|/(1+G^2) = 0.6, min|S21| = (1-G^2)/(1+G^2) = 0.8
     g = th["gamma"]
     assert abs(np.abs(r["S11"][band]).max() - 2 * abs(g) / (1 + g * g)) < 0.02

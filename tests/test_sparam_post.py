@@ -101,3 +101,26 @@ def test_drive_port_moves_the_source():
         assert (t["sj0"], t["sj1"], t["sk0"], t["sk1"]) == (t["vj0"], t["vj1"], t["vk0"], t["vk1"])
         assert (t["ip"] - t["is"]) * d == abs(w["ports"][0]["ip"] - w["ports"][0]["is"])
     assert w["ports"][0]["has_source"] == 1                  # the input workload is not modified
+
+
+def test_abcd_and_telegrapher_recover_a_lossy_line():
+    """PAPER.md:89 (S* -> ABCD -> characteristic impedance and RLGC of the simplest Telegrapher's model): a uniform lossy
+    line built from R, L, G, C by textbook circuit theory must come back, through several turns of phase."""
+    R_, L_, G_, C_ = 120.0, 2.5e-7, 0.02, 1.0e-10
+    l = 0.05
+    f = np.linspace(0.2e9, 20e9, 400)
+    w = 2 * np.pi * f
+    z = R_ + 1j * w * L_
+    y = G_ + 1j * w * C_
+    gamma, zc = np.sqrt(z * y), np.sqrt(z / y)
+    A = np.cosh(gamma * l); B = zc * np.sinh(gamma * l); Cm = np.sinh(gamma * l) / zc
+    # S on 50 ohm from ABCD (textbook), then back through the package
+    den = A + B / 50 + Cm * 50 + A
+    S = np.array([[(A + B / 50 - Cm * 50 - A) / den, 2 * (A * A - B * Cm) / den], [2 / den, (-A + B / 50 - Cm * 50 + A) / den]])
+    abcd = P.abcd_from_s(S)
+    assert np.abs(abcd[0, 0] - A).max() < 1e-9 and np.abs(abcd[0, 1] - B).max() < 1e-7 and np.abs(abcd[1, 0] - Cm).max() < 1e-11
+    t = P.telegrapher_from_abcd(abcd, l, f)
+    assert np.abs(t["Z0"] / zc - 1).max() < 1e-9
+    assert np.abs(t["R"] / R_ - 1).max() < 1e-6 and np.abs(t["L"] / L_ - 1).max() < 1e-8
+    assert np.abs(t["G"] / G_ - 1).max() < 1e-6 and np.abs(t["C"] / C_ - 1).max() < 1e-8
+    assert (np.diff(t["gamma"].imag) > 0).all() and t["gamma"].imag[-1] * l > 4 * np.pi      # unwrapped past 2 turns
