@@ -124,7 +124,6 @@ struct Solver : fdtd {
   int kz = 0;
   int sm_count = 148;
   unsigned probe_blocks = 1; // blocks per port of k_probe_dft: about 1024 samples of the largest V box each
-  double tuned_ms = 0.0;     // field-kernel time of the configuration autotune() kept
   FusedParams<T> fpar[2];
   cudaGraphExec_t gexec2 = nullptr;  // graph captured with cur == 1
   std::vector<T> h_tab;        // host staging of the material table (kept alive for the async upload)
@@ -541,12 +540,8 @@ int Solver<T>::build_fused() {
     default: e = fused_set_attr<T, 3>(); break;
   }
   if (e != cudaSuccess) return cuda_fail(e, "fdtd_commit: shared memory opt-in of the fused kernel");
-  // planes per z chunk.  Blocks are dispatched chunk by chunk (blockIdx.z slowest), so the co-resident blocks sit within
-  // two chunks of each other in z: short chunks keep their 13 streams inside a narrow band of planes (measured on C3:
-  // 9.0 ms/step at 128 planes, 8.2 ms at 24..32, 8.4 ms at 16 where the two priming planes per chunk start to cost).
-  const long long tiles = (long long)((nx + C::TX - 1) / C::TX) * ((ny + C::TY - 1) / C::TY);
-  // fdtd_commit then times the candidates on the committed (all-zero) state and keeps the fastest: autotune().
-  (void)tiles;
+  // planes per z chunk: the caller set a starting value; fdtd_commit then times the candidates on the committed
+  // (all-zero) state and keeps the fastest: autotune().  Why short chunks win is in fdtd_fused.cuh / DESIGN.md 6.2.
   if (kz > nz) kz = nz;
   if (kz < 1) kz = 1;
   {
@@ -655,7 +650,6 @@ int Solver<T>::autotune() {
   kz = best_kz;
   fpar[0].kz = fpar[1].kz = kz;
   cur = 0;
-  tuned_ms = best;
   cudaError_t e = cudaMemsetAsync(sp.nstep, 0, sizeof(long long), stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
   if (e != cudaSuccess) return cuda_fail(e, "fdtd_commit: autotune");
