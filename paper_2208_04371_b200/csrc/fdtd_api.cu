@@ -479,11 +479,10 @@ int Solver<T>::set_materials_full(const void* const eps[3], const void* const si
 template <typename T, int MODE>
 static void launch_two_pass(const StepParams<T>& sp, cudaStream_t st, cudaEvent_t* ev) {
   constexpr int V = VecOf<T>::V;
-  const int nvec = (sp.nx + V - 1) / V;
-  int bx = 1;
-  while (bx < nvec && bx < 128) bx <<= 1;
-  const int by = 128 / bx;
-  const dim3 block(bx, by, 1), grid((nvec + bx - 1) / bx, (sp.ny + by - 1) / by, sp.nz);
+  const int nrow = (sp.nx + V - 1) / V;                                 // vectors per row
+  const long long nvec = (long long)nrow * sp.ny;                        // ... per plane, rows back to back
+  const dim3 block(128, 1, 1);
+  const dim3 grid = (nrow % 128 == 0 && sp.ny > 1) ? dim3(nrow / 128, sp.ny, sp.nz) : dim3((unsigned)((nvec + 127) / 128), 1, sp.nz);
   if (ev) cudaEventRecord(ev[0], st);
   k_update_H<T, MODE><<<grid, block, 0, st>>>(sp);
   if (ev) cudaEventRecord(ev[1], st);
@@ -909,11 +908,8 @@ int Solver<T>::step_begin() {
 template <typename T, int MODE>
 static void launch_E_plane0(const StepParams<T>& q, cudaStream_t st) {
   constexpr int V = VecOf<T>::V;
-  const int nvec = (q.nx + V - 1) / V;
-  int bx = 1;
-  while (bx < nvec && bx < 128) bx <<= 1;
-  const int by = 128 / bx;
-  k_update_E<T, MODE><<<dim3((nvec + bx - 1) / bx, (q.ny + by - 1) / by, 1), dim3(bx, by, 1), 0, st>>>(q);
+  const long long nvec = (long long)((q.nx + V - 1) / V) * q.ny;
+  k_update_E<T, MODE><<<dim3((unsigned)((nvec + 127) / 128), 1, 1), dim3(128, 1, 1), 0, st>>>(q);
 }
 
 template <typename T>

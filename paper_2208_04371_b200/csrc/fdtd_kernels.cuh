@@ -190,11 +190,14 @@ __device__ __forceinline__ void update_H_vec(const StepParams<T>& p, int i0, int
 template <typename T, int MODE>
 __global__ void __launch_bounds__(128) k_update_H(const StepParams<T> p) {
   constexpr int V = VecOf<T>::V;
-  const int i0 = (blockIdx.x * blockDim.x + threadIdx.x) * V;
-  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  // threads are numbered along the row vectors of a plane, rows back to back: no idle lanes when a row is not a
+  // multiple of the block (the X3-shaped grid: 50 vectors per row)
+  // (rows that are a whole number of blocks keep one row per blockIdx.y and skip the division)
+  const int nvec = (p.nx + V - 1) / V, v = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = gridDim.y > 1 ? (int)blockIdx.y : v / nvec, i0 = (gridDim.y > 1 ? v : v - j * nvec) * V;
   const int k = blockIdx.z;
-  if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && threadIdx.x == 0 && threadIdx.y == 0) *p.nstep += 1;
-  if (i0 >= p.nx || j >= p.ny) return;
+  if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && threadIdx.x == 0) *p.nstep += 1;
+  if (j >= p.ny) return;
   update_H_vec<T, MODE>(p, i0, j, k);
 }
 
@@ -324,10 +327,10 @@ __device__ __forceinline__ void update_E_vec(const StepParams<T>& p, int i0, int
 template <typename T, int MODE>
 __global__ void __launch_bounds__(128) k_update_E(const StepParams<T> p) {
   constexpr int V = VecOf<T>::V;
-  const int i0 = (blockIdx.x * blockDim.x + threadIdx.x) * V;
-  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int nvec = (p.nx + V - 1) / V, v = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = gridDim.y > 1 ? (int)blockIdx.y : v / nvec, i0 = (gridDim.y > 1 ? v : v - j * nvec) * V;
   const int k = blockIdx.z;
-  if (i0 >= p.nx || j >= p.ny) return;
+  if (j >= p.ny) return;
   update_E_vec<T, MODE>(p, i0, j, k);
 }
 
