@@ -672,7 +672,7 @@ template <typename T>
 int Solver<T>::launch_persistent(const PortParams<T>& q, long n) {
   cudaError_t e = cudaSuccess;
   while (n > 0 && e == cudaSuccess) {
-    const int m = (int)(n > (1L << 20) ? (1L << 20) : n);
+    const int m = (int)(n > 4096 ? 4096 : n);   // a launch stays well under a second even on the largest eligible grid
     switch (mode()) {
       case 0: e = persistent_launch<T, 0>(sp, q, m, persist_blocks, stream); break;
       case 1: e = persistent_launch<T, 1>(sp, q, m, persist_blocks, stream); break;
@@ -861,7 +861,7 @@ int Solver<T>::step(long n) {
   if (persistent && n > 0) {
     const int r = launch_persistent(pp, n);
     if (r != FDTD_OK) return r;
-    launches += 1;
+    launches += (n + 4095) / 4096;
     nstep += n;
     return FDTD_OK;
   }
