@@ -50,11 +50,12 @@ enum { FDTD_EX = 0, FDTD_EY, FDTD_EZ, FDTD_HX, FDTD_HY, FDTD_HZ };
 
 /* Options for fdtd_set_option (before commit). */
 enum {
-  FDTD_OPT_STEP_IMPL = 1,   /* 0 = auto (two-pass below 4 Mi cells; above, whichever fdtd_commit measures faster),
+  FDTD_OPT_STEP_IMPL = 1,   /* 0 = auto: fdtd_commit measures the candidates on the committed all-zero state and keeps the
+                                   fastest (below 4 Mi cells: two-pass vs persistent; above: two-pass vs fused),
                                1 = two-pass (H kernel, E kernel, in place),
                                2 = fused E+H kernel (temporal blocking over the half steps; a second field set),
-                               3 = persistent: every fdtd_step(n) is ONE cooperative launch that does all n steps with
-                                   grid-wide barriers between the half steps (grids that live in L2; same arithmetic as 1) */
+                               3 = persistent: fdtd_step(n) is one cooperative launch per 4096 steps, with grid-wide
+                                   barriers between the half steps (grids that live in L2; the arithmetic of 1)         */
   FDTD_OPT_USE_GRAPH = 2,   /* 1 (default) = replay a captured CUDA graph per step; 0 = plain launches                  */
   FDTD_OPT_GRAPH_UNROLL = 3,/* steps per captured graph (default 8; rounded up to even for the fused step)              */
   FDTD_OPT_FUSED_KZ = 4     /* planes per z chunk of the fused kernel (0 = auto: measured at commit)                    */
