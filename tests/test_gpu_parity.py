@@ -165,6 +165,9 @@ def test_C3_small_scale_indexed_six_face_cpml(impl):
     w = W.throughput_c3(div=8, steps=300, npml=6, nf=16)
     o, s, rep = run_pair(w, 300, options={FDTD_OPT_STEP_IMPL: impl}, checkpoints=[20, 300])
     assert_fields(rep, FDTD_F32)
+    # the S* column of port 1 over the four ports (one structure: tot == inc, so S*_11 = 0 and the rest are transfer ratios)
+    So, Sg = _sstar(o, o, 4, osp), _sstar(s, s, 4, sparams)
+    assert np.isfinite(Sg).all() and np.abs(So - Sg).max() <= 1e-3
 
 
 @pytest.mark.parametrize("impl", IMPLS)
