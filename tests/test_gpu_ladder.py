@@ -40,6 +40,18 @@ def test_C1_full_length_sparams():
     # R14: raw fp32 DFTs drift ~1.2e-8 per step against fp64 in the DC-limit band: informational, but it must stay drift-sized
     assert max(rep["dft_err"]) <= 5e-3
     s.destroy()
+    # the yardstick of R14 / SURVEY G31: the oracle's own fp32 instantiation (same algorithm, same order) against its fp64
+    # run.  The GPU's gap to the fp64 oracle must be of the size of that gap: it is fp32 time stepping, not the kernels.
+    from oracle.yee import YeeOracle
+    o32 = YeeOracle.from_workload(w, f32=True)
+    o32.step(w["steps"])
+    vmax = max(np.abs(o.read_port_dft(p)[0]).max() for p in range(2))
+    imax = max(np.abs(o.read_port_dft(p)[1]).max() for p in range(2))
+    y_v = max(np.abs(o32.read_port_dft(p)[0] - o.read_port_dft(p)[0]).max() for p in range(2)) / vmax
+    y_i = max(np.abs(o32.read_port_dft(p)[1] - o.read_port_dft(p)[1]).max() for p in range(2)) / imax
+    S32 = _sstar(o32, 2, osp)
+    print(f"C1 40k steps, yardstick: fp32 oracle vs fp64 oracle raw dft (V, I) = ({y_v:.3e}, {y_i:.3e}), dS = {np.abs(S32 - So).max():.3e}")
+    assert rep["dft_err"][0] <= 4 * y_v + 1e-6 and rep["dft_err"][1] <= 4 * y_i + 1e-6
 
 
 @pytest.mark.parametrize("impl", [0, 2])
