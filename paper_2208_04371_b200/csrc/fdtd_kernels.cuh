@@ -217,6 +217,9 @@ __device__ __forceinline__ void update_E_vec(const StepParams<T>& p, int i0, int
   ldv(p.src[kHx] + o - p.P, hxj);  ldv(p.src[kHz] + o - p.P, hzj);
   const T hyi = p.src[kHy][o - 1], hzi = p.src[kHz][o - 1];
   ldv(p.src[kEx] + o, ex); ldv(p.src[kEy] + o, ey); ldv(p.src[kEz] + o, ez);
+  // the material index goes out with the field loads: it heads the longest dependent chain (index -> table -> update)
+  unsigned char mi[V];
+  if (!(MODE & kModeFull)) ld_index<V>(p.idx + o, mi);
 
   const int sj = slab_coord(j, p.lo[1], p.hi[1], p.ny);
   const int sk = slab_coord(k, p.lo[2], p.hi[2], p.nz);
@@ -301,12 +304,10 @@ __device__ __forceinline__ void update_E_vec(const StepParams<T>& p, int i0, int
     ldv(p.Ca[0] + o, cax); ldv(p.Ca[1] + o, cay); ldv(p.Ca[2] + o, caz);
     ldv(p.Cb[0] + o, cbx); ldv(p.Cb[1] + o, cby); ldv(p.Cb[2] + o, cbz);
   } else {
-    unsigned char m[V];
-    ld_index<V>(p.idx + o, m);    // one 32-bit (16-bit) load for the thread's 4 (2) cells
 #pragma unroll
-    for (int v = 0; v < V; ++v) {
-      const Vec4<T> a = ld4(p.tab + 8 * (int)m[v]);       // {Cax, Cay, Caz, Cbx}
-      const Vec4<T> b = ld4(p.tab + 8 * (int)m[v] + 4);   // {Cby, Cbz, -, -}
+    for (int v = 0; v < V; ++v) {   // mi: one 32-bit (16-bit) load for the thread's 4 (2) cells, issued with the field loads
+      const Vec4<T> a = ld4(p.tab + 8 * (int)mi[v]);       // {Cax, Cay, Caz, Cbx}
+      const Vec4<T> b = ld4(p.tab + 8 * (int)mi[v] + 4);   // {Cby, Cbz, -, -}
       cax[v] = a.a; cay[v] = a.b; caz[v] = a.c; cbx[v] = a.d; cby[v] = b.a; cbz[v] = b.b;
     }
   }
