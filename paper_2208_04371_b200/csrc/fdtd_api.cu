@@ -617,7 +617,7 @@ double Solver<T>::time_field_kernels(int reps) {
 // Choice of the step implementation and of the z chunk length, measured rather than modelled.  How well the fused kernel
 // does depends on how the (tile, chunk) blocks fill the SMs (mid-size grids give only a few waves of blocks) and on how far
 // apart in z the co-resident blocks drift; both are properties of this grid on this device.
-//   FDTD_OPT_STEP_IMPL 0 (auto): two-pass and fused with kz in {12, 16, 20, 24, 32, 48} compete;
+//   FDTD_OPT_STEP_IMPL 0 (auto): two-pass and fused with kz in {8, 12, 16, 20, 24, 32, 48} compete;
 //   FDTD_OPT_STEP_IMPL 2 with FDTD_OPT_FUSED_KZ 0: the kz candidates compete.
 template <typename T>
 int Solver<T>::autotune() {
@@ -626,8 +626,8 @@ int Solver<T>::autotune() {
   int best_kz = kz;
   bool best_fused = true;
   if (opt_kz <= 0) {
-    const int cand[6] = {12, 16, 20, 24, 32, 48};
-    for (int c = 0; c < 6; ++c) {
+    const int cand[7] = {8, 12, 16, 20, 24, 32, 48};
+    for (int c = 0; c < 7; ++c) {
       if (cand[c] > nz && c > 0) break;
       kz = cand[c] > nz ? nz : cand[c];
       fpar[0].kz = fpar[1].kz = kz;
