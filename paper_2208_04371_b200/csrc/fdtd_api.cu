@@ -209,7 +209,7 @@ struct Solver : fdtd {
   int autotune();
   int autotune_kz_only() { const long keep = opt_impl; opt_impl = 2; const int r = autotune(); opt_impl = keep; return r; }
   int setup_persistent();
-  int launch_persistent(const PortParams<T>& q, long n);
+  int launch_persistent(const PortParams<T>& q, long n, long* done = nullptr);
   double time_field_kernels(int reps);
   void launch_fused(cudaEvent_t* ev);
 
@@ -669,8 +669,9 @@ static cudaError_t persistent_occupancy(int* per_sm) {
 }
 
 template <typename T>
-int Solver<T>::launch_persistent(const PortParams<T>& q, long n) {
+int Solver<T>::launch_persistent(const PortParams<T>& q, long n, long* done) {
   cudaError_t e = cudaSuccess;
+  if (done) *done = 0;
   while (n > 0 && e == cudaSuccess) {
     const int m = (int)(n > 4096 ? 4096 : n);   // a launch stays well under a second even on the largest eligible grid
     switch (mode()) {
@@ -680,6 +681,7 @@ int Solver<T>::launch_persistent(const PortParams<T>& q, long n) {
       default: e = persistent_launch<T, 3>(sp, q, m, persist_blocks, stream); break;
     }
     n -= m;
+    if (e == cudaSuccess && done) *done += m;
   }
   return e == cudaSuccess ? FDTD_OK : cuda_fail(e, "cooperative launch of the persistent step kernel");
 }
@@ -859,11 +861,17 @@ int Solver<T>::step(long n) {
     return fail(FDTD_ESTATE, "fdtd_step: a z slab advances with fdtd_step_begin / plane exchange / fdtd_step_end");
   long left = n;
   if (persistent && n > 0) {
-    const int r = launch_persistent(pp, n);
-    if (r != FDTD_OK) return r;
-    launches += (n + 4095) / 4096;
-    nstep += n;
-    return FDTD_OK;
+    long done = 0;
+    const int r = launch_persistent(pp, n, &done);
+    launches += (done + 4095) / 4096;
+    nstep += done;
+    if (r == FDTD_OK) return FDTD_OK;
+    // A cooperative launch can be refused when fewer SMs are available than at commit.  If that happens before anything
+    // was enqueued and the persistent step was not asked for by name, the handle drops to the two-pass kernels for good.
+    cudaGetLastError();
+    if (opt_impl == 3 || done != 0) return r;
+    persistent = false;
+    err.clear();
   }
   graph_steps = (int)opt_unroll + ((fused && (opt_unroll & 1)) ? 1 : 0);
   if (opt_graph && stream != nullptr && left >= graph_steps) {
