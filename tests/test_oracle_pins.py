@@ -492,3 +492,26 @@ def test_fp32_instantiation_tracks_fp64():
     for c in range(6):
         e = np.abs(a.read_field(c) - b.read_field(c)).max() / (emax if c < 3 else hmax)
         assert 0 < e < 1e-5
+
+
+def test_R31_far_end_drive_orientation_and_reciprocity_of_the_protocol():
+    """Driving the parallel-plate line from its far port (workloads.drive_port) sends the wave towards -x: V/I changes
+    sign, and the oriented reference impedance Z_r = -d V/I (R31; d = +1 for a +x drive, -1 for a -x drive) is
+    +eta0 gap/width for both drives -- the sign Eq. 5 needs.  The two S*_21 of the two-run-per-port protocol
+    agree: the uniform vacuum line is reciprocal."""
+    fr = np.linspace(5e12, 250e12, 24)
+    w = W.parallel_plate(freqs=fr, steps=3000)
+    Z_th = ETA0 * w["gap_m"] / w["width_m"]
+    S21 = []
+    for j in (0, 1):
+        wj, d = W.drive_port(w, j)
+        assert d == (1, -1)[j]
+        o = YeeOracle.from_workload(wj)
+        o.step(3000)
+        V = [o.read_port_dft(p)[0] for p in range(2)]
+        I = [o.read_port_dft(p)[1] for p in range(2)]
+        zr = -d * V[j] / I[j]
+        assert np.abs(zr.real / Z_th - 1).max() < 1e-3 and np.abs(zr.imag).max() < 0.1 * Z_th
+        S = osp.s_star_column(j, V, I, V)
+        S21.append(np.array(S[1 - j]))
+    assert np.abs(S21[0] - S21[1]).max() < 1e-5
