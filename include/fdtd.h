@@ -28,6 +28,10 @@
  *             fdtd_set_option} in any order -> fdtd_workspace_bytes -> fdtd_commit -> {fdtd_set_materials_*,
  *             fdtd_step, fdtd_read_*, fdtd_write_fields, fdtd_reset} -> fdtd_destroy.
  *             Calling out of order returns FDTD_ESTATE.  A freshly committed object is vacuum, all state zero.
+ *   Device    a handle belongs to the device its workspace lives on (fdtd_commit asks the runtime).  Every later call
+ *             makes that device current for its own duration and restores the caller's, so a handle committed on
+ *             device 1 may be driven while device 0 is current.  The stream given to fdtd_commit must be one of that
+ *             device.
  *   Threads   one handle must not be used from two host threads at once.
  */
 #ifndef FDTD_B200_H
@@ -56,7 +60,9 @@ enum {
                                2 = fused E+H kernel (temporal blocking over the half steps; a second field set),
                                3 = persistent: fdtd_step(n) is one cooperative launch per 4096 steps, with grid-wide
                                    barriers between the half steps (grids that live in L2; the arithmetic of 1)         */
-  FDTD_OPT_USE_GRAPH = 2,   /* 1 (default) = replay a captured CUDA graph per step; 0 = plain launches                  */
+  FDTD_OPT_USE_GRAPH = 2,   /* 1 (default) = replay a captured CUDA graph per FDTD_OPT_GRAPH_UNROLL steps; 0 = plain launches.
+                               Capture needs a real stream: on the NULL (legacy default) stream fdtd_step always issues
+                               plain launches (fdtd_graph_replays() stays 0)                                             */
   FDTD_OPT_GRAPH_UNROLL = 3,/* steps per captured graph (default 8; rounded up to even for the fused step)              */
   FDTD_OPT_FUSED_KZ = 4     /* planes per z chunk of the fused kernel (0 = auto: measured at commit)                    */
 };
@@ -96,7 +102,8 @@ int fdtd_set_boundary(fdtd_t*, const int pml_cells[6], const double* cpml);
  * has_mu != 0 reserves room for per-entry / per-cell permeability. */
 int fdtd_set_material_mode(fdtd_t*, int mode, int has_mu);
 
-/* Add a port; *port_id (may be NULL) receives its index.  FDTD_ERANGE if a sample lies outside the grid. */
+/* Add a port; *port_id (may be NULL) receives its index.  FDTD_ERANGE if a sample lies outside the grid, or if the source
+ * box touches the plane i = 0 or the row j = 0: E_z there is a PEC wall sample that stays zero (R1). */
 int fdtd_add_port(fdtd_t*, const fdtd_port* p, int* port_id);
 
 /* Frequencies [Hz] of the running DFT of every port's V and I.  nf = 0 switches it off. */
@@ -108,8 +115,9 @@ int fdtd_set_option(fdtd_t*, int option, long value);
 size_t fdtd_workspace_bytes(const fdtd_t*);
 
 /* Adopt the caller's device buffer (device pointer, >= fdtd_workspace_bytes(), 256-byte aligned) and CUDA stream
- * (a cudaStream_t passed as void*; NULL = the legacy default stream), build the CPML / port tables, zero all state,
- * set vacuum everywhere.  All later work is enqueued on that stream. */
+ * (a cudaStream_t passed as void*; NULL = the legacy default stream, on which no CUDA graph can be captured), build the
+ * CPML / port tables, zero all state, set vacuum everywhere.  All later work is enqueued on that stream.
+ * FDTD_EINVAL also when FDTD_OPT_STEP_IMPL = 2 was asked for with more than 64 CPML cells (lo + hi) on an axis. */
 int fdtd_commit(fdtd_t*, void* device_workspace, size_t bytes, void* cuda_stream);
 
 /* Materials, component-sampled at the location of each E (eps_r, sigma) and H (mu_r) sample; the library never
@@ -129,12 +137,14 @@ int fdtd_step(fdtd_t*, long n);
 /* Run n full steps exactly like fdtd_step (plain launches, no graph) with CUDA events recorded on the stream between
  * the kernels, and return the average device time per step, in milliseconds, of
  *   ms_avg[0] = H pass (or the fused E+H kernel), ms_avg[1] = E pass (0 when fused), ms_avg[2] = source injection,
- *   ms_avg[3] = probes + DFT.   This is the measurement hook of bench.py's roofline line.  Synchronises the stream. */
+ *   ms_avg[3] = probes + DFT.   This is the measurement hook of bench.py's roofline line.  Synchronises the stream.
+ * FDTD_ESTATE on a z slab (fdtd_set_z_interfaces) or between fdtd_step_begin and fdtd_step_end. */
 int fdtd_profile_step(fdtd_t*, long n, double ms_avg[4]);
 
 /* Copy one field component (FDTD_EX..FDTD_HZ) to / from a caller array of N elements of the field precision, host or
  * device.  Stream-ordered; synchronises the stream before returning when the caller array is in host memory.
- * write_fields is the test hook for initial conditions and the resume path. */
+ * write_fields is the test hook for initial conditions and the resume path; FDTD_ESTATE between fdtd_step_begin and
+ * fdtd_step_end (the two field sets are half updated then). */
 int fdtd_read_fields(fdtd_t*, int comp, void* dst);
 int fdtd_write_fields(fdtd_t*, int comp, const void* src);
 
@@ -171,6 +181,10 @@ int fdtd_plane(fdtd_t*, int comp, int k, void** dev_ptr, size_t* bytes);
 long fdtd_step_count(const fdtd_t*);
 /* Number of kernel launches the library has enqueued since commit (graph nodes count individually). */
 long fdtd_launch_count(const fdtd_t*);
+/* Number of CUDA-graph replays fdtd_step has issued since commit (each covers FDTD_OPT_GRAPH_UNROLL steps). */
+long fdtd_graph_replays(const fdtd_t*);
+/* Ordinal of the CUDA device the handle was committed on (-1 before commit). */
+int fdtd_device(const fdtd_t*);
 /* Name of the step implementation in use after commit ("two_pass", "fused"), for reports. */
 const char* fdtd_impl_name(const fdtd_t*);
 /* z chunk length of the fused step in use after commit (0 for the two-pass step), for reports.  With

@@ -55,6 +55,7 @@ def lib():
         L.yo_read_port_last.argtypes = [C.c_void_p, C.c_int, dp, dp]
         L.yo_running_max.argtypes = [C.c_void_p, dp, dp]
         L.yo_psi_norms.argtypes = [C.c_void_p, dp]
+        L.yo_cpml_profile.argtypes = [C.c_void_p, C.c_int, C.c_int, dp]
         _lib = L
     return _lib
 
@@ -219,6 +220,17 @@ class YeeOracle:
         h = C.c_double()
         self.L.yo_running_max(self.h, C.byref(e), C.byref(h))
         return e.value, h.value
+
+    def cpml_profile(self, axis):
+        """R4 coefficient vectors of one axis (0 x, 1 y, 2 z) at every index: dict bE cE ikE (integer positions),
+        bH cH ikH (half-integer positions); outside the slabs b = 1, c = 0, 1/kappa = 1."""
+        out = {}
+        for which, name in enumerate(("bE", "cE", "ikE", "bH", "cH", "ikH")):
+            v = np.zeros(self.shape[axis])
+            if self.L.yo_cpml_profile(self.h, axis, which, _dp(v)) != 0:
+                raise RuntimeError("yo_cpml_profile before commit")
+            out[name] = v
+        return out
 
     def psi_norms(self):
         out = np.zeros(12)

@@ -71,6 +71,7 @@ struct Base {
   virtual void read_field(int comp, double* dst) const = 0;
   virtual void write_field(int comp, const double* src) = 0;
   virtual void read_psi_norms(double* out12) const = 0;
+  virtual void read_cpml_profile(int axis, int which, double* out_n) const = 0;
 
   int nx = 0, ny = 0, nz = 0;
   double dx = 0, dy = 0, dz = 0, dt = 0;
@@ -347,6 +348,11 @@ struct Oracle : Base {
     const size_t n = N();
     for (size_t q = 0; q < n; ++q) F[comp][q] = (T)src[q];
   }
+  // which: 0 bE, 1 cE, 2 1/kappaE (integer positions), 3 bH, 4 cH, 5 1/kappaH (half-integer positions); n_of(axis) values
+  void read_cpml_profile(int a, int which, double* out) const override {
+    const std::vector<T>* v[6] = {&bE[a], &cE[a], &ikE[a], &bH[a], &cH[a], &ikH[a]};
+    for (int u = 0; u < n_of(a); ++u) out[u] = (double)(*v[which])[u];
+  }
   void read_psi_norms(double* out) const override {
     const std::vector<T>* v[12] = {&psiHxy, &psiHxz, &psiHyz, &psiHyx, &psiHzx, &psiHzy,
                                    &psiExy, &psiExz, &psiEyz, &psiEyx, &psiEzx, &psiEzy};
@@ -482,6 +488,14 @@ int yo_read_port_last(void* h, int port, double* V, double* I) {
 int yo_running_max(void* h, double* e, double* hm) {
   Base* b = static_cast<Base*>(h);
   *e = b->emax; *hm = b->hmax;
+  return 0;
+}
+
+// R4: the CPML coefficient vectors of one axis as the oracle uses them (pin: tests/golden/cpml_profile_lo4_hi3.txt)
+int yo_cpml_profile(void* h, int axis, int which, double* out_n) {
+  Base* b = static_cast<Base*>(h);
+  if (!b->committed || axis < 0 || axis > 2 || which < 0 || which > 5) return -1;
+  b->read_cpml_profile(axis, which, out_n);
   return 0;
 }
 

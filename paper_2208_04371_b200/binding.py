@@ -62,6 +62,8 @@ SYMBOLS = {
     "fdtd_reset": (C.c_int, [_vp]),
     "fdtd_step_count": (C.c_long, [_vp]),
     "fdtd_launch_count": (C.c_long, [_vp]),
+    "fdtd_graph_replays": (C.c_long, [_vp]),
+    "fdtd_device": (C.c_int, [_vp]),
     "fdtd_impl_name": (C.c_char_p, [_vp]),
     "fdtd_fused_kz": (C.c_int, [_vp]),
     "fdtd_set_z_interfaces": (C.c_int, [_vp, C.c_int, C.c_int]),
@@ -173,11 +175,34 @@ def fdtd_set_materials_indexed(h, idx, eps_r, sigma, mu_r=None):
         raise ValueError("eps_r, sigma, mu_r must be [n_entries, 3]")
     if isinstance(idx, np.ndarray):
         idx = np.ascontiguousarray(idx, dtype=np.uint8)
+    elif hasattr(idx, "element_size") and idx.element_size() != 1:
+        raise ValueError("material index tensor must be uint8")
     _check(h, lib().fdtd_set_materials_indexed(h, _ptr(idx), ne, e.ctypes.data_as(_dp), s.ctypes.data_as(_dp),
                                                 None if m is None else m.ctypes.data_as(_dp)))
 
 
-def fdtd_set_materials_full(h, eps_r, sigma, mu_r=None):
+def _check_cell_array(a, n_cells, itemsize, what):
+    """A per-cell array handed over by address must hold n_cells elements of the handle's precision (the C side sees a
+    bare pointer: a float64 array given to an fp32 handle would be reinterpreted silently)."""
+    if isinstance(a, np.ndarray):
+        size, isz, kind = a.size, a.dtype.itemsize, a.dtype.kind
+    else:
+        size, isz, kind = a.numel(), a.element_size(), ("f" if a.dtype.is_floating_point else "?")
+    if kind != "f" or isz != itemsize or size != n_cells:
+        raise ValueError(f"{what}: expected {n_cells} floating-point elements of {itemsize} bytes, got {size} x {isz} bytes ({kind})")
+
+
+def fdtd_set_materials_full(h, eps_r, sigma, mu_r=None, n_cells=None, precision=None):
+    """eps_r, sigma, mu_r: three arrays each (x, y, z component), host or device.  With n_cells and precision given (Solver
+    passes them) every array is checked for element count, element type and contiguity before its address is used."""
+    if n_cells is not None and precision is not None:
+        for name, xs in (("eps_r", eps_r), ("sigma", sigma), ("mu_r", mu_r)):
+            if xs is not None:
+                if len(xs) != 3:
+                    raise ValueError(f"{name}: three component arrays expected")
+                for x in xs:
+                    _check_cell_array(x, n_cells, 8 if precision == FDTD_F64 else 4, f"fdtd_set_materials_full {name}")
+
     def arr3(xs):
         return None if xs is None else (_vp * 3)(*[_ptr(x) for x in xs])
     _check(h, lib().fdtd_set_materials_full(h, arr3(eps_r), arr3(sigma), arr3(mu_r)))
@@ -225,6 +250,14 @@ def fdtd_step_count(h) -> int:
 
 def fdtd_launch_count(h) -> int:
     return int(lib().fdtd_launch_count(h))
+
+
+def fdtd_graph_replays(h) -> int:
+    return int(lib().fdtd_graph_replays(h))
+
+
+def fdtd_device(h) -> int:
+    return int(lib().fdtd_device(h))
 
 
 def fdtd_impl_name(h) -> str:

@@ -27,12 +27,13 @@ using namespace fdtd_b200;
 
 namespace {
 
-// R2: constants chosen so that c is exact.
-constexpr double kC0 = 299792458.0;
-constexpr double kPi = 3.14159265358979323846264338327950288;
-constexpr double kMu0 = 4.0e-7 * kPi;
-constexpr double kEps0 = 1.0 / (kMu0 * kC0 * kC0);
-constexpr double kEta0 = kMu0 * kC0;
+// R2: vacuum constants; c and mu0 are taken as exact, eps0 and eta0 follow from them.
+namespace phys {
+constexpr double c = 299792458.0;                      // m/s
+constexpr double mu0 = 4.0e-7 * 3.14159265358979323846264338327950288;   // H/m
+constexpr double eps0 = 1.0 / (mu0 * c * c);           // F/m
+constexpr double eta0 = mu0 * c;                       // ohm
+}  // namespace phys
 
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
@@ -56,6 +57,8 @@ struct fdtd {
   bool committed = false;
   long nstep = 0;
   long launches = 0;
+  long graph_replays = 0;             // cudaGraphLaunch calls since commit (0 on the NULL stream: no capture there)
+  int device = -1;                    // ordinal of the device that owns the workspace (set by fdtd_commit)
   std::string err;
   cudaStream_t stream = nullptr;
 
@@ -98,6 +101,27 @@ struct fdtd {
 };
 
 namespace {
+
+// Every ABI entry that touches the device runs with the handle's device current and puts the caller's device back: a
+// handle committed on cuda:1 works whatever device the calling thread has selected.
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  explicit DeviceGuard(int dev) {
+    if (dev < 0 || cudaGetDevice(&prev) != cudaSuccess) { cudaGetLastError(); return; }
+    if (prev != dev) switched = cudaSetDevice(dev) == cudaSuccess;
+  }
+  ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+  DeviceGuard(const DeviceGuard&) = delete;
+  DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
+
+// ordinal of the device a pointer lives on, or -1 for anything that is not device memory
+int device_of(const void* p) {
+  cudaPointerAttributes a;
+  if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return -1; }
+  return (a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged) ? a.device : -1;
+}
 
 bool is_device_ptr(const void* p) {
   cudaPointerAttributes a;
@@ -220,36 +244,38 @@ struct Solver : fdtd {
   int build_graph(cudaGraphExec_t* out);
 };
 
-// R4 (CPML, convolutional PML with recursive convolution): per axis, per slab coordinate s, at the E positions
-// (integer) and the H positions (half-integer):
-//   rho = depth into the layer in [0,1];  sigma = sigma_max rho^m;  kappa = 1 + (kappa_max-1) rho^m;
-//   alpha = alpha_max (1-rho)^m_a;  b = exp(-(sigma/kappa + alpha) dt/eps0);  c = sigma (b-1) / (kappa (sigma + kappa alpha))
+// R4 (CPML: stretched-coordinate PML, the convolution with the stretching function carried as a one-pole recursion).
+// The layer of `thick` cells on a face is graded by the distance t (in cells) of a sample from the layer's inner surface,
+// rho = t / thick:  sigma = sigma_max rho^m,  kappa = 1 + (kappa_max - 1) rho^m,  alpha = alpha_max (1 - rho)^m_a,
+//   b = exp(-(sigma/kappa + alpha) dt/eps0),  c = sigma (b - 1) / (kappa (sigma + kappa alpha)),  stored 1/kappa;
 //   sigma_max = sigma_factor (m+1) / (eta0 d_axis sqrt(eps_r_pml)).
+// Where the samples sit (include/fdtd.h "Grid"): on an axis the E-profile samples lie ON the cell boundaries and the
+// H-profile samples half a cell further up.  Slab coordinate s walks the low layer outside-in (cell s, s < lo), then the
+// high layer inside-out (cell n - hi + (s - lo)).  Hence, counting from the inner surface:
+//   low layer,  cell q = s:        E sample lo - q cells deep,  H sample lo - q - 1/2
+//   high layer, cell r = s - lo:   E sample r cells deep (r = 0 lies on the surface itself: no loss), H sample r + 1/2
 template <typename T>
 void Solver<T>::build_cpml_vectors() {
-  const double m = cpml[0], ma = cpml[1], kmax = cpml[2], amax = cpml[3], sfac = cpml[4], erp = cpml[5];
-  const int nn[3] = {nx, ny, nz};
-  const double dd[3] = {dx, dy, dz};
+  struct Grade { double b, c, inv_kappa; };
+  const double order = cpml[0], order_a = cpml[1], kappa_max = cpml[2], alpha_max = cpml[3];
+  const double cell[3] = {dx, dy, dz};
   for (int a = 0; a < 3; ++a) {
-    const int lo = npml[2 * a], hi = npml[2 * a + 1], n = nn[a], s_tot = lo + hi;
-    for (int v = 0; v < 6; ++v) h_vec[a * 6 + v].assign(s_tot > 0 ? s_tot : 1, T(v % 3 == 1 ? 0 : 1));
-    const double smax = sfac * (m + 1.0) / (kEta0 * dd[a] * std::sqrt(erp));
-    for (int s = 0; s < s_tot; ++s) {
-      const int u = s < lo ? s : n - hi + (s - lo);
-      for (int half = 0; half < 2; ++half) {
-        const double pos = u + 0.5 * half;
-        double rho = 0.0;
-        if (lo > 0 && pos < lo) rho = (lo - pos) / lo;
-        else if (hi > 0 && pos > n - hi) rho = (pos - (n - hi)) / hi;
-        const double g = std::pow(rho, m);
-        const double sg = smax * g, kp = 1.0 + (kmax - 1.0) * g, al = amax * std::pow(1.0 - rho, ma);
-        const double b = std::exp(-(sg / kp + al) * dt / kEps0);
-        const double c = sg == 0.0 ? 0.0 : sg * (b - 1.0) / (kp * (sg + kp * al));
-        h_vec[a * 6 + 3 * half + 0][s] = T(b);
-        h_vec[a * 6 + 3 * half + 1][s] = T(c);
-        h_vec[a * 6 + 3 * half + 2][s] = T(1.0 / kp);
-      }
-    }
+    const int lo = npml[2 * a], hi = npml[2 * a + 1];
+    const double sigma_max = cpml[4] * (order + 1.0) / (phys::eta0 * cell[a] * std::sqrt(cpml[5]));
+    auto grade = [&](double depth_cells, int thick) -> Grade {
+      const double rho = depth_cells / thick, shape = std::pow(rho, order);
+      const double sigma = sigma_max * shape, kappa = 1.0 + (kappa_max - 1.0) * shape;
+      const double alpha = alpha_max * std::pow(1.0 - rho, order_a);
+      const double b = std::exp(-(sigma / kappa + alpha) * dt / phys::eps0);
+      return Grade{b, sigma > 0.0 ? sigma * (b - 1.0) / (kappa * (sigma + kappa * alpha)) : 0.0, 1.0 / kappa};
+    };
+    std::vector<T>* vE = &h_vec[a * 6];      // bE cE kE
+    std::vector<T>* vH = &h_vec[a * 6 + 3];  // bH cH kH
+    const size_t len = lo + hi > 0 ? lo + hi : 1;
+    for (int v = 0; v < 3; ++v) { vE[v].assign(len, T(v == 1 ? 0 : 1)); vH[v].assign(len, T(v == 1 ? 0 : 1)); }
+    auto put = [](std::vector<T>* v, int s, const Grade& g) { v[0][s] = T(g.b); v[1][s] = T(g.c); v[2][s] = T(g.inv_kappa); };
+    for (int q = 0; q < lo; ++q) { put(vE, q, grade(lo - q, lo)); put(vH, q, grade(lo - q - 0.5, lo)); }
+    for (int r = 0; r < hi; ++r) { put(vE, lo + r, grade(r, hi)); put(vH, lo + r, grade(r + 0.5, hi)); }
   }
 }
 
@@ -261,6 +287,10 @@ int Solver<T>::commit(void* w, size_t bytes, void* st) {
   if (e != cudaSuccess || ndev == 0) { cudaGetLastError(); return fail(FDTD_ECUDA, "fdtd_commit: no CUDA device (there is no CPU fallback)"); }
   if (!w || ((uintptr_t)w & 255)) return fail(FDTD_EINVAL, "fdtd_commit: workspace must be a 256-byte aligned device pointer");
   if (!is_device_ptr(w)) return fail(FDTD_EINVAL, "fdtd_commit: workspace is not device memory");
+  device = device_of(w);
+  DeviceGuard on_device(device);
+  if (opt_impl == 2 && !slabs_fit())
+    return fail(FDTD_EINVAL, "fdtd_commit: FDTD_OPT_STEP_IMPL = 2 (fused) takes at most %d CPML cells per axis (lo + hi)", kMaxSlab);
   cv = layout();
   if (bytes < cv.total) return fail(FDTD_ENOMEM, "fdtd_commit: workspace of %zu bytes given, %zu needed", bytes, cv.total);
   ws = static_cast<char*>(w);
@@ -281,7 +311,7 @@ int Solver<T>::commit(void* w, size_t bytes, void* st) {
       if (has_mu) sp.Db[c] = reinterpret_cast<T*>(ws + cv.coef[6 + c]) + plane();
     }
   }
-  sp.db0 = T(dt / kMu0);
+  sp.db0 = T(dt / phys::mu0);
   sp.idx_ = T(1.0 / dx); sp.idy_ = T(1.0 / dy); sp.idz_ = T(1.0 / dz);
   for (int a = 0; a < 3; ++a) { sp.lo[a] = npml[2 * a]; sp.hi[a] = npml[2 * a + 1]; }
   build_cpml_vectors();
@@ -351,16 +381,16 @@ int Solver<T>::commit(void* w, size_t bytes, void* st) {
     for (int m = 0; m < kMaxTable; ++m)
       for (int c = 0; c < 3; ++c) {
         h_tab[8 * m + c] = T(1);
-        h_tab[8 * m + 3 + c] = T(dt / kEps0);
-        h_tab[kTabH + 4 * m + c] = T(dt / kMu0);
+        h_tab[8 * m + 3 + c] = T(dt / phys::eps0);
+        h_tab[kTabH + 4 * m + c] = T(dt / phys::mu0);
       }
     if ((e = cudaMemcpyAsync(ws + cv.tab, h_tab.data(), h_tab.size() * sizeof(T), cudaMemcpyHostToDevice, stream)) != cudaSuccess)
       return cuda_fail(e, "fdtd_commit: upload table");
   } else {
     for (int c = 0; c < 3; ++c) {
       k_fill<T><<<nb, 256, 0, stream>>>(reinterpret_cast<T*>(ws + cv.coef[c]), np, T(1));
-      k_fill<T><<<nb, 256, 0, stream>>>(reinterpret_cast<T*>(ws + cv.coef[3 + c]), np, T(dt / kEps0));
-      if (has_mu) k_fill<T><<<nb, 256, 0, stream>>>(reinterpret_cast<T*>(ws + cv.coef[6 + c]), np, T(dt / kMu0));
+      k_fill<T><<<nb, 256, 0, stream>>>(reinterpret_cast<T*>(ws + cv.coef[3 + c]), np, T(dt / phys::eps0));
+      if (has_mu) k_fill<T><<<nb, 256, 0, stream>>>(reinterpret_cast<T*>(ws + cv.coef[6 + c]), np, T(dt / phys::mu0));
     }
   }
   if ((e = cudaStreamSynchronize(stream)) != cudaSuccess) return cuda_fail(e, "fdtd_commit");
@@ -378,6 +408,7 @@ int Solver<T>::commit(void* w, size_t bytes, void* st) {
   committed = true;
   nstep = 0;
   launches = 0;
+  graph_replays = 0;
   return FDTD_OK;
 }
 
@@ -405,6 +436,7 @@ template <typename T>
 int Solver<T>::copy_field(int comp, void* user, bool to_user) {
   if (!committed) return fail(FDTD_ESTATE, "fields are available after fdtd_commit");
   if (comp < 0 || comp > 5 || !user) return fail(FDTD_EINVAL, "bad component or null pointer");
+  if (!to_user && mid_step) return fail(FDTD_ESTATE, "fdtd_write_fields: fdtd_step_end is pending (the field sets are half updated)");
   return copy3d(ws + (cur ? cv.field2[comp] : cv.field[comp]), sizeof(T), user, to_user);
 }
 
@@ -425,10 +457,10 @@ int Solver<T>::set_materials_indexed(const uint8_t* idx, int ne, const double* e
     for (int c = 0; c < 3; ++c) {
       const double er = eps[3 * s + c], sg = sig[3 * s + c], mr = mu ? mu[3 * s + c] : 1.0;
       double ca = 0.0, cb = 0.0;
-      if (!std::isinf(sg)) { const double a = sg * dt / (2.0 * kEps0 * er); ca = (1.0 - a) / (1.0 + a); cb = (dt / (kEps0 * er)) / (1.0 + a); }
+      if (!std::isinf(sg)) { const double a = sg * dt / (2.0 * phys::eps0 * er); ca = (1.0 - a) / (1.0 + a); cb = (dt / (phys::eps0 * er)) / (1.0 + a); }
       h_tab[8 * m + c] = T(ca);
       h_tab[8 * m + 3 + c] = T(cb);
-      h_tab[kTabH + 4 * m + c] = T(dt / (kMu0 * mr));
+      h_tab[kTabH + 4 * m + c] = T(dt / (phys::mu0 * mr));
     }
   }
   cudaError_t e = cudaMemcpyAsync(ws + cv.tab, h_tab.data(), h_tab.size() * sizeof(T), cudaMemcpyHostToDevice, stream);
@@ -458,15 +490,15 @@ int Solver<T>::set_materials_full(const void* const eps[3], const void* const si
     int r = copy3d(ca, sizeof(T), const_cast<void*>(eps[c]), false);
     if (r != FDTD_OK) return r;
     if ((r = copy3d(cb, sizeof(T), const_cast<void*>(sig[c]), false)) != FDTD_OK) return r;
-    k_coef_E<T><<<nb, 256, 0, stream>>>(ca, cb, np, dt, kEps0);
+    k_coef_E<T><<<nb, 256, 0, stream>>>(ca, cb, np, dt, phys::eps0);
     if (has_mu) {
       T* db = reinterpret_cast<T*>(ws + cv.coef[6 + c]);
       if (mu) {
         if ((e = cudaMemsetAsync(db, 0, np * sizeof(T), stream)) != cudaSuccess) return cuda_fail(e, "memset");
         if ((r = copy3d(db, sizeof(T), const_cast<void*>(mu[c]), false)) != FDTD_OK) return r;
-        k_coef_H<T><<<nb, 256, 0, stream>>>(db, np, dt, kMu0);
+        k_coef_H<T><<<nb, 256, 0, stream>>>(db, np, dt, phys::mu0);
       } else {
-        k_fill<T><<<nb, 256, 0, stream>>>(db, np, T(dt / kMu0));
+        k_fill<T><<<nb, 256, 0, stream>>>(db, np, T(dt / phys::mu0));
       }
     }
   }
@@ -812,6 +844,8 @@ template <typename T>
 int Solver<T>::profile_step(long n, double* ms) {
   if (!committed) return fail(FDTD_ESTATE, "fdtd_profile_step: call after fdtd_commit");
   if (n < 1 || !ms) return fail(FDTD_EINVAL, "fdtd_profile_step: n < 1 or null pointer");
+  if (mid_step || z_lo_open || z_hi_open)
+    return fail(FDTD_ESTATE, "fdtd_profile_step: a z slab advances with fdtd_step_begin / fdtd_step_end only");
   cudaEvent_t ev[5];
   for (int q = 0; q < 5; ++q)
     if (cudaEventCreate(&ev[q]) != cudaSuccess) return cuda_fail(cudaGetLastError(), "fdtd_profile_step: event");
@@ -883,6 +917,7 @@ int Solver<T>::step(long n) {
     while (left >= graph_steps) {
       const cudaError_t e = cudaGraphLaunch(*g, stream);
       if (e != cudaSuccess) return cuda_fail(e, "graph launch");
+      ++graph_replays;
       left -= graph_steps;
       launches += nodes * graph_steps;
     }
@@ -1011,7 +1046,7 @@ int fdtd_create(int nx, int ny, int nz, double dx, double dy, double dz, double 
   if (precision != FDTD_F32 && precision != FDTD_F64) return FDTD_EINVAL;
   if ((long long)nx * ny * nz > (1LL << 40) || nz > 65535 || ny > 65535 * 128) return FDTD_EINVAL;
   // the explicit scheme is run at a CFL number of 0.9; the limit itself:
-  const double dt_max = 1.0 / (kC0 * std::sqrt(1.0 / (dx * dx) + 1.0 / (dy * dy) + 1.0 / (dz * dz)));
+  const double dt_max = 1.0 / (phys::c * std::sqrt(1.0 / (dx * dx) + 1.0 / (dy * dy) + 1.0 / (dz * dz)));
   if (dt > dt_max) return FDTD_ECFL;
   fdtd* h = nullptr;
   if (precision == FDTD_F64) h = new (std::nothrow) Solver<double>();
@@ -1057,6 +1092,8 @@ int fdtd_add_port(fdtd_t* h, const fdtd_port* p, int* port_id) {
   if (p->has_source) {
     if (!(in(p->is, 0, h->nx) && in(p->sj0, 0, h->ny) && in(p->sj1, p->sj0, h->ny) && in(p->sk0, 0, h->nz) && p->sk1 > p->sk0 && p->sk1 <= h->nz))
       return h->fail(FDTD_ERANGE, "fdtd_add_port: source box outside the grid");
+    if (p->is == 0 || p->sj0 == 0)
+      return h->fail(FDTD_ERANGE, "fdtd_add_port: source box touches i = 0 or j = 0, where E_z is a PEC wall sample (R1)");
     if (p->waveform < FDTD_W_DGAUSS || p->waveform > FDTD_W_GSINE || !(p->sigma > 0))
       return h->fail(FDTD_EINVAL, "fdtd_add_port: bad waveform or sigma <= 0");
   }
@@ -1097,15 +1134,17 @@ int fdtd_set_option(fdtd_t* h, int option, long value) {
 
 size_t fdtd_workspace_bytes(const fdtd_t* h) { return h ? h->workspace_bytes() : 0; }
 int fdtd_commit(fdtd_t* h, void* ws, size_t bytes, void* stream) { return h ? h->commit(ws, bytes, stream) : FDTD_EINVAL; }
+// after commit: run on the handle's device, whatever device the caller has current
+#define FDTD_ON_DEVICE(h) if (!(h)) return FDTD_EINVAL; DeviceGuard fdtd_guard_((h)->device)
 int fdtd_set_materials_indexed(fdtd_t* h, const uint8_t* idx, int n_entries, const double* eps_r, const double* sigma, const double* mu_r) {
-  return h ? h->set_materials_indexed(idx, n_entries, eps_r, sigma, mu_r) : FDTD_EINVAL;
+  FDTD_ON_DEVICE(h); return h->set_materials_indexed(idx, n_entries, eps_r, sigma, mu_r);
 }
 int fdtd_set_materials_full(fdtd_t* h, const void* const eps_r[3], const void* const sigma[3], const void* const mu_r[3]) {
-  return h ? h->set_materials_full(eps_r, sigma, mu_r) : FDTD_EINVAL;
+  FDTD_ON_DEVICE(h); return h->set_materials_full(eps_r, sigma, mu_r);
 }
-int fdtd_step(fdtd_t* h, long n) { return h ? h->step(n) : FDTD_EINVAL; }
-int fdtd_step_begin(fdtd_t* h) { return h ? h->step_begin() : FDTD_EINVAL; }
-int fdtd_step_end(fdtd_t* h) { return h ? h->step_end() : FDTD_EINVAL; }
+int fdtd_step(fdtd_t* h, long n) { FDTD_ON_DEVICE(h); return h->step(n); }
+int fdtd_step_begin(fdtd_t* h) { FDTD_ON_DEVICE(h); return h->step_begin(); }
+int fdtd_step_end(fdtd_t* h) { FDTD_ON_DEVICE(h); return h->step_end(); }
 int fdtd_plane(fdtd_t* h, int comp, int k, void** dev_ptr, size_t* bytes) { return h ? h->plane_ptr(comp, k, dev_ptr, bytes) : FDTD_EINVAL; }
 int fdtd_set_z_interfaces(fdtd_t* h, int lo_open, int hi_open) {
   if (!h) return FDTD_EINVAL;
@@ -1114,17 +1153,23 @@ int fdtd_set_z_interfaces(fdtd_t* h, int lo_open, int hi_open) {
   h->z_hi_open = hi_open ? 1 : 0;
   return FDTD_OK;
 }
-int fdtd_profile_step(fdtd_t* h, long n, double ms_avg[4]) { return h ? h->profile_step(n, ms_avg) : FDTD_EINVAL; }
-int fdtd_read_fields(fdtd_t* h, int comp, void* dst) { return h ? h->read_field(comp, dst) : FDTD_EINVAL; }
-int fdtd_write_fields(fdtd_t* h, int comp, const void* src) { return h ? h->write_field(comp, src) : FDTD_EINVAL; }
-int fdtd_read_port_dft(fdtd_t* h, int port, double* V, double* I) { return h ? h->read_port_dft(port, V, I) : FDTD_EINVAL; }
-int fdtd_read_port_last(fdtd_t* h, int port, double* V, double* I) { return h ? h->read_port_last(port, V, I) : FDTD_EINVAL; }
-int fdtd_reset(fdtd_t* h) { return h ? h->reset() : FDTD_EINVAL; }
+int fdtd_profile_step(fdtd_t* h, long n, double ms_avg[4]) { FDTD_ON_DEVICE(h); return h->profile_step(n, ms_avg); }
+int fdtd_read_fields(fdtd_t* h, int comp, void* dst) { FDTD_ON_DEVICE(h); return h->read_field(comp, dst); }
+int fdtd_write_fields(fdtd_t* h, int comp, const void* src) { FDTD_ON_DEVICE(h); return h->write_field(comp, src); }
+int fdtd_read_port_dft(fdtd_t* h, int port, double* V, double* I) { FDTD_ON_DEVICE(h); return h->read_port_dft(port, V, I); }
+int fdtd_read_port_last(fdtd_t* h, int port, double* V, double* I) { FDTD_ON_DEVICE(h); return h->read_port_last(port, V, I); }
+int fdtd_reset(fdtd_t* h) { FDTD_ON_DEVICE(h); return h->reset(); }
 long fdtd_step_count(const fdtd_t* h) { return h ? h->nstep : -1; }
 long fdtd_launch_count(const fdtd_t* h) { return h ? h->launches : -1; }
+long fdtd_graph_replays(const fdtd_t* h) { return h ? h->graph_replays : -1; }
+int fdtd_device(const fdtd_t* h) { return h ? h->device : -1; }
 const char* fdtd_impl_name(const fdtd_t* h) { return h && h->committed ? h->impl_name() : ""; }
 int fdtd_fused_kz(const fdtd_t* h) { return h && h->committed ? h->fused_kz() : 0; }
 const char* fdtd_last_error(const fdtd_t* h) { return h ? h->err.c_str() : "null handle"; }
-void fdtd_destroy(fdtd_t* h) { delete h; }
+void fdtd_destroy(fdtd_t* h) {
+  if (!h) return;
+  DeviceGuard on_device(h->device);   // the graph executables are destroyed on their device
+  delete h;
+}
 
 }  // extern "C"

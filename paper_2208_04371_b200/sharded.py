@@ -93,18 +93,18 @@ class ShardedSolver:
         if missing:
             raise ValueError(f"ports {missing} are cut by a slab interface: choose another number of slabs")
 
-    def _copy(self, src, dst):
+    def _copy(self, src_solver, src, dst_solver, dst):
+        """One plane from src_solver's workspace to dst_solver's, ordered after the producer's stream; the producer's next
+        kernel waits for the copy (it will overwrite the plane two steps later)."""
         import torch
-        if src.device == dst.device:
+        done = torch.cuda.Event()
+        done.record(src_solver.stream)
+        dst_solver.stream.wait_event(done)
+        with torch.cuda.device(dst_solver.device), torch.cuda.stream(dst_solver.stream):
             dst.copy_(src, non_blocking=True)
-        else:
-            # peer copy on the destination's stream after the source's work is done
-            ev = torch.cuda.Event()
-            with torch.cuda.device(src.device):
-                ev.record(torch.cuda.current_stream(src.device))
-            with torch.cuda.device(dst.device):
-                torch.cuda.current_stream(dst.device).wait_event(ev)
-                dst.copy_(src, non_blocking=True)
+        copied = torch.cuda.Event()
+        copied.record(dst_solver.stream)
+        src_solver.stream.wait_event(copied)
 
     def step(self, n=1):
         S = self.solvers
@@ -117,12 +117,12 @@ class ShardedSolver:
             for lo, up in zip(S[:-1], S[1:]):
                 top = lo.shape[0] - 1
                 for c in (HX, HY):
-                    self._copy(lo.plane(c, top), up.plane(c, -1))
+                    self._copy(lo, lo.plane(c, top), up, up.plane(c, -1))
             for s in S:
                 s.step_end()
             for lo, up in zip(S[:-1], S[1:]):
                 for c in (EX, EY):
-                    self._copy(up.plane(c, 0), lo.plane(c, lo.shape[0]))
+                    self._copy(up, up.plane(c, 0), lo, lo.plane(c, lo.shape[0]))
 
     def read_fields(self, comp):
         import torch
@@ -182,8 +182,14 @@ class DistributedSlab:
                 if self.rank < self.world - 1:
                     ops.append(d.P2POp(d.irecv, s.plane(c, nzl), self.rank + 1))
         if ops:
+            st = getattr(s, "stream", None)          # a CUDA solver runs on its own stream; the collectives on the current one
+            if st is not None:
+                import torch
+                torch.cuda.current_stream(s.device).wait_stream(st)
             for r in d.batch_isend_irecv(ops):
                 r.wait()
+            if st is not None:
+                st.wait_stream(torch.cuda.current_stream(s.device))
 
     def step(self, n=1):
         if self.world == 1:

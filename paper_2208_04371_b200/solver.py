@@ -1,7 +1,10 @@
 """`Solver`: a handle plus its torch workspace -- a convenience wrapper over the C-ABI functions of binding.py.
 
-Nothing here computes: setup arguments are marshalled to the library, the workspace is one torch uint8 CUDA tensor,
-the stream is torch's current stream.  Fields come back as torch CUDA tensors shaped [nz, ny, nx] (x fastest).
+Nothing here computes: setup arguments are marshalled to the library, the workspace is one torch uint8 CUDA tensor and
+the solver owns a torch.cuda.Stream of its device (a real stream: fdtd_step replays captured CUDA graphs on it, which the
+NULL stream cannot do).  Tensors that cross the boundary are ordered against torch's current stream: device inputs are
+waited for before the library reads them, device outputs are handed to the current stream after the library wrote them.
+Fields come back as torch CUDA tensors shaped [nz, ny, nx] (x fastest).
 """
 from __future__ import annotations
 
@@ -51,20 +54,49 @@ class Solver:
     def workspace_bytes(self):
         return B.fdtd_workspace_bytes(self.h)
 
-    def commit(self, device="cuda:0"):
+    def commit(self, device="cuda:0", stream=None):
+        """Allocate the workspace on `device` and commit.  `stream`: a torch.cuda.Stream of that device to run on (default:
+        a new one owned by this solver)."""
         torch = _torch()
         self.device = torch.device(device)
+        if self.device.index is None:
+            self.device = torch.device("cuda", torch.cuda.current_device())
         with torch.cuda.device(self.device):
             self.workspace = torch.empty(self.workspace_bytes(), dtype=torch.uint8, device=self.device)
-            self.stream = torch.cuda.current_stream(self.device)
+            self.stream = stream if stream is not None else torch.cuda.Stream(self.device)
+            self.stream.wait_stream(torch.cuda.current_stream(self.device))   # the allocator may still be clearing the block
             B.fdtd_commit(self.h, self.workspace, self.stream.cuda_stream)
+
+    # ---- ordering against torch's current stream for tensors that cross the boundary -------------------------------
+    def _before_read_of(self, *tensors):
+        """The library is about to read these (device) tensors on its stream: wait for their producers."""
+        torch = _torch()
+        if any(hasattr(t, "is_cuda") and t.is_cuda for t in tensors):
+            self.stream.wait_stream(torch.cuda.current_stream(self.device))
+
+    def _after_write_of(self, *tensors):
+        """The library has enqueued writes to these (device) tensors: later work on the current stream waits for them."""
+        torch = _torch()
+        if any(hasattr(t, "is_cuda") and t.is_cuda for t in tensors):
+            torch.cuda.current_stream(self.device).wait_stream(self.stream)
+
+    def _check_field_array(self, a, what):
+        nz, ny, nx = self.shape
+        B._check_cell_array(a, nx * ny * nz, 8 if self.precision == B.FDTD_F64 else 4, what)
 
     # ---- after commit ------------------------------------------------------------------------------------------
     def set_materials_indexed(self, idx, eps_r, sigma, mu_r=None):
+        nz, ny, nx = self.shape
+        n = idx.size if isinstance(idx, np.ndarray) else idx.numel()
+        if n != nx * ny * nz:
+            raise ValueError(f"material index: {nx * ny * nz} cells expected, got {n}")
+        self._before_read_of(idx)
         B.fdtd_set_materials_indexed(self.h, idx, eps_r, sigma, mu_r)
 
     def set_materials_full(self, eps_r, sigma, mu_r=None):
-        B.fdtd_set_materials_full(self.h, eps_r, sigma, mu_r)
+        nz, ny, nx = self.shape
+        self._before_read_of(*eps_r, *sigma, *(mu_r or ()))
+        B.fdtd_set_materials_full(self.h, eps_r, sigma, mu_r, n_cells=nx * ny * nz, precision=self.precision)
 
     def step(self, n=1):
         B.fdtd_step(self.h, n)
@@ -80,10 +112,15 @@ class Solver:
     def read_fields(self, comp, out=None):
         if out is None:
             out = _torch().empty(self.shape, dtype=self.dtype, device=self.device)
+        self._check_field_array(out, "read_fields")
+        self._before_read_of(out)                   # `out` may still be in use by work queued on the current stream
         B.fdtd_read_fields(self.h, comp, out)
+        self._after_write_of(out)
         return out
 
     def write_fields(self, comp, src):
+        self._check_field_array(src, "write_fields")
+        self._before_read_of(src)
         B.fdtd_write_fields(self.h, comp, src)
 
     def read_port_dft(self, port):
@@ -102,6 +139,10 @@ class Solver:
     @property
     def launch_count(self):
         return B.fdtd_launch_count(self.h)
+
+    @property
+    def graph_replays(self):
+        return B.fdtd_graph_replays(self.h)
 
     @property
     def impl_name(self):

@@ -69,13 +69,17 @@ class NumpyYee:
         for ai, a in enumerate("xyz"):
             n, lo, hi = self.n[a], w["pml"][2 * ai], w["pml"][2 * ai + 1]
             smax = sfac * (mm + 1) / (ETA0 * self.d[a] * np.sqrt(erp))
-            for half, tag in ((0.0, "E"), (0.5, "H")):
-                pos = np.arange(n) + half
+            # depth into the layer from PHYSICAL coordinates: the inner CPML surfaces are the planes x = lo*d and
+            # x = (n-hi)*d; an E sample sits at x = u*d, an H sample at x = (u+1/2)*d; rho = distance beyond the
+            # surface / layer thickness (deliberately not the index rule the oracle and the library use)
+            for tag, x in (("E", np.arange(n) * self.d[a]), ("H", (np.arange(n) + 0.5) * self.d[a])):
+                x_lo, x_hi = lo * self.d[a], (n - hi) * self.d[a]
                 rho = np.zeros(n)
                 if lo:
-                    rho = np.where(pos < lo, (lo - pos) / lo, rho)
+                    rho = np.maximum(rho, (x_lo - x) / (lo * self.d[a]))
                 if hi:
-                    rho = np.where(pos > n - hi, (pos - (n - hi)) / hi, rho)
+                    rho = np.maximum(rho, (x - x_hi) / (hi * self.d[a]))
+                rho = np.clip(rho, 0.0, None)
                 inslab = (np.arange(n) < lo) | (np.arange(n) >= n - hi)
                 sg = smax * rho**mm
                 kp = 1 + (kmax - 1) * rho**mm
@@ -98,6 +102,10 @@ class NumpyYee:
         self.freqs = np.asarray(w.get("freqs", []), dtype=float)
         self.Vhat = np.zeros((len(w["ports"]), self.freqs.size), dtype=complex)
         self.Ihat = np.zeros_like(self.Vhat)
+        # R13: running maxima over space AND time, kept as two separate scalars, plus the per-step history
+        self.emax = 0.0
+        self.hmax = 0.0
+        self.emax_hist, self.hmax_hist = [], []
 
     def _curl_term(self, psi, key, field, diff, tag):
         """derivative of `field` along axis key[1], CPML-stretched; updates psi[key] in place."""
@@ -135,6 +143,11 @@ class NumpyYee:
                 self.Vhat[q] += V * np.exp(-2j * np.pi * self.freqs * tE) * self.dt
                 self.Ihat[q] += I * np.exp(-2j * np.pi * self.freqs * tH) * self.dt
                 self.lastV, self.lastI = V, I
+            e_now = max(float(np.abs(E[c]).max()) for c in "xyz")     # E^{n+1} with the source added
+            h_now = max(float(np.abs(H[c]).max()) for c in "xyz")     # H^{n+1/2}
+            self.emax_hist.append(e_now)
+            self.hmax_hist.append(h_now)
+            self.emax, self.hmax = max(self.emax, e_now), max(self.hmax, h_now)
             self.nstep += 1
 
     def field(self, comp):

@@ -71,6 +71,11 @@ def test_setup_checks_and_lifecycle_without_gpu():
         with pytest.raises(B.FdtdError) as e:
             B.fdtd_add_port(h, bad)
         assert e.value.code == B.FDTD_ERANGE
+        for wall in (dict(port, sj0=0), {**port, "is": 0}):      # E_z on i = 0 / j = 0 is a PEC wall sample (R1)
+            with pytest.raises(B.FdtdError) as e:
+                B.fdtd_add_port(h, wall)
+            assert e.value.code == B.FDTD_ERANGE
+        assert B.fdtd_device(h) == -1 and B.fdtd_graph_replays(h) == 0
         B.fdtd_set_dft(h, np.linspace(1e9, 5e11, 128))
         B.fdtd_set_material_mode(h, B.FDTD_MAT_FULL, True)
         assert B.fdtd_workspace_bytes(h) > small            # nine coefficient arrays instead of an index
@@ -109,3 +114,16 @@ def test_workspace_size_is_the_documented_layout():
         got = B.fdtd_workspace_bytes(h)
         B.fdtd_destroy(h)
         assert expect <= got <= expect * 1.01 + (1 << 20), (impl, expect, got)
+
+
+def test_binding_refuses_material_arrays_of_the_wrong_type_or_size():
+    """The C side sees bare pointers, so the binding checks element type, count and contiguity first (no GPU needed:
+    the check runs before the library is called)."""
+    n = 6 * 5 * 4
+    ok = [np.ones(n, dtype=np.float32)] * 3
+    for bad in ([np.ones(n, dtype=np.float64)] * 3, [np.ones(n - 1, dtype=np.float32)] * 3, [np.ones(n, dtype=np.int32)] * 3,
+                ok[:2]):
+        with pytest.raises(ValueError):
+            B.fdtd_set_materials_full(None, bad, ok, n_cells=n, precision=B.FDTD_F32)
+    with pytest.raises(ValueError):
+        B.fdtd_set_materials_full(None, ok, [np.ones((n, 2), dtype=np.float32)[:, 0]] * 3, n_cells=n, precision=B.FDTD_F32)

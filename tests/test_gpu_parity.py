@@ -172,20 +172,95 @@ def test_C3_small_scale_indexed_six_face_cpml(impl):
 
 @pytest.mark.parametrize("impl", IMPLS)
 def test_graph_replay_equals_plain_launches(impl):
-    """fdtd_step(n) through CUDA-graph replay (unroll 4 + remainder) is bit-identical to one launch per step."""
+    """fdtd_step(n) through CUDA-graph replay (unroll 4 + remainder) is bit-identical to one launch per step, and the
+    graph really is what ran: Solver owns a real stream, so fdtd_step(27) issues 6 replays of 4 steps + 3 plain steps
+    (the persistent kernel, impl 3, has no graph: one cooperative launch covers the whole call)."""
     w = W.random_box(11, nx=40, ny=22, nz=18, steps=27, precision=FDTD_F32)
     out = []
     for graph in (0, 1):
         s = Solver.from_workload(w, options={FDTD_OPT_STEP_IMPL: impl, FDTD_OPT_USE_GRAPH: graph, FDTD_OPT_GRAPH_UNROLL: 4})
+        assert s.stream.cuda_stream != 0
         if graph:
             s.step(27)
         else:
             for _ in range(27):
                 s.step(1)
         assert s.step_count == 27
+        assert s.graph_replays == (6 if graph and impl != 3 else 0), (impl, graph, s.graph_replays)
         out.append([s.read_fields(c).cpu().numpy() for c in range(6)] + list(s.read_port_dft(0)))
+        s.destroy()
     for a, b in zip(*out):
         assert np.array_equal(a, b)
+
+
+def test_null_stream_runs_plain_launches_with_the_same_result():
+    """include/fdtd.h: on the NULL (legacy default) stream no graph can be captured; fdtd_step falls back to plain
+    launches there and says so through fdtd_graph_replays."""
+    import torch
+    w = W.random_box(11, nx=40, ny=22, nz=18, steps=27, precision=FDTD_F32)
+    out = []
+    for null in (False, True):
+        s = Solver(w["nx"], w["ny"], w["nz"], w["dx"], w["dy"], w["dz"], w["dt"], FDTD_F32)
+        s.set_boundary(w["pml"], w["cpml"])
+        for p in w["ports"]:
+            s.add_port(p)
+        s.set_dft(w["freqs"])
+        s.set_option(FDTD_OPT_STEP_IMPL, 1)
+        s.set_option(FDTD_OPT_GRAPH_UNROLL, 4)
+        s.commit("cuda:0", stream=torch.cuda.default_stream() if null else None)
+        m = w["materials"]
+        s.set_materials_indexed(m["idx"], m["eps_r"], m["sigma"], m.get("mu_r"))
+        s.step(27)
+        assert (s.stream.cuda_stream == 0) == null and (s.graph_replays == 0) == null
+        out.append([s.read_fields(c).cpu().numpy() for c in range(6)])
+        s.destroy()
+    for a, b in zip(*out):
+        assert np.array_equal(a, b)
+
+
+def test_handle_runs_on_its_own_device_whatever_device_is_current():
+    """the library records the device of its workspace at commit and makes it current inside every call.  With
+    two GPUs the handle lives on cuda:1 while cuda:0 is current; with one GPU the test checks the recorded ordinal and
+    that the caller's current device is left alone."""
+    import torch
+    from paper_2208_04371_b200 import binding as B
+    dev = torch.cuda.device_count() - 1
+    w = W.random_box(13, steps=12, precision=FDTD_F32)
+    o = YeeOracle.from_workload(w, track_max=True)
+    o.step(12)
+    torch.cuda.set_device(0)
+    s = Solver.from_workload(w, device=f"cuda:{dev}", options={FDTD_OPT_STEP_IMPL: 1})
+    assert B.fdtd_device(s.h) == dev and torch.cuda.current_device() == 0
+    s.step(12)
+    assert torch.cuda.current_device() == 0
+    emax, hmax = o.running_max()
+    for c in range(6):
+        g = s.read_fields(c).cpu().numpy().astype(np.float64)
+        assert np.abs(g - o.read_field(c)).max() <= 1e-4 * (emax if c < 3 else hmax)
+    s.destroy()
+
+
+def test_state_errors_of_z_slabs_and_oversized_cpml():
+    """profile_step on a z slab and write_fields between step_begin and step_end are refused; the fused step
+    asked for by name with more CPML cells than its shared memory holds is an error, not a silent two-pass run."""
+    w = W.random_box(14, nx=40, ny=22, nz=18, steps=4, precision=FDTD_F32, pml=(3, 3, 3, 3, 0, 0))
+    s = Solver.from_workload(w, options={FDTD_OPT_STEP_IMPL: 2}, z_open=(False, True))
+    with pytest.raises(FdtdError) as e:
+        s.profile_step(1)
+    assert e.value.code == -3
+    s.step_begin()
+    with pytest.raises(FdtdError) as e:
+        s.write_fields(0, s.read_fields(0))
+    assert e.value.code == -3
+    s.step_end()
+    s.write_fields(0, s.read_fields(0))
+    s.destroy()
+    big = Solver(200, 16, 16, 1e-9, 1e-9, 1e-9, 1e-18, FDTD_F32)
+    big.set_boundary([40, 40, 0, 0, 0, 0])
+    big.set_option(FDTD_OPT_STEP_IMPL, 2)
+    with pytest.raises(FdtdError) as e:
+        big.commit()
+    assert e.value.code == -1
 
 
 def test_reset_and_device_pointers():

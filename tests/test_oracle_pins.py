@@ -5,6 +5,7 @@ mistake anywhere in oracle/yee_oracle.cpp (dropped term, wrong sign or index, tr
 wrong time stamp) fails at least one of them.
 """
 import math
+from fractions import Fraction
 import os
 
 import numpy as np
@@ -401,6 +402,9 @@ def test_P10_oracle_equals_numpy_formulation(seed, indexed, with_mu, pml):
     r.step(40)
     emax, hmax = o.running_max()
     assert emax > 0 and hmax > 0
+    # R13: the running maxima are max|E| and max|H| over space and time, two separate scalars (the numpy formulation
+    # tracks them itself; fields agree to 1e-12, so do their maxima)
+    assert abs(emax / r.emax - 1) < 1e-12 and abs(hmax / r.hmax - 1) < 1e-12
     for c in range(6):
         scale = emax if c < 3 else hmax
         assert np.abs(o.read_field(c) - r.field(c)).max() / scale < 1e-12, c
@@ -410,6 +414,116 @@ def test_P10_oracle_equals_numpy_formulation(seed, indexed, with_mu, pml):
         assert np.abs(I - r.Ihat[p]).max() <= 1e-12 * np.abs(r.Ihat).max()
     if any(pml):
         assert o.psi_norms().max() > 0
+
+
+# ------------------------------------------------------------------------------------------------
+# R13  the running maximum (denominator of every field tolerance of the GPU parity tests)
+# ------------------------------------------------------------------------------------------------
+def test_R13_running_max_is_separate_for_E_and_H_over_space_and_time_and_resets_at_commit():
+    """A pulse in a lossy box peaks mid-run and decays: "the maximum of the last step", "one maximum over E and H
+    together", "a sum" and "never reset at commit" all fail one of the asserts below.  The expected values come from
+    the independent numpy formulation's own per-step history."""
+    w = W.random_box(7, indexed=False, with_mu=False, pml=(3, 3, 3, 3, 0, 3), steps=160, pec_frac=0.0)
+    for c in range(3):                                                   # lossy everywhere: the pulse dies out
+        w["materials"]["sigma"][c] = np.maximum(np.where(np.isinf(w["materials"]["sigma"][c]), 0.0,
+                                                         w["materials"]["sigma"][c]), 3e5)
+    o = YeeOracle.from_workload(w, track_max=True)
+    r = NumpyYee(w)
+    o.step(160); r.step(160)
+    emax, hmax = o.running_max()
+    eh, hh = np.array(r.emax_hist), np.array(r.hmax_hist)
+    # the case discriminates: the peak lies mid-run, the last step is far below it, |E| and |H| differ by orders
+    assert 5 < eh.argmax() < 100 and eh[-1] < 0.2 * eh.max() and hh[-1] < 0.2 * hh.max()
+    assert eh.max() > 50 * hh.max()
+    assert abs(emax / eh.max() - 1) < 1e-12                             # max over time of max over space of |E| ...
+    assert abs(hmax / hh.max() - 1) < 1e-12                             # ... and of |H|, separately
+    # and it is the maximum over all three components of the family, not of one of them
+    per_comp = [max(np.abs(r.field(c)).max() for c in (0, 1, 2)), max(np.abs(r.field(c)).max() for c in (3, 4, 5))]
+    assert per_comp[0] <= emax and per_comp[1] <= hmax
+    # without tracking the maxima stay zero (the GPU tests would divide by zero, loudly)
+    o2 = YeeOracle.from_workload(w, track_max=False)
+    o2.step(5)
+    assert o2.running_max() == (0.0, 0.0)
+    # a second commit zeroes the maxima with the rest of the state
+    o.commit()
+    assert o.running_max() == (0.0, 0.0) and o.step_count == 0
+    o.step(4)
+    e4, h4 = o.running_max()
+    assert abs(e4 / eh[:4].max() - 1) < 1e-12 and abs(h4 / hh[:4].max() - 1) < 1e-12
+
+
+def test_R13_running_max_from_an_initial_state_whose_E_peak_is_at_step_zero():
+    """An initial E_z column profile (written through write_field, source off) that only decays afterwards: the E
+    maximum is the one of the first steps, the H maximum is reached later, and in SI units |H| is two orders below
+    |E|, so one maximum over E and H together (or H scaled by eta0) shows up here.  Expected values: the numpy
+    formulation started from the same state."""
+    w = W.random_box(8, indexed=False, with_mu=False, pml=(0, 0, 0, 0, 0, 0), steps=6, pec_frac=0.0)
+    for c in range(3):
+        w["materials"]["sigma"][c] = np.zeros_like(w["materials"]["sigma"][c])
+        w["materials"]["eps_r"][c] = np.ones_like(w["materials"]["eps_r"][c])
+    w["ports"][0]["amp"] = 0.0
+    nz, ny, nx = w["nz"], w["ny"], w["nx"]
+    ez0 = np.zeros((nz, ny, nx))
+    ez0[:, 1:, 1:] = (1.0 + np.arange(nz))[:, None, None]                # uniform in x, y; rows i = 0, j = 0 are walls
+    o = YeeOracle.from_workload(w, track_max=True)
+    r = NumpyYee(w)
+    o.write_field(EZ, ez0)
+    r.E["z"] = ez0.copy()
+    o.step(6); r.step(6)
+    emax, hmax = o.running_max()
+    assert abs(emax / r.emax - 1) < 1e-12 and abs(hmax / r.hmax - 1) < 1e-12
+    assert emax > 0.9 * nz and 0 < 100 * hmax < emax
+    assert np.argmax(r.emax_hist) != np.argmax(r.hmax_hist)              # the two maxima are reached at different steps
+
+
+# ------------------------------------------------------------------------------------------------
+# R4  CPML sample POSITIONS (integer E positions, half-integer H positions, low and high face)
+# ------------------------------------------------------------------------------------------------
+def _read_cpml_golden(golden_dir):
+    rows = {}
+    for line in open(os.path.join(golden_dir, "cpml_profile_lo4_hi3.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        u, rho_e, ce, rho_h, ch = [x.strip() for x in line.split("|")]
+        rows[int(u)] = (Fraction(rho_e), [float(x) for x in ce.split()], Fraction(rho_h), [float(x) for x in ch.split()])
+    return rows
+
+
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_R4_cpml_profile_positions_against_hand_written_fixture(golden_dir, axis):
+    """tests/golden/cpml_profile_lo4_hi3.txt lists, for n = 12, lo = 4, hi = 3, the depth rho at every E index and every
+    H index (typed by hand from R4's two sentences) and b, c, 1/kappa from the closed forms.  A half-cell offset, a
+    swapped E/H profile or a mirrored high side changes rho at every slab index."""
+    rows = _read_cpml_golden(golden_dir)
+    d = 5e-9
+    dt = d / (2.0 * C0)
+    n = [6, 6, 6]
+    n[axis] = 12
+    pml = [0] * 6
+    pml[2 * axis], pml[2 * axis + 1] = 4, 3
+    o = YeeOracle(n[0], n[1], n[2], d, d, d, dt)
+    o.set_boundary(pml, [3.0, 1.0, 5.0, 0.05, 0.8, 4.0])
+    o.commit()
+    prof = o.cpml_profile(axis)
+    assert sorted(rows) == [0, 1, 2, 3, 9, 10, 11]
+    for u, (rho_e, ce, rho_h, ch) in rows.items():
+        for name, ref in zip(("bE", "cE", "ikE"), ce):
+            assert abs(prof[name][u] - ref) <= 1e-14, (name, u)
+        for name, ref in zip(("bH", "cH", "ikH"), ch):
+            assert abs(prof[name][u] - ref) <= 1e-14, (name, u)
+    for u in range(4, 9):                                                # interior: no absorption, no stretching
+        for name, ref in (("bE", 1), ("cE", 0), ("ikE", 1), ("bH", 1), ("cH", 0), ("ikH", 1)):
+            assert prof[name][u] == ref
+    # the other axes have no layer at all
+    for a in range(3):
+        if a != axis:
+            q = o.cpml_profile(a)
+            assert (q["cE"] == 0).all() and (q["cH"] == 0).all() and (q["ikE"] == 1).all()
+    # the fixture's own depth table is monotone towards the walls and E/H interleave by half a cell
+    assert [rows[u][0] for u in (0, 1, 2, 3)] == [Fraction(4 - u, 4) for u in (0, 1, 2, 3)]
+    assert [rows[u][2] for u in (0, 1, 2, 3)] == [Fraction(7 - 2 * u, 8) for u in (0, 1, 2, 3)]
+    assert [rows[u][0] for u in (9, 10, 11)] == [Fraction(0), Fraction(1, 3), Fraction(2, 3)]
+    assert [rows[u][2] for u in (9, 10, 11)] == [Fraction(1, 6), Fraction(1, 2), Fraction(5, 6)]
 
 
 # ------------------------------------------------------------------------------------------------
