@@ -12,13 +12,20 @@ N counts the CPML cells.  Prints ONE JSON line (rank 0).
                 host->device (fdtd_set_materials_indexed), fdtd_reset, K steps, every port's DFT device->host
   roofline      dominant kernel: algorithmic bytes per launch / its average duration from CUDA events
                 (fdtd_profile_step) vs MEASURED_PEAKS.json hbm_gbs
-  cpu_baseline  the fp64 oracle, as it stands, on the host cores, on a bounded crop of the same workload (rank 0, N=1)
+  sustained     BASELINE.json's "2000 steps timed" on C3, with its own clock samples, whatever --steps says (c3 only;
+                --sustained-steps 0 switches it off)
+  cpu_baseline  the fp64 oracle, as it stands, on the host cores (all cores, and one thread), on the z-cropped
+                1536x768x96 grid of the same generator (SURVEY 8(d) "Oracle timing"; full C3 needs ~150 GB of host
+                arrays in fp64), rank 0, N=1
   --impl reference   times the oracle instead (there is no installable reference implementation: /root/reference holds
                 a paper only); rank 0 alone works.
 
-Multi-GPU: the path does not shard in this build ("replicas only"): every rank runs an independent replica
-of the workload on its own GPU, no data-path collective; torch.distributed is used for the barrier and the max of the
-times only.
+Multi-GPU.  north_star: one GPU, no sharding => the default mode is "replicas": every rank runs an
+independent replica of the workload on its own GPU, no data-path collective; torch.distributed is used for the barrier
+and the max of the times only.  `--mode sharded` is the z-slab decomposition of SURVEY 8(f) f4 (Table I:
+weak scaling at 600^3 cells per GPU): one slab per rank, halo planes pushed into the neighbour's memory by the kernels.
+With --gpus N > 1 and no WORLD_SIZE in the environment bench.py starts the N ranks itself (torchrun, 127.0.0.1) and the
+line still comes from rank 0 with "n_gpus": N.
 """
 from __future__ import annotations
 
@@ -40,12 +47,34 @@ METRIC = "Mcell-updates/s per Yee E+H step"
 UNIT = "Mcell-updates/s"
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch, from the ncu captures summarised under profiles/
-NCU_TRAFFIC = {
-    ("c3", "k_step_fused", 32): (47.98e9, "profiles/r01_final.md, group dispatch (24.78 GB read + 23.21 GB written)"),
-    ("c3", "k_update_E", 32): (35.24e9, "profiles/r01_twopass.md"),
-    ("c3", "k_update_H", 32): (34.39e9, "profiles/r01_twopass.md"),
-}
+def csrc_hash():
+    """sha256 (first 16 hex digits) over the kernel sources, in name order: ties an ncu capture to the build it was taken from."""
+    import glob
+    import hashlib
+    h = hashlib.sha256()
+    for f in sorted(glob.glob(os.path.join(ROOT, "paper_2208_04371_b200", "csrc", "*"))):
+        h.update(os.path.basename(f).encode())
+        h.update(open(f, "rb").read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(workload_name, kernel, dtype, kz):
+    """dram__bytes_read.sum + dram__bytes_write.sum of ONE launch from the `ncu --set full` capture recorded in
+    profiles/traffic.json for exactly this (workload, kernel, dtype, kz, kernel-source hash); (None, why) otherwise."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    if not os.path.exists(path):
+        return None, "no profiles/traffic.json"
+    sha = csrc_hash()
+    near = None
+    for e in json.load(open(path))["captures"]:
+        if (e["workload"], e["kernel"], e["dtype"]) == (workload_name, kernel, dtype):
+            if e["kz"] == kz and e["csrc_sha16"] == sha:
+                return float(e["dram_bytes"]), e["source"]
+            near = e
+    if near is not None:
+        return None, (f"capture in profiles/traffic.json is for kz={near['kz']}, csrc {near['csrc_sha16']} "
+                      f"({near['dram_bytes'] / 1e9:.2f} GB); this run: kz={kz}, csrc {sha}")
+    return None, "no capture of this workload / kernel in profiles/traffic.json"
 
 
 def workload(name, steps):
@@ -125,7 +154,26 @@ class ClockSampler:
 # --------------------------------------------------------------------------------------------------------------------
 # the oracle on the host cores (cpu_baseline leg and --impl reference): bounded sample of the same workload
 # --------------------------------------------------------------------------------------------------------------------
-CPU_SAMPLE_LADDER = [(512, 384, 192), (384, 256, 160), (256, 192, 128), (192, 128, 96), (128, 96, 80)]
+# z-cropped C3 first (full-length rows and planes, 96 of the 768 planes); the smaller crops are fall-backs for
+# hosts without the ~30 GB the fp64 oracle needs for it, and for the --impl reference arm's wall-clock bound
+CPU_SAMPLE_LADDER = [(1536, 768, 96), (512, 384, 192), (384, 256, 160), (256, 192, 128), (192, 128, 96), (128, 96, 80)]
+ORACLE_BYTES_PER_CELL = 8 * (6 + 9 + 6) + 8 * 6 + 2      # fields, coefficients, eps/sigma, the gather's temporaries, index
+
+
+def _host_mem_available():
+    try:
+        for line in open("/proc/meminfo"):
+            if line.startswith("MemAvailable:"):
+                return int(line.split()[1]) * 1024
+    except OSError:
+        pass
+    return 0
+
+
+def _fits_host(shape):
+    need = shape[0] * shape[1] * shape[2] * ORACLE_BYTES_PER_CELL
+    avail = _host_mem_available()
+    return avail == 0 or need * 1.3 < avail
 
 
 def _oracle_on(shape):
@@ -136,12 +184,20 @@ def _oracle_on(shape):
     return YeeOracle.from_workload(w), w["nx"] * w["ny"] * w["nz"]
 
 
-def oracle_sample(budget_s=15.0, steps=None, warmup=1, wall_s=150.0):
-    """Time the fp64 oracle as it stands on a bounded crop of C3.  With steps=None the step count fills budget_s on
-    the largest crop; with steps given (the --impl reference arm) the crop is the largest of CPU_SAMPLE_LADDER whose
-    steps+warmup steps are expected to fit in wall_s.  Returns (Mcell/s, s/step, steps, cores, description, shape)."""
-    from oracle.yee import num_threads
-    shape = CPU_SAMPLE_LADDER[0]
+def _describe(shape, steps):
+    return (f"fp64 oracle (g++ -O2 -fopenmp), C3 generator on {shape[0]}x{shape[1]}x{shape[2]} cells"
+            f"{' (C3 cropped in z)' if shape[:2] == (1536, 768) else ' (bounded crop of C3)'}, 64-entry indexed materials, "
+            f"16-cell six-face CPML, 4 ports, 128-frequency DFT, {steps} steps")
+
+
+def oracle_sample(budget_s=15.0, steps=None, warmup=1, wall_s=150.0, one_thread=False):
+    """Time the fp64 oracle as it stands on a bounded sample of C3.  With steps=None the step count fills budget_s on
+    the largest crop the host holds; with steps given (the --impl reference arm) the crop is the largest of
+    CPU_SAMPLE_LADDER whose steps+warmup steps are expected to fit in wall_s.
+    Returns dict(value Mcell/s, s_per_step, steps, cores, sample, shape[, one_thread: {value, steps}])."""
+    from oracle import yee
+    ladder = [sh for sh in CPU_SAMPLE_LADDER if _fits_host(sh)] or CPU_SAMPLE_LADDER[-1:]
+    shape = ladder[0]
     if steps is not None:
         o, n = _oracle_on(CPU_SAMPLE_LADDER[-1])
         o.step(1)
@@ -149,10 +205,11 @@ def oracle_sample(budget_s=15.0, steps=None, warmup=1, wall_s=150.0):
         o.step(2)
         rate = 2 * n / (time.perf_counter() - t)            # cells/s estimate
         del o
-        for shape in CPU_SAMPLE_LADDER:
+        for shape in ladder:
             if shape[0] * shape[1] * shape[2] * (steps + warmup) / rate <= wall_s:
                 break
     o, n = _oracle_on(shape)
+    cores = yee.num_threads()
     t = time.perf_counter()
     o.step(max(1, warmup))
     t1 = (time.perf_counter() - t) / max(1, warmup)
@@ -161,20 +218,31 @@ def oracle_sample(budget_s=15.0, steps=None, warmup=1, wall_s=150.0):
     t = time.perf_counter()
     o.step(steps)
     el = time.perf_counter() - t
-    desc = (f"fp64 oracle (g++ -O2 -fopenmp), C3 generator cropped to {shape[0]}x{shape[1]}x{shape[2]} cells "
-            f"(64-entry indexed materials, 16-cell six-face CPML, 4 ports, 128-frequency DFT), {steps} steps")
-    return n * steps / el / 1e6, el / steps, steps, num_threads(), desc, shape
+    out = {"value": n * steps / el / 1e6, "s_per_step": el / steps, "steps": steps, "cores": cores,
+           "sample": _describe(shape, steps), "shape": shape}
+    if one_thread:
+        n1 = int(max(1, min(steps, round(0.5 * budget_s / (el / steps * cores)))))   # about half the budget again
+        yee.set_num_threads(1)
+        try:
+            t = time.perf_counter()
+            o.step(n1)
+            e1 = time.perf_counter() - t
+        finally:
+            yee.set_num_threads(cores)
+        out["one_thread"] = {"value": n * n1 / e1 / 1e6, "unit": UNIT, "cores": 1, "steps": n1}
+    return out
 
 
 def run_reference(args, rank):
     if rank != 0:
         return
     # each "step" of this arm = one oracle step on the bounded crop; K steps after W warm-up steps
-    v, sps, k, cores, desc, shape = oracle_sample(steps=args.steps, warmup=args.warmup)
+    r = oracle_sample(steps=args.steps, warmup=args.warmup)
+    v, sps, k, cores, desc, shape = r["value"], r["s_per_step"], r["steps"], r["cores"], r["sample"], r["shape"]
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": k,
             "warmup": args.warmup, "ms_per_step": sps * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "c3 (bounded crop, CPU oracle)", "grid": list(shape)},
+            "config": {"workload": "c3 (bounded sample, CPU oracle)", "grid": list(shape)},
             "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
             "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0,
@@ -277,13 +345,30 @@ def run_ours(args, rank, world, local_rank):
     achieved = ab / (kms * 1e-3) / 1e9
     step_bytes = algorithmic_bytes(w, impl, "H") + (algorithmic_bytes(w, impl, "E") if impl != "fused" else 0)
     # DRAM bytes of one launch from the committed `ncu --set full` capture of this workload and kernel (profiles/), else null
-    traffic, traffic_src = NCU_TRAFFIC.get((args.workload, kname, w["precision"]), (None, None))
+    traffic, traffic_src = ncu_traffic(args.workload, kname, "f32" if w["precision"] == 32 else "f64", s.fused_kz)
     roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": ab, "kernel_ms": kms,
                 "kernel_ms_all": {"H_or_fused": ms[0], "E": ms[1], "source": ms[2], "probe_dft": ms[3]},
                 "bytes_per_cell_update_step": step_bytes / n_cells,
                 "step_achieved_gbs": step_bytes * K / t_s / 1e9, "frac_of_8000": step_bytes * K / t_s / 1e9 / 8000.0}
+
+    # ---- sustained: BASELINE.json's "2000 steps timed" on C3, own clock samples ---------------------------------------
+    sustained = None
+    if args.workload == "c3" and args.sustained_steps > 0:
+        barrier()
+        ck2 = ClockSampler(local_rank)
+        ck2.start()
+        e0.record(s.stream)
+        s.step(args.sustained_steps)
+        e1.record(s.stream)
+        barrier()
+        c2 = ck2.stop()
+        ts = max_over_ranks(e0.elapsed_time(e1) * 1e-3, world, dev)
+        sustained = {"steps": args.sustained_steps, "ms_per_step": ts / args.sustained_steps * 1e3,
+                     "value": job_throughput(n_cells, args.sustained_steps, world, ts), "unit": UNIT, "clocks": c2,
+                     "step_achieved_gbs": step_bytes * args.sustained_steps / ts / 1e9,
+                     "frac_of_peak": step_bytes * args.sustained_steps / ts / 1e9 / peak}
 
     # ---- end to end through the C ABI with host buffers ---------------------------------------------------------------
     m = w["materials"]
@@ -314,17 +399,30 @@ def run_ours(args, rank, world, local_rank):
                        "step_impl": impl, "fused_kz": s.fused_kz, "l2": "inputs larger than L2 (no flush needed)" if n_cells * 24 > 2.6e8 else
                        "grid fits in L2: launch-bound case, not a roofline case",
                        "parallelism": "replicas only" if world > 1 else "1 GPU", "library": os.path.basename(binding.library_path())},
-            "clocks": ck, "e2e": e2e, "gpu_launches": launches, "roofline": roofline}
+            "clocks": ck, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "sustained": sustained}
     s.destroy()
     del s
     torch.cuda.empty_cache()
     if rank == 0 and world == 1 and not args.no_cpu:
-        v, sps, k, cores, desc, _ = oracle_sample(budget_s=args.cpu_budget)
-        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+        r = oracle_sample(budget_s=args.cpu_budget, one_thread=True)
+        line["cpu_baseline"] = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"],
+                                "one_thread": r.get("one_thread")}
     if rank == 0:
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
+
+
+def spawn_ranks(n):
+    """`python bench.py --gpus N` without a launcher: start the N ranks under torchrun (one process per GPU, rendezvous on
+    127.0.0.1) with this command line; rank 0 of that job prints the line."""
+    import socket
+    with socket.socket() as so:
+        so.bind(("127.0.0.1", 0))
+        port = so.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd))
 
 
 def main():
@@ -337,8 +435,16 @@ def main():
     ap.add_argument("--step-impl", type=int, default=0, help="FDTD_OPT_STEP_IMPL: 0 auto, 1 two-pass, 2 fused")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--cpu-budget", type=float, default=15.0)
+    ap.add_argument("--sustained-steps", type=int, default=2000,
+                    help="steps of the sustained leg on c3 (BASELINE.json: '2000 steps timed'); 0 = off")
+    ap.add_argument("--mode", default="replicas", choices=["replicas", "sharded"],
+                    help="multi-GPU: independent replicas (default) or one z slab of a (600 x 600 x 600 N) grid per rank")
+    ap.add_argument("--slabs", type=int, default=0,
+                    help="--mode sharded on ONE rank: cut the rank's grid into this many slabs on its GPU (protocol cost)")
     args = ap.parse_args()
     args.warmup = max(3, args.warmup)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        spawn_ranks(args.gpus)
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))

@@ -92,6 +92,13 @@ def num_threads():
         return os.cpu_count() or 1
 
 
+def set_num_threads(n):
+    """Number of threads the oracle's OpenMP loops use from now on (bench.py's one-thread figure): omp_set_num_threads of
+    the OpenMP runtime the oracle library is linked against."""
+    lib()
+    C.CDLL("libgomp.so.1").omp_set_num_threads(int(n))
+
+
 class YeeOracle:
     def __init__(self, nx, ny, nz, dx, dy, dz, dt, f32=False, periodic_y=False):
         self.L = lib()

@@ -6,17 +6,28 @@
       and with the fused kernel forced.
   C4  full grid (1024x512x256, fp64, full anisotropic coefficient arrays, 4 ports, 512 frequencies), first 40 steps:
       fields and raw DFTs to 1e-11.
+Rung (ii) of SURVEY 8(d) -- reduced linear scale, FULL step count, S* formed (the method needs 1e5-1e6 steps,
+PAPER.md:116; SURVEY G31 flagged S*_11 at 200 k steps in fp32 as the risk):
+  C2  1/4 scale (128x64x32), all 200 000 steps, inc + tot (via stub => a real S*_11), fp32 GPU in the configuration commit
+      selects and with the fused kernel forced, against the fp64 oracle: fields at 5 checkpoints, S*_11 and S*_21 over the
+      1-500 GHz band.  With FDTD_SLOW=1 also R14's yardstick: the oracle's own fp32 instantiation over the same 200 000 steps.
+  C4  1/8 scale (128x64x32; 1/4 scale = 256x128x64 with FDTD_SLOW=1), all 50 000 steps, inc + tot, fp64 full coefficient
+      arrays: fields 1e-11 at 5 checkpoints, raw DFTs 1e-11, S* column formed.
+  C3  1/4 scale (384x192x192), all 2000 steps: fields at 5 checkpoints, raw DFTs, S* column.
 The oracle is the unmodified fp64 CPU oracle on the same seeded inputs; nothing here comes from the CUDA path.
 """
+import os
 import numpy as np
 import pytest
 
 import workloads as W
 from oracle import sparams as osp
-from paper_2208_04371_b200 import FDTD_F32, FDTD_F64, FDTD_OPT_STEP_IMPL, sparams
-from tests.parity_util import assert_fields, run_pair
+from oracle.yee import YeeOracle
+from paper_2208_04371_b200 import FDTD_F32, FDTD_F64, FDTD_OPT_STEP_IMPL, Solver, sparams
+from tests.parity_util import TOL, assert_fields, run_pair
 
 pytestmark = pytest.mark.gpu
+SLOW = os.environ.get("FDTD_SLOW", "0") == "1"
 
 
 def _sstar(sim, nports, module):
@@ -88,3 +99,116 @@ def test_X3_shaped_full_grid_first_steps():
         assert_fields(rep, FDTD_F32)
         assert max(rep["dft_err"]) <= 1e-4
         s.destroy()
+
+
+# ---- rung (ii): reduced scale, full step count, S* ---------------------------------------------------------------------
+def _run_to_checkpoints(w, gpu_options, checkpoints, prec):
+    """The fp64 oracle and one GPU solver per entry of gpu_options through the same workload; fields compared at every
+    checkpoint against the oracle's running maxima (R13).  Returns (oracle, {name: solver}, {name: worst field error})."""
+    o = YeeOracle.from_workload(w, track_max=True)
+    gpus = {name: Solver.from_workload(w, precision=prec, options=opts) for name, opts in gpu_options.items()}
+    worst = {name: 0.0 for name in gpus}
+    done = 0
+    for cp in checkpoints:
+        o.step(cp - done)
+        for g in gpus.values():
+            g.step(cp - done)
+        done = cp
+        emax, hmax = o.running_max()
+        assert emax > 0 and hmax > 0
+        for c in range(6):
+            ref = o.read_field(c)
+            for name, g in gpus.items():
+                d = np.abs(g.read_fields(c).cpu().numpy().astype(np.float64) - ref).max()
+                worst[name] = max(worst[name], d / (emax if c < 3 else hmax))
+    return o, gpus, worst
+
+
+def _dfts(sim, nports):
+    V, I = zip(*[sim.read_port_dft(p) for p in range(nports)])
+    return np.array(V), np.array(I)
+
+
+def _s_column(inc, tot, nports, module):
+    Vi, Ii = _dfts(inc, nports)
+    Vt, _ = _dfts(tot, nports)
+    return np.array(module.s_star_column(0, list(Vi), list(Ii), list(Vt)))
+
+
+def test_C2_quarter_scale_full_200k_steps_sparams():
+    cps = [2000, 20000, 60000, 120000, 200000]
+    opts = {"auto": None, "fused": {FDTD_OPT_STEP_IMPL: 2}}
+    sims = {}
+    for run in ("inc", "tot"):
+        w = W.interconnect_c2(run=run, div=4)
+        assert (w["nx"], w["ny"], w["nz"], w["steps"], len(w["freqs"])) == (128, 64, 32, 200000, 256)
+        o, gpus, worst = _run_to_checkpoints(w, opts, cps, FDTD_F32)
+        print(f"C2/4 {run} 200k steps: field_err " + ", ".join(f"{k} ({g.impl_name}) {worst[k]:.3e}" for k, g in gpus.items()))
+        assert max(worst.values()) <= TOL[FDTD_F32], worst
+        sims[run] = (o, gpus, w)
+    So = _s_column(sims["inc"][0], sims["tot"][0], 2, osp)
+    assert np.abs(So[0]).max() > 1e-2, "the via stub must reflect: S*_11 of this test is meant to be non-trivial"
+    Vo, Io = _dfts(sims["tot"][0], 2)
+    for name in opts:
+        Sg = _s_column(sims["inc"][1][name], sims["tot"][1][name], 2, sparams)
+        d11, d21 = np.abs(So[0] - Sg[0]).max(), np.abs(So[1] - Sg[1]).max()
+        Vg, Ig = _dfts(sims["tot"][1][name], 2)
+        raw = (np.abs(Vg - Vo).max() / np.abs(Vo).max(), np.abs(Ig - Io).max() / np.abs(Io).max())
+        print(f"C2/4 200k steps {name}: |dS*_11| = {d11:.3e}, |dS*_21| = {d21:.3e} (max|S*_11| = {np.abs(So[0]).max():.3f}, "
+              f"max|S*_21| = {np.abs(So[1]).max():.3f}); raw fp32 DFT drift (V, I) = ({raw[0]:.3e}, {raw[1]:.3e}), informational (R14)")
+        assert d11 <= 1e-3 and d21 <= 1e-3
+    if SLOW:   # R14's yardstick: what fp32 time stepping itself loses over 200 000 steps (same algorithm, same order, on the CPU)
+        y = {}
+        for run in ("inc", "tot"):
+            o32 = YeeOracle.from_workload(sims[run][2], f32=True)
+            o32.step(200000)
+            y[run] = o32
+        S32 = _s_column(y["inc"], y["tot"], 2, osp)
+        V32, I32 = _dfts(y["tot"], 2)
+        print(f"C2/4 200k steps yardstick (fp32 oracle vs fp64 oracle): |dS*_11| = {np.abs(So[0] - S32[0]).max():.3e}, "
+              f"|dS*_21| = {np.abs(So[1] - S32[1]).max():.3e}, raw DFT (V, I) = ({np.abs(V32 - Vo).max() / np.abs(Vo).max():.3e}, "
+              f"{np.abs(I32 - Io).max() / np.abs(Io).max():.3e})")
+    for _, gpus, _ in sims.values():
+        for g in gpus.values():
+            g.destroy()
+
+
+@pytest.mark.parametrize("div", [8] + ([4] if SLOW else []))
+def test_C4_reduced_scale_full_50k_steps_fp64(div):
+    cps = [500, 5000, 15000, 30000, 50000]
+    sims = {}
+    for run in ("inc", "tot"):
+        w = W.interconnect_c4(run=run, div=div)
+        assert (w["steps"], len(w["freqs"]), len(w["ports"]), w["precision"]) == (50000, 512, 4, FDTD_F64)
+        o, gpus, worst = _run_to_checkpoints(w, {"auto": None, "fused": {FDTD_OPT_STEP_IMPL: 2}}, cps, FDTD_F64)
+        print(f"C4/{div} {run} 50k steps: field_err " + ", ".join(f"{k} ({g.impl_name}) {worst[k]:.3e}" for k, g in gpus.items()))
+        assert max(worst.values()) <= TOL[FDTD_F64], worst
+        sims[run] = (o, gpus)
+    So = _s_column(sims["inc"][0], sims["tot"][0], 4, osp)
+    Vo, Io = _dfts(sims["tot"][0], 4)
+    for name in ("auto", "fused"):
+        Vg, Ig = _dfts(sims["tot"][1][name], 4)
+        raw = max(np.abs(Vg - Vo).max() / np.abs(Vo).max(), np.abs(Ig - Io).max() / np.abs(Io).max())
+        Sg = _s_column(sims["inc"][1][name], sims["tot"][1][name], 4, sparams)
+        dS = np.abs(So - Sg).max()
+        print(f"C4/{div} 50k steps {name}: raw DFT {raw:.3e}, |dS*| = {dS:.3e} (max|S*_11| = {np.abs(So[0]).max():.3f})")
+        assert raw <= 1e-11 and dS <= 1e-7
+    for _, gpus in sims.values():
+        for g in gpus.values():
+            g.destroy()
+
+
+def test_C3_quarter_scale_full_2000_steps():
+    w = W.throughput_c3(div=4)
+    assert (w["nx"], w["ny"], w["nz"], w["steps"], w["pml"]) == (384, 192, 192, 2000, [16] * 6)
+    o, gpus, worst = _run_to_checkpoints(w, {"auto": None}, [100, 500, 1000, 1500, 2000], FDTD_F32)
+    g = gpus["auto"]
+    print(f"C3/4 2000 steps ({g.impl_name}, kz {g.fused_kz}): field_err {worst['auto']:.3e}")
+    assert worst["auto"] <= TOL[FDTD_F32]
+    So, Sg = _s_column(o, o, 4, osp), _s_column(g, g, 4, sparams)     # one structure: tot == inc
+    Vo, Io = _dfts(o, 4)
+    Vg, Ig = _dfts(g, 4)
+    raw = max(np.abs(Vg - Vo).max() / np.abs(Vo).max(), np.abs(Ig - Io).max() / np.abs(Io).max())
+    print(f"C3/4 2000 steps: raw DFT {raw:.3e}, |dS*| = {np.abs(So - Sg).max():.3e}")
+    assert raw <= 1e-4 and np.abs(So - Sg).max() <= 1e-3
+    g.destroy()

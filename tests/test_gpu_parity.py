@@ -197,7 +197,7 @@ def test_null_stream_runs_plain_launches_with_the_same_result():
     """include/fdtd.h: on the NULL (legacy default) stream no graph can be captured; fdtd_step falls back to plain
     launches there and says so through fdtd_graph_replays."""
     import torch
-    w = W.random_box(11, nx=40, ny=22, nz=18, steps=27, precision=FDTD_F32)
+    w = W.random_box(11, nx=40, ny=22, nz=18, steps=27, precision=FDTD_F32, with_mu=False)
     out = []
     for null in (False, True):
         s = Solver(w["nx"], w["ny"], w["nz"], w["dx"], w["dy"], w["dz"], w["dt"], FDTD_F32)
