@@ -413,6 +413,99 @@ def run_ours(args, rank, world, local_rank):
         dist.destroy_process_group()
 
 
+# --------------------------------------------------------------------------------------------------------------------
+# --mode sharded: z-slab decomposition, weak scaling at 600^3 cells per GPU (Table I)
+# --------------------------------------------------------------------------------------------------------------------
+def run_sharded(args, rank, world, local_rank):
+    """One 600^3 slab per rank of a 600 x 600 x 600N grid; the slabs push their boundary planes into each other's halo from
+    the kernels (paper_2208_04371_b200/sharded.py).  With ONE rank and --slabs S the rank's grid is cut into S slabs on its
+    own GPU instead (they share a stream): that measures what the protocol itself costs, not a scaling point."""
+    import torch
+    import torch.distributed as dist
+
+    import workloads as W
+    from paper_2208_04371_b200 import binding
+    from paper_2208_04371_b200.sharded import DistributedSlab, ShardedSolver
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    K, Wm = args.steps, args.warmup
+    on_one_gpu = world == 1
+    n_slabs = world if world > 1 else max(1, args.slabs)
+    per_gpu = 1 if world > 1 else n_slabs                      # slabs that share this rank's GPU
+    edge = args.edge
+    # weak scaling: edge^3 cells per GPU.  One rank with --slabs S keeps ONE GPU's load (edge^2 x edge planes) and cuts it.
+    w = W.weak_scaling_600(n_slabs=world, steps=K, edge=edge)
+    n_cells = w["nx"] * w["ny"] * w["nz"]
+    if on_one_gpu:
+        sim = ShardedSolver(w, [str(dev)] * n_slabs)
+        stream = sim.solvers[0].stream
+        first = sim.solvers[0]
+    else:
+        sim = DistributedSlab(w, str(dev), transport="peer")
+        stream = sim.solver.stream
+        first = sim.solver
+    torch.cuda.synchronize(dev)
+    sim.step(Wm)
+    barrier()
+    clocks = ClockSampler(local_rank)
+    clocks.start()
+    l0 = sim.launch_count
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    sim.step(K)
+    e1.record(stream)
+    barrier()
+    ck = clocks.stop()
+    launches = sim.launch_count - l0
+    t_s = max_over_ranks(e0.elapsed_time(e1) * 1e-3, world, dev)
+    value = n_cells * K / t_s / 1e6
+    ab = algorithmic_bytes(dict(w, nz=w["nz"] // world, pml=w["pml"][:4] + [w["pml"][4] if world == 1 else 0, w["pml"][5] if world == 1 else 0]),
+                           "fused", "H")
+    peak, peak_src = measured_peak()
+    # end to end: every slab's material slice from pinned host memory, reset, K steps, the port DFTs back to the host
+    barrier()
+    t0 = time.perf_counter()
+    h2d = sim.upload_materials(pinned=True) if on_one_gpu else sim.upload_materials(w, pinned=True)
+    sim.reset()
+    sim.step(K)
+    out = [sim.read_port_dft(p) for p in range(len(w["ports"]))]
+    torch.cuda.synchronize(dev)
+    te = max_over_ranks(time.perf_counter() - t0, world, dev)
+    assert all(np.isfinite(v).all() and np.isfinite(i).all() for v, i in out)
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+            "ms_per_step": t_s / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic",
+            "config": {"workload": w["name"], "grid": [w["nx"], w["ny"], w["nz"]], "cells": n_cells,
+                       "cells_per_gpu": n_cells // world, "materials": "indexed", "cpml_cells": w["pml"], "ports": len(w["ports"]),
+                       "dft_freqs": len(w["freqs"]), "step_impl": first.impl_name, "fused_kz": first.fused_kz,
+                       "parallelism": (f"z-slabs x{world}, one per GPU, halo planes stored into the neighbour by the kernels (NVLink peer stores)"
+                                       if world > 1 else f"1 GPU, its grid cut into {per_gpu} z slab(s) on the same device (protocol cost only)"),
+                       "l2": "inputs larger than L2 (no flush needed)", "library": os.path.basename(binding.library_path())},
+            "clocks": ck,
+            "e2e": {"value": n_cells * K / te / 1e6, "unit": UNIT, "h2d_bytes_per_step": h2d / K,
+                    "d2h_bytes_per_step": len(w["ports"]) * len(w["freqs"]) * 32 / K,
+                    "what": "per slab: fdtd_set_materials_indexed(pinned host slice) + fdtd_reset; K steps; fdtd_read_port_dft x ports"},
+            "gpu_launches": launches,
+            "roofline": {"bound": "hbm", "kernel": "k_step_fused (one slab's step incl. hand-over kernels)", "achieved": ab / (t_s / K) / 1e9,
+                         "peak": peak, "unit": "GB/s", "frac": ab / (t_s / K) / 1e9 / peak, "traffic": None, "peak_source": peak_src,
+                         "algorithmic_bytes_per_launch": ab}}
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def spawn_ranks(n):
     """`python bench.py --gpus N` without a launcher: start the N ranks under torchrun (one process per GPU, rendezvous on
     127.0.0.1) with this command line; rank 0 of that job prints the line."""
@@ -441,6 +534,7 @@ def main():
                     help="multi-GPU: independent replicas (default) or one z slab of a (600 x 600 x 600 N) grid per rank")
     ap.add_argument("--slabs", type=int, default=0,
                     help="--mode sharded on ONE rank: cut the rank's grid into this many slabs on its GPU (protocol cost)")
+    ap.add_argument("--edge", type=int, default=600, help="--mode sharded: cells per GPU = edge^3 (the paper's Table I: 600)")
     args = ap.parse_args()
     args.warmup = max(3, args.warmup)
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
@@ -450,6 +544,9 @@ def main():
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
         run_reference(args, rank)
+        return
+    if args.mode == "sharded":
+        run_sharded(args, rank, world, local_rank)
         return
     run_ours(args, rank, world, local_rank)
 

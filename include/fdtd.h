@@ -64,7 +64,8 @@ enum {
                                Capture needs a real stream: on the NULL (legacy default) stream fdtd_step always issues
                                plain launches (fdtd_graph_replays() stays 0)                                             */
   FDTD_OPT_GRAPH_UNROLL = 3,/* steps per captured graph (default 8; rounded up to even for the fused step)              */
-  FDTD_OPT_FUSED_KZ = 4     /* planes per z chunk of the fused kernel (0 = auto: measured at commit)                    */
+  FDTD_OPT_FUSED_KZ = 4,    /* planes per z chunk of the fused kernel (0 = auto: measured at commit)                    */
+  FDTD_OPT_Z_SPIN = 5       /* linked z slabs: polls of a hand-over counter before a wait gives up (default 2e7, ~2 s)  */
 };
 
 /* A port (Fig. 1a): a soft E_z source on a box of the plane i = is (surface 'e'), a voltage box and
@@ -177,6 +178,31 @@ int fdtd_set_z_interfaces(fdtd_t*, int lo_open, int hi_open);
 int fdtd_step_begin(fdtd_t*);
 int fdtd_step_end(fdtd_t*);
 int fdtd_plane(fdtd_t*, int comp, int k, void** dev_ptr, size_t* bytes);
+
+/* Linked z slabs: the exchange moves INTO the kernels.  Instead of the caller copying planes between
+ * fdtd_step_begin and fdtd_step_end, a slab is given the addresses of its neighbours' halo planes once, and from then on
+ *   - the fused kernel stores the new Hx, Hy of its top plane also into the upper slab's halo plane -1,
+ *   - the kernel that updates E on plane 0 stores the new Ex, Ey also into the lower slab's halo plane nz
+ * (plain global stores: NVLink peer stores when the neighbour lives on another GPU -- peer access of another device of
+ * this process is enabled by fdtd_z_link; memory of another process must have been opened with CUDA IPC by the caller),
+ * and the hand-over is ordered by one 64-bit arrival counter per face in the RECEIVER's memory: the sender posts the step
+ * number after its kernel (release at system scope), the receiver's stream waits for it before the kernel that reads the
+ * halo (acquire; a bounded spin: FDTD_OPT_Z_SPIN).  Sequence of one step, all of it enqueued by the library:
+ *     [wait E(n) from above]  fused kernel  [post H(n+1/2) up]      [wait H(n+1/2) from below]  E on plane 0, source,
+ *     probes, DFT  [post E(n+1) down]
+ *   fdtd_z_halo(side, planes, flag)   side 0 (z-): where the slab BELOW must put Hx, Hy of its top plane (my halo plane
+ *                                     -1), side 1 (z+): where the slab ABOVE must put Ex, Ey of its plane 0 (my halo plane
+ *                                     nz): planes[comp + 2*set] for field set 0 and 1 (the step ping-pongs between them;
+ *                                     all slabs must step in lockstep from the same reset), flag = my arrival counter.
+ *   fdtd_z_link(side, peer_planes, peer_flag)   give this slab the fdtd_z_halo answer of the neighbour on `side`
+ *                                     (side 1: the upper slab's side-0 answer; side 0: the lower slab's side-1 answer).
+ * Once every open side is linked, fdtd_step(n) works on the slab (and replays captured graphs).  fdtd_step_begin /
+ * fdtd_step_end stay available and do the same per half step: slabs that share ONE stream must be advanced that way
+ * (all begins, then all ends, in ascending slab order), so that no wait ever precedes its post in stream order; slabs on
+ * their own GPUs run fdtd_step(n) concurrently.  A wait that gives up makes the next synchronising read return FDTD_ECUDA.
+ * Errors: FDTD_ESTATE before commit / for a face that is not an interface; FDTD_ECUDA without a peer path. */
+int fdtd_z_halo(fdtd_t*, int side, void* planes[4], void** flag);
+int fdtd_z_link(fdtd_t*, int side, void* const peer_planes[4], void* peer_flag);
 
 long fdtd_step_count(const fdtd_t*);
 /* Number of kernel launches the library has enqueued since commit (graph nodes count individually). */

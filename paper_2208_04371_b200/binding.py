@@ -18,7 +18,7 @@ FDTD_F32, FDTD_F64 = 32, 64
 FDTD_W_DGAUSS, FDTD_W_GAUSS, FDTD_W_GSINE = 0, 1, 2
 FDTD_MAT_INDEXED, FDTD_MAT_FULL = 0, 1
 FDTD_EX, FDTD_EY, FDTD_EZ, FDTD_HX, FDTD_HY, FDTD_HZ = range(6)
-FDTD_OPT_STEP_IMPL, FDTD_OPT_USE_GRAPH, FDTD_OPT_GRAPH_UNROLL, FDTD_OPT_FUSED_KZ = 1, 2, 3, 4
+FDTD_OPT_STEP_IMPL, FDTD_OPT_USE_GRAPH, FDTD_OPT_GRAPH_UNROLL, FDTD_OPT_FUSED_KZ, FDTD_OPT_Z_SPIN = 1, 2, 3, 4, 5
 
 _ERRNAMES = {-1: "FDTD_EINVAL", -2: "FDTD_ECFL", -3: "FDTD_ESTATE", -4: "FDTD_ENOMEM", -5: "FDTD_ECUDA", -6: "FDTD_ERANGE"}
 
@@ -70,6 +70,8 @@ SYMBOLS = {
     "fdtd_step_begin": (C.c_int, [_vp]),
     "fdtd_step_end": (C.c_int, [_vp]),
     "fdtd_plane": (C.c_int, [_vp, C.c_int, C.c_int, C.POINTER(C.c_void_p), C.POINTER(C.c_size_t)]),
+    "fdtd_z_halo": (C.c_int, [_vp, C.c_int, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)]),
+    "fdtd_z_link": (C.c_int, [_vp, C.c_int, C.POINTER(C.c_void_p), C.c_void_p]),
     "fdtd_last_error": (C.c_char_p, [_vp]),
     "fdtd_destroy": (None, [_vp]),
 }
@@ -285,6 +287,18 @@ def fdtd_plane(h, comp, k):
     p, n = C.c_void_p(), C.c_size_t()
     _check(h, lib().fdtd_plane(h, int(comp), int(k), C.byref(p), C.byref(n)))
     return int(p.value), int(n.value)
+
+
+def fdtd_z_halo(h, side):
+    """([4 plane addresses: comp + 2 * set], counter address) a neighbour's kernels write for this slab's face `side`."""
+    planes, flag = (C.c_void_p * 4)(), C.c_void_p()
+    _check(h, lib().fdtd_z_halo(h, int(side), planes, C.byref(flag)))
+    return [int(p) for p in planes], int(flag.value)
+
+
+def fdtd_z_link(h, side, peer_planes, peer_flag):
+    """Give this slab the fdtd_z_halo answer (addresses valid in THIS process) of its neighbour on `side`."""
+    _check(h, lib().fdtd_z_link(h, int(side), (C.c_void_p * 4)(*[int(p) for p in peer_planes]), C.c_void_p(int(peer_flag))))
 
 
 def fdtd_last_error(h) -> str:

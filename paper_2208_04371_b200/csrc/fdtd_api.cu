@@ -53,6 +53,8 @@ struct fdtd {
   std::vector<double> freqs;
   long opt_impl = 0, opt_graph = 1, opt_unroll = 8, opt_kz = 0;
   int z_lo_open = 0, z_hi_open = 0;   // this grid is a z slab of a larger one (fdtd_set_z_interfaces)
+  bool z_linked[2] = {false, false};  // fdtd_z_link: the kernels push my boundary planes into the neighbour on that side
+  long opt_zspin = 20000000;          // polls of a hand-over flag before the wait kernel gives up (about 2 s)
   bool mid_step = false;              // between fdtd_step_begin and fdtd_step_end
   bool committed = false;
   long nstep = 0;
@@ -81,6 +83,18 @@ struct fdtd {
   long long plane() const { return (long long)pitch() * (ny + 1); }
   long long cells_padded() const { return plane() * (nz + 2); }
   int S(int a) const { return npml[2 * a] + npml[2 * a + 1]; }
+  // x slabs are stored in whole 16-byte vectors (fdtd_params.h): [0, xlo_end) and [xhi_begin, round_up(nx, V)); when the two
+  // would meet, the whole row is one slab.  xslab(i) = padded slab coordinate of cell i, or -1.
+  int vlen() const { return 16 / (int)esize(); }
+  int nx_up() const { return (nx + vlen() - 1) / vlen() * vlen(); }
+  bool x_whole() const {
+    return npml[0] > 0 && npml[1] > 0 && (npml[0] + vlen() - 1) / vlen() * vlen() >= (nx - npml[1]) / vlen() * vlen();
+  }
+  int xlo_end() const { return x_whole() ? nx_up() : (npml[0] + vlen() - 1) / vlen() * vlen(); }
+  int xhi_begin() const { return (x_whole() || npml[1] == 0) ? (1 << 30) : (nx - npml[1]) / vlen() * vlen(); }
+  int Sxp() const { return xlo_end() + (xhi_begin() < (1 << 30) ? nx_up() - xhi_begin() : 0); }
+  int xslab(int i) const { return i < xlo_end() ? i : (i >= xhi_begin() ? xlo_end() + (i - xhi_begin()) : -1); }
+  int Sp(int a) const { return a == 0 ? Sxp() : S(a); }   // slab cells per line as stored
 
   virtual size_t workspace_bytes() const = 0;
   virtual int commit(void* ws, size_t bytes, void* stream) = 0;
@@ -90,6 +104,8 @@ struct fdtd {
   virtual int step_begin() = 0;
   virtual int step_end() = 0;
   virtual int plane_ptr(int comp, int k, void** ptr, size_t* bytes) = 0;
+  virtual int z_halo(int side, void** planes, void** flag) = 0;
+  virtual int z_link(int side, void* const* peer_planes, void* peer_flag) = 0;
   virtual int profile_step(long n, double* ms) = 0;
   virtual int read_field(int comp, void* dst) = 0;
   virtual int write_field(int comp, const void* src) = 0;
@@ -133,7 +149,7 @@ template <typename T>
 struct Solver : fdtd {
   // workspace carve (byte offsets), filled by layout()
   struct Carve {
-    size_t field[6], field2[6], idx, tab, coef[9], psi[12], psiH2[6], vec[18], ports, freqs, dftV, dftI, lastV, lastI, nstep, partial, pcount, total;
+    size_t field[6], field2[6], idx, tab, coef[9], psi[12], psiH2[6], vec[18], ports, freqs, dftV, dftI, lastV, lastI, zflags, nstep, partial, pcount, total;
   };
   char* ws = nullptr;
   Carve cv{};
@@ -149,6 +165,11 @@ struct Solver : fdtd {
   int sm_count = 148;
   unsigned probe_blocks = 1; // blocks per port of k_probe_dft: about 1024 samples of the largest V box each
   FusedParams<T> fpar[2];
+  // z-slab links (fdtd_z_link): side 0 = lower neighbour's halo plane nz of Ex, Ey, side 1 = upper neighbour's halo plane -1
+  // of Hx, Hy, each in field set 0 and 1 ([comp + 2 * set]); and the neighbour's arrival counter for those planes
+  T* peer_planes[2][4] = {{nullptr, nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr, nullptr}};
+  unsigned long long* peer_flag[2] = {nullptr, nullptr};
+  unsigned long long* zflag(int q) const { return reinterpret_cast<unsigned long long*>(ws + cv.zflags) + q; }
   cudaGraphExec_t gexec2 = nullptr;  // graph captured with cur == 1
   std::vector<T> h_tab;        // host staging of the material table (kept alive for the async upload)
   std::vector<T> h_vec[18];
@@ -160,13 +181,13 @@ struct Solver : fdtd {
     if (gexec2) cudaGraphExecDestroy(gexec2);
   }
   // auto: the fused kernel pays off once the grid no longer fits in L2 (small grids are launch-bound)
-  bool slabs_fit() const { return S(0) <= kMaxSlab && S(1) <= kMaxSlab && S(2) <= kMaxSlab; }
+  bool slabs_fit() const { return Sp(0) <= kMaxSlab && S(1) <= kMaxSlab && S(2) <= kMaxSlab; }
   bool want_fused() const { return slabs_fit() && (opt_impl == 2 || z_lo_open || z_hi_open || (opt_impl == 0 && (long long)nx * ny * nz >= (4LL << 20))); }
 
   int mode() const { return (mat_mode == FDTD_MAT_FULL ? kModeFull : 0) | (has_mu ? kModeMu : 0); }
   size_t psi_elems(int a) const {
     if (S(a) == 0) return 0;
-    if (a == 0) return (size_t)S(0) * ny * nz;
+    if (a == 0) return (size_t)Sxp() * ny * nz;
     if (a == 1) return (size_t)pitch() * S(1) * nz;
     return (size_t)pitch() * ny * S(2);
   }
@@ -192,7 +213,7 @@ struct Solver : fdtd {
     if (want_fused()) for (int q = 0; q < 6; ++q) c.psiH2[q] = take(psi_elems(psi_axis(q)) * sizeof(T));
     {  // 18 CPML vectors in one block, [axis][bE cE kE bH cH kH][stride]: the fused kernel copies it to shared memory whole
       int stride = kMaxSlab;
-      for (int a = 0; a < 3; ++a) if (S(a) > stride) stride = (S(a) + 3) / 4 * 4;
+      for (int a = 0; a < 3; ++a) if (Sp(a) > stride) stride = (Sp(a) + 3) / 4 * 4;
       const size_t base = take((size_t)18 * stride * sizeof(T));
       for (int q = 0; q < 18; ++q) c.vec[q] = base + (size_t)q * stride * sizeof(T);
     }
@@ -202,6 +223,7 @@ struct Solver : fdtd {
     c.dftI = take((ports.size() * freqs.size() + 1) * 2 * sizeof(double));
     c.lastV = take((ports.size() + 1) * sizeof(double));
     c.lastI = take((ports.size() + 1) * sizeof(double));
+    c.zflags = take(4 * sizeof(unsigned long long));   // [0] H planes arrived from below, [1] E planes arrived from above, [2] time-out
     c.nstep = take(sizeof(long long));
     c.partial = take((ports.size() + 1) * kProbeMaxBlocks * 2 * sizeof(double));
     c.pcount = take((ports.size() + 1) * sizeof(int));
@@ -219,6 +241,13 @@ struct Solver : fdtd {
   int step_begin() override;
   int step_end() override;
   int plane_ptr(int comp, int k, void** ptr, size_t* bytes) override;
+  int z_halo(int side, void** planes, void** flag) override;
+  int z_link(int side, void* const* peer_planes, void* peer_flag) override;
+  bool z_slab() const { return z_lo_open || z_hi_open; }
+  bool z_all_linked() const { return (!z_lo_open || z_linked[0]) && (!z_hi_open || z_linked[1]); }
+  int z_check_timeout(const char* who);
+  void enqueue_begin();
+  void enqueue_end();
   void enqueue_ports();
   void enqueue_ports_ev(cudaEvent_t* ev);
   int profile_step(long n, double* ms) override;
@@ -277,6 +306,19 @@ void Solver<T>::build_cpml_vectors() {
     for (int q = 0; q < lo; ++q) { put(vE, q, grade(lo - q, lo)); put(vH, q, grade(lo - q - 0.5, lo)); }
     for (int r = 0; r < hi; ++r) { put(vE, lo + r, grade(r, hi)); put(vH, lo + r, grade(r + 0.5, hi)); }
   }
+  // x: the kernels address the x slabs in whole vectors (padded slab coordinate, fdtd_params.h); cells of those vectors that
+  // lie outside the layer get b = 1, c = 0, 1/kappa = 1, which leaves their psi at zero and their update plain
+  if (S(0) > 0) {
+    const int lo = npml[0], hi = npml[1], len = Sxp();
+    for (int v = 0; v < 6; ++v) {
+      std::vector<T> padded(len, T(v % 3 == 1 ? 0 : 1));
+      for (int i = 0; i < nx; ++i) {
+        const int sp_ = xslab(i), st = i < lo ? i : (i >= nx - hi ? lo + i - (nx - hi) : -1);
+        if (sp_ >= 0 && st >= 0) padded[sp_] = h_vec[v][st];
+      }
+      h_vec[v].swap(padded);
+    }
+  }
 }
 
 template <typename T>
@@ -314,6 +356,9 @@ int Solver<T>::commit(void* w, size_t bytes, void* st) {
   sp.db0 = T(dt / phys::mu0);
   sp.idx_ = T(1.0 / dx); sp.idy_ = T(1.0 / dy); sp.idz_ = T(1.0 / dz);
   for (int a = 0; a < 3; ++a) { sp.lo[a] = npml[2 * a]; sp.hi[a] = npml[2 * a + 1]; }
+  sp.xlo_end = S(0) > 0 ? xlo_end() : 0;
+  sp.xhi_begin = S(0) > 0 ? xhi_begin() : (1 << 30);
+  sp.Sxp = S(0) > 0 ? Sxp() : 0;
   build_cpml_vectors();
   for (int a = 0; a < 3; ++a) {
     const T** tgt[6] = {&sp.bE[a], &sp.cE[a], &sp.kE[a], &sp.bH[a], &sp.cH[a], &sp.kH[a]};
@@ -436,6 +481,7 @@ template <typename T>
 int Solver<T>::copy_field(int comp, void* user, bool to_user) {
   if (!committed) return fail(FDTD_ESTATE, "fields are available after fdtd_commit");
   if (comp < 0 || comp > 5 || !user) return fail(FDTD_EINVAL, "bad component or null pointer");
+  if (to_user) { const int r = z_check_timeout("fdtd_read_fields"); if (r != FDTD_OK) return r; }
   if (!to_user && mid_step) return fail(FDTD_ESTATE, "fdtd_write_fields: fdtd_step_end is pending (the field sets are half updated)");
   return copy3d(ws + (cur ? cv.field2[comp] : cv.field[comp]), sizeof(T), user, to_user);
 }
@@ -593,6 +639,7 @@ int Solver<T>::build_fused() {
   for (int c = 0; c < 2; ++c) {
     FusedParams<T>& fp = fpar[c];
     fp.sp = sp;
+    fp.peer_H[0] = fp.peer_H[1] = nullptr;
     for (int f = 0; f < 6; ++f) { fp.sp.src[f] = field_origin(f, c); fp.sp.dst[f] = field_origin(f, 1 - c); }
     for (int q = 0; q < 6; ++q) {
       fp.psiH_src[q] = reinterpret_cast<T*>(ws + (c ? cv.psiH2[q] : cv.psi[q]));
@@ -801,6 +848,7 @@ void Solver<T>::launch_fused(cudaEvent_t* ev) {
 
 template <typename T>
 void Solver<T>::enqueue_step(cudaEvent_t* ev) {
+  if (z_slab()) { enqueue_begin(); enqueue_end(); return; }
   if (fused) {
     launch_fused(ev);
     launches += 1;
@@ -891,8 +939,9 @@ int Solver<T>::step(long n) {
   if (!committed) return fail(FDTD_ESTATE, "fdtd_step: call after fdtd_commit");
   if (n < 0) return fail(FDTD_EINVAL, "fdtd_step: n < 0");
   if (mid_step) return fail(FDTD_ESTATE, "fdtd_step: fdtd_step_end is pending");
-  if ((z_lo_open || z_hi_open) && n > 0)
-    return fail(FDTD_ESTATE, "fdtd_step: a z slab advances with fdtd_step_begin / plane exchange / fdtd_step_end");
+  if (z_slab() && !z_all_linked() && n > 0)
+    return fail(FDTD_ESTATE, "fdtd_step: a z slab that is not linked to its neighbours (fdtd_z_link) advances with "
+                             "fdtd_step_begin / plane exchange / fdtd_step_end");
   long left = n;
   if (persistent && n > 0) {
     long done = 0;
@@ -914,6 +963,7 @@ int Solver<T>::step(long n) {
     if (r != FDTD_OK) return r;
     long nodes = fused ? 1 : 2;
     if (!ports.empty()) { nodes += 1; for (const PortDev& q : ports) if (q.has_source) nodes += 1; }
+    if (z_slab()) nodes += 3 * (z_lo_open + z_hi_open) - z_hi_open;   // E on plane 0, one wait and one post per open side
     while (left >= graph_steps) {
       const cudaError_t e = cudaGraphLaunch(*g, stream);
       if (e != cudaSuccess) return cuda_fail(e, "graph launch");
@@ -936,13 +986,32 @@ int Solver<T>::step(long n) {
 // end:   E^{n+1} on plane 0 of a lo-open slab with the two-pass E kernel (same R5 arithmetic; old E from the previous
 //        set, new H of planes -1 and 0 from the new one), then source, probes, DFT.
 // [caller: my new Ex, Ey of plane 0 -> halo plane nz of the lower neighbour]
+// With links (fdtd_z_link) the planes are not copied by the caller: the kernels store them into the neighbour's halo and
+// the hand-over is ordered by the neighbours' arrival counters (k_z_post / k_z_wait):
+//   begin: [wait: E planes of the previous step have arrived from above]  fused kernel (+ Hx, Hy of my top plane into the
+//          upper slab's halo plane -1)  [post to the upper slab: H planes of this step delivered]
+//   end:   [wait: H planes of this step have arrived from below]  E on plane 0 (+ Ex, Ey into the lower slab's halo plane
+//          nz), source, probes, DFT  [post to the lower slab: E planes of this step delivered]
+template <typename T>
+void Solver<T>::enqueue_begin() {
+  if (z_hi_open && z_linked[1]) {   // the device counter still holds the number of completed steps
+    k_z_wait<<<1, 1, 0, stream>>>(zflag(1), sp.nstep, 0, reinterpret_cast<int*>(zflag(2)), (long long)opt_zspin);
+    ++launches;
+  }
+  launch_fused(nullptr);
+  launches += 1;
+  if (z_hi_open && z_linked[1]) {   // the fused kernel has incremented the counter: this step's number
+    k_z_post<<<1, 1, 0, stream>>>(peer_flag[1], sp.nstep, 0);
+    ++launches;
+  }
+}
+
 template <typename T>
 int Solver<T>::step_begin() {
   if (!committed) return fail(FDTD_ESTATE, "fdtd_step_begin: call after fdtd_commit");
   if (!fused) return fail(FDTD_ESTATE, "fdtd_step_begin: the handle does not run the fused step");
   if (mid_step) return fail(FDTD_ESTATE, "fdtd_step_begin: fdtd_step_end is pending");
-  launch_fused(nullptr);
-  launches += 1;
+  enqueue_begin();
   mid_step = true;
   const cudaError_t e = cudaGetLastError();
   return e == cudaSuccess ? FDTD_OK : cuda_fail(e, "fdtd_step_begin");
@@ -952,15 +1021,20 @@ template <typename T, int MODE>
 static void launch_E_plane0(const StepParams<T>& q, cudaStream_t st) {
   constexpr int V = VecOf<T>::V;
   const long long nvec = (long long)((q.nx + V - 1) / V) * q.ny;
-  k_update_E<T, MODE><<<dim3((unsigned)((nvec + 127) / 128), 1, 1), dim3(128, 1, 1), 0, st>>>(q);
+  k_update_E<T, MODE, true><<<dim3((unsigned)((nvec + 127) / 128), 1, 1), dim3(128, 1, 1), 0, st>>>(q);
 }
 
 template <typename T>
-int Solver<T>::step_end() {
-  if (!mid_step) return fail(FDTD_ESTATE, "fdtd_step_end: no fdtd_step_begin is pending");
+void Solver<T>::enqueue_end() {
   if (z_lo_open) {
+    if (z_linked[0]) {
+      k_z_wait<<<1, 1, 0, stream>>>(zflag(0), sp.nstep, 0, reinterpret_cast<int*>(zflag(2)), (long long)opt_zspin);
+      ++launches;
+    }
     StepParams<T> q = fpar[cur ^ 1].sp;               // the launch that just ran: src = old set, dst = new (= current) set
     for (int f = kHx; f <= kHz; ++f) q.src[f] = q.dst[f];   // H^{n+1/2} is read from the new set (halo plane -1 included)
+    q.peer_E[0] = z_linked[0] ? peer_planes[0][0 + 2 * cur] : nullptr;
+    q.peer_E[1] = z_linked[0] ? peer_planes[0][1 + 2 * cur] : nullptr;
     switch (mode()) {
       case 0: launch_E_plane0<T, 0>(q, stream); break;
       case 1: launch_E_plane0<T, 1>(q, stream); break;
@@ -970,10 +1044,79 @@ int Solver<T>::step_end() {
     launches += 1;
   }
   enqueue_ports();
+  if (z_lo_open && z_linked[0]) {
+    k_z_post<<<1, 1, 0, stream>>>(peer_flag[0], sp.nstep, 0);
+    ++launches;
+  }
+}
+
+template <typename T>
+int Solver<T>::step_end() {
+  if (!mid_step) return fail(FDTD_ESTATE, "fdtd_step_end: no fdtd_step_begin is pending");
+  enqueue_end();
   mid_step = false;
   nstep += 1;
   const cudaError_t e = cudaGetLastError();
   return e == cudaSuccess ? FDTD_OK : cuda_fail(e, "fdtd_step_end");
+}
+
+// ---- links between z slabs ---------------------------------------------------------------------------------------------
+// z_halo: where a neighbour's kernels must put the planes this slab reads from its halo -- side 0: Hx, Hy of plane -1
+// (written by the slab below), side 1: Ex, Ey of plane nz (written by the slab above) -- in field set 0 and set 1
+// ([comp + 2 * set]), and this slab's arrival counter for them.
+template <typename T>
+int Solver<T>::z_halo(int side, void** planes, void** flag) {
+  if (!committed) return fail(FDTD_ESTATE, "fdtd_z_halo: call after fdtd_commit");
+  if (side < 0 || side > 1 || !planes || !flag) return fail(FDTD_EINVAL, "fdtd_z_halo: bad side or null pointer");
+  if (!(side ? z_hi_open : z_lo_open)) return fail(FDTD_ESTATE, "fdtd_z_halo: that z face is not an interface (fdtd_set_z_interfaces)");
+  const int comp0 = side ? kEx : kHx;
+  const long long k = side ? nz : -1;
+  for (int set = 0; set < 2; ++set)
+    for (int c = 0; c < 2; ++c) planes[c + 2 * set] = field_origin(comp0 + c, set) + k * plane();
+  *flag = zflag(side);
+  return FDTD_OK;
+}
+
+// z_link: the neighbour's z_halo answer for the face that touches this slab's `side`.  From now on the kernels of this slab
+// store their boundary planes there and post the neighbour's counter; fdtd_step(n) becomes available once every open
+// side is linked.  A neighbour on another device of this process gets peer access enabled here.
+template <typename T>
+int Solver<T>::z_link(int side, void* const* pl, void* pflag) {
+  if (!committed) return fail(FDTD_ESTATE, "fdtd_z_link: call after fdtd_commit");
+  if (mid_step) return fail(FDTD_ESTATE, "fdtd_z_link: fdtd_step_end is pending");
+  if (side < 0 || side > 1 || !pl || !pflag) return fail(FDTD_EINVAL, "fdtd_z_link: bad side or null pointer");
+  if (!(side ? z_hi_open : z_lo_open)) return fail(FDTD_ESTATE, "fdtd_z_link: that z face is not an interface (fdtd_set_z_interfaces)");
+  for (int q = 0; q < 4; ++q) if (!pl[q]) return fail(FDTD_EINVAL, "fdtd_z_link: null plane pointer");
+  const int pdev = device_of(pflag);
+  if (pdev < 0) return fail(FDTD_EINVAL, "fdtd_z_link: the neighbour's counter is not device memory");
+  if (pdev != device) {
+    int can = 0;
+    if (cudaDeviceCanAccessPeer(&can, device, pdev) != cudaSuccess || !can)
+      return fail(FDTD_ECUDA, "fdtd_z_link: device %d cannot access device %d (no NVLink / PCIe peer path)", device, pdev);
+    const cudaError_t e = cudaDeviceEnablePeerAccess(pdev, 0);
+    if (e != cudaSuccess && e != cudaErrorPeerAccessAlreadyEnabled) return cuda_fail(e, "fdtd_z_link: cudaDeviceEnablePeerAccess");
+    cudaGetLastError();
+  }
+  for (int q = 0; q < 4; ++q) peer_planes[side][q] = static_cast<T*>(pl[q]);
+  peer_flag[side] = static_cast<unsigned long long*>(pflag);
+  z_linked[side] = true;
+  if (side == 1)   // the launch that reads set c writes set 1 - c: its top-plane H goes to the upper slab's set 1 - c
+    for (int c = 0; c < 2; ++c) { fpar[c].peer_H[0] = peer_planes[1][0 + 2 * (1 - c)]; fpar[c].peer_H[1] = peer_planes[1][1 + 2 * (1 - c)]; }
+  // graphs captured before the link do not contain the hand-over
+  if (gexec) { cudaGraphExecDestroy(gexec); gexec = nullptr; }
+  if (gexec2) { cudaGraphExecDestroy(gexec2); gexec2 = nullptr; }
+  return FDTD_OK;
+}
+
+// a wait kernel that gave up has recorded it in the slab's flag block; every synchronising read checks
+template <typename T>
+int Solver<T>::z_check_timeout(const char* who) {
+  if (!z_slab() || !(z_linked[0] || z_linked[1])) return FDTD_OK;
+  int flag = 0;
+  const cudaError_t e = cudaMemcpyAsync(&flag, zflag(2), sizeof(int), cudaMemcpyDeviceToHost, stream);
+  if (e != cudaSuccess || cudaStreamSynchronize(stream) != cudaSuccess) return cuda_fail(cudaGetLastError(), who);
+  if (flag) return fail(FDTD_ECUDA, "%s: a z-slab hand-over timed out (a neighbouring slab did not deliver its planes)", who);
+  return FDTD_OK;
 }
 
 // Device address and size of the padded plane k in [-1, nz] of component comp in the set that holds the current state
@@ -999,7 +1142,7 @@ int Solver<T>::read_port_dft(int port, double* V, double* I) {
   }
   if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
   if (e != cudaSuccess) return cuda_fail(e, "fdtd_read_port_dft");
-  return FDTD_OK;
+  return z_check_timeout("fdtd_read_port_dft");
 }
 
 template <typename T>
@@ -1010,7 +1153,7 @@ int Solver<T>::read_port_last(int port, double* V, double* I) {
   if (e == cudaSuccess) e = cudaMemcpyAsync(I, pp.lastI + port, sizeof(double), cudaMemcpyDeviceToHost, stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
   if (e != cudaSuccess) return cuda_fail(e, "fdtd_read_port_last");
-  return FDTD_OK;
+  return z_check_timeout("fdtd_read_port_last");
 }
 
 template <typename T>
@@ -1128,6 +1271,7 @@ int fdtd_set_option(fdtd_t* h, int option, long value) {
     case FDTD_OPT_USE_GRAPH: h->opt_graph = value ? 1 : 0; return FDTD_OK;
     case FDTD_OPT_GRAPH_UNROLL: if (value < 1 || value > 1024) break; h->opt_unroll = value; return FDTD_OK;
     case FDTD_OPT_FUSED_KZ: if (value < 0 || value > 65535) break; h->opt_kz = value; return FDTD_OK;
+    case FDTD_OPT_Z_SPIN: if (value < 1) break; h->opt_zspin = value; return FDTD_OK;
   }
   return h->fail(FDTD_EINVAL, "fdtd_set_option: unknown option %d or bad value %ld", option, value);
 }
@@ -1146,6 +1290,8 @@ int fdtd_step(fdtd_t* h, long n) { FDTD_ON_DEVICE(h); return h->step(n); }
 int fdtd_step_begin(fdtd_t* h) { FDTD_ON_DEVICE(h); return h->step_begin(); }
 int fdtd_step_end(fdtd_t* h) { FDTD_ON_DEVICE(h); return h->step_end(); }
 int fdtd_plane(fdtd_t* h, int comp, int k, void** dev_ptr, size_t* bytes) { return h ? h->plane_ptr(comp, k, dev_ptr, bytes) : FDTD_EINVAL; }
+int fdtd_z_halo(fdtd_t* h, int side, void* planes[4], void** flag) { return h ? h->z_halo(side, planes, flag) : FDTD_EINVAL; }
+int fdtd_z_link(fdtd_t* h, int side, void* const peer_planes[4], void* peer_flag) { FDTD_ON_DEVICE(h); return h->z_link(side, peer_planes, peer_flag); }
 int fdtd_set_z_interfaces(fdtd_t* h, int lo_open, int hi_open) {
   if (!h) return FDTD_EINVAL;
   if (h->committed) return h->fail(FDTD_ESTATE, "fdtd_set_z_interfaces: call before fdtd_commit");

@@ -48,6 +48,8 @@ struct FusedParams {
   int ntx, nty, group;   // tiles in x, y; dispatch order: groups of `group` tiles, all z chunks of a group in ascending
                          // order before the next group (1-D grid: block -> (group, chunk, tile of the group))
   const T* cpack;        // the 18 CPML vectors [axis][bE cE kE bH cH kH][kMaxSlab], contiguous
+  T* peer_H[2];          // z slab linked to its upper neighbour (fdtd_z_link): that slab's halo plane -1 of Hx, Hy in the
+                         // set this launch writes (element (0,0) of the plane, same pitch); nullptr = not linked
 };
 
 __host__ __device__ constexpr int round128(int v) { return (v + 127) / 128 * 128; }
@@ -293,14 +295,12 @@ __global__ void __launch_bounds__((TY + 2) * 32, 1) k_step_fused(const __grid_co
   const bool cin = rowwarp ? (jin && i0 < p.nx) : (jin && i0 >= 0 && lane < TY);  // the thread's cell(s) exist
   const bool owned = rowwarp && r >= 1 && cin;                                    // ... and this thread stores them
   const int nvalid = rowwarp ? min(V, p.nx - i0) : 1;                             // cells of the vector inside the grid
-  const int Sx = p.lo[0] + p.hi[0], Sy = p.lo[1] + p.hi[1], Sz = p.lo[2] + p.hi[2];
+  const int Sx = p.Sxp, Sy = p.lo[1] + p.hi[1], Sz = p.lo[2] + p.hi[2];
   const int sj = (cin && Sy > 0) ? slab_coord(j, p.lo[1], p.hi[1], p.ny) : -1;
-  // x slab: coordinate of the thread's first cell; the whole vector is handled with 128-bit psi accesses when the slab
-  // edges fall on vector boundaries (xvec), cell by cell otherwise
-  const bool xs = cin && Sx > 0 && (rowwarp ? ((i0 < p.lo[0]) || (i0 + V > p.nx - p.hi[0]))
-                                            : (slab_coord(i0, p.lo[0], p.hi[0], p.nx) >= 0));
-  const bool xvec = (p.lo[0] % V == 0) && ((p.nx - p.hi[0]) % V == 0) && (p.nx % V == 0);
-  const int si0 = xs ? slab_coord(i0, p.lo[0], p.hi[0], p.nx) : -1;
+  // x slab: padded coordinate of the thread's first cell (the x slabs are stored in whole vectors, fdtd_params.h: a row
+  // warp's vector is wholly inside or wholly outside, always 128-bit psi accesses)
+  const int si0 = (cin && Sx > 0) ? xslab_coord(p, i0) : -1;
+  const bool xs = si0 >= 0;
   const bool wj = (j == 0), wi = (i0 == 0);
   const bool xtail = x0 + TX > p.nx;
   const int kzlo = p.lo[2], kzhi = p.nz - p.hi[2];
@@ -512,34 +512,23 @@ __global__ void __launch_bounds__((TY + 2) * 32, 1) k_step_fused(const __grid_co
         }
         if (xs) {  // x slab: psiHyx (from D+x Ez) -> Hy, psiHzx (from D+x Ey) -> Hz
           const long long q0 = qx(k);
-          if (xvec) {
-            T a[V], d[V];
-            ldv(fp.psiH_src[pHyx] + q0, a); ldv(fp.psiH_src[pHzx] + q0, d);
+          T a[V], d[V];
+          ldv(fp.psiH_src[pHyx] + q0, a); ldv(fp.psiH_src[pHzx] + q0, d);
 #pragma unroll
-            for (int v = 0; v < V; ++v) {
-              const T b = cp(0, 3, si0 + v), c = cp(0, 4, si0 + v) * p.idx_, km = (cp(0, 5, si0 + v) - T(1)) * p.idx_;
-              a[v] = b * a[v] + c * dEz_x[v]; d[v] = b * d[v] + c * dEy_x[v];
-              hy[v] += dby[v] * (km * dEz_x[v] + a[v]); hz[v] -= dbz[v] * (km * dEy_x[v] + d[v]);
-            }
-            if (wr) { stv(p.psi[pHyx] + q0, a); stv(p.psi[pHzx] + q0, d); }
-          } else {
-#pragma unroll
-            for (int v = 0; v < V; ++v) {
-              const int si = slab_coord(i0 + v, p.lo[0], p.hi[0], p.nx);
-              if (si >= 0 && v < nvalid) {
-                const long long q = q0 + si - (si0 >= 0 ? si0 : 0);
-                const T b = cp(0, 3, si), c = cp(0, 4, si) * p.idx_, km = (cp(0, 5, si) - T(1)) * p.idx_;
-                const T pyx = b * fp.psiH_src[pHyx][q] + c * dEz_x[v], pzx = b * fp.psiH_src[pHzx][q] + c * dEy_x[v];
-                if (wr) { p.psi[pHyx][q] = pyx; p.psi[pHzx][q] = pzx; }
-                hy[v] += dby[v] * (km * dEz_x[v] + pyx); hz[v] -= dbz[v] * (km * dEy_x[v] + pzx);
-              }
-            }
+          for (int v = 0; v < V; ++v) {
+            const T b = cp(0, 3, si0 + v), c = cp(0, 4, si0 + v) * p.idx_, km = (cp(0, 5, si0 + v) - T(1)) * p.idx_;
+            a[v] = b * a[v] + c * dEz_x[v]; d[v] = b * d[v] + c * dEy_x[v];
+            hy[v] += dby[v] * (km * dEz_x[v] + a[v]); hz[v] -= dbz[v] * (km * dEy_x[v] + d[v]);
           }
+          if (wr) { stv(p.psi[pHyx] + q0, a); stv(p.psi[pHzx] + q0, d); }
         }
       }
       if (r < TY) { stv(hnb + oHn, hx); stv(hnb + TY * TX + oHn, hz); }
       if (owned && it >= 2) {
         stv_stream(p.dst[kHx] + o, hx); stv_stream(p.dst[kHy] + o, hy); stv_stream(p.dst[kHz] + o, hz);
+        // top plane of a linked z slab: the tangential H the slab above needs for its E update on plane 0 goes straight
+        // into that slab's halo plane (NVLink peer stores from the kernel that computes them)
+        if (k == p.nz - 1 && fp.peer_H[0] != nullptr) { stv(fp.peer_H[0] + orow, hx); stv(fp.peer_H[1] + orow, hy); }
       }
     }
     __syncwarp();
@@ -596,29 +585,15 @@ __global__ void __launch_bounds__((TY + 2) * 32, 1) k_step_fused(const __grid_co
         }
         if (xs) {  // x slab: psiEyx (from D-x Hz) -> Ey, psiEzx (from D-x Hy) -> Ez
           const long long q0 = qx(k);
-          if (xvec) {
-            T a[V], d[V];
-            ldv(p.psi[pEyx] + q0, a); ldv(p.psi[pEzx] + q0, d);
+          T a[V], d[V];
+          ldv(p.psi[pEyx] + q0, a); ldv(p.psi[pEzx] + q0, d);
 #pragma unroll
-            for (int v = 0; v < V; ++v) {
-              const T b = cp(0, 0, si0 + v), c = cp(0, 1, si0 + v) * p.idx_, km = (cp(0, 2, si0 + v) - T(1)) * p.idx_;
-              a[v] = b * a[v] + c * dHz_x[v]; d[v] = b * d[v] + c * dHy_x[v];
-              ay[v] -= km * dHz_x[v] + a[v]; az[v] += km * dHy_x[v] + d[v];
-            }
-            stv(p.psi[pEyx] + q0, a); stv(p.psi[pEzx] + q0, d);
-          } else {
-#pragma unroll
-            for (int v = 0; v < V; ++v) {
-              const int si = slab_coord(i0 + v, p.lo[0], p.hi[0], p.nx);
-              if (si >= 0 && v < nvalid) {
-                const long long q = q0 + si - (si0 >= 0 ? si0 : 0);
-                const T b = cp(0, 0, si), c = cp(0, 1, si) * p.idx_, km = (cp(0, 2, si) - T(1)) * p.idx_;
-                const T pyx = b * p.psi[pEyx][q] + c * dHz_x[v], pzx = b * p.psi[pEzx][q] + c * dHy_x[v];
-                p.psi[pEyx][q] = pyx; p.psi[pEzx][q] = pzx;
-                ay[v] -= km * dHz_x[v] + pyx; az[v] += km * dHy_x[v] + pzx;
-              }
-            }
+          for (int v = 0; v < V; ++v) {
+            const T b = cp(0, 0, si0 + v), c = cp(0, 1, si0 + v) * p.idx_, km = (cp(0, 2, si0 + v) - T(1)) * p.idx_;
+            a[v] = b * a[v] + c * dHz_x[v]; d[v] = b * d[v] + c * dHy_x[v];
+            ay[v] -= km * dHz_x[v] + a[v]; az[v] += km * dHy_x[v] + d[v];
           }
+          stv(p.psi[pEyx] + q0, a); stv(p.psi[pEzx] + q0, d);
         }
       }
       if (owned) {

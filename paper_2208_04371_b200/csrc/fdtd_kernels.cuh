@@ -58,6 +58,11 @@ template <> __device__ __forceinline__ void ld_index<2>(const uint8_t* p, unsign
 __device__ __forceinline__ int slab_coord(int u, int lo, int hi, int n) {
   return u < lo ? u : (u >= n - hi ? lo + u - (n - hi) : -1);
 }
+// padded x-slab coordinate of cell i (fdtd_params.h: the x slabs are stored in whole vectors), or -1 outside
+template <typename T>
+__device__ __forceinline__ int xslab_coord(const StepParams<T>& p, int i) {
+  return i < p.xlo_end ? i : (i >= p.xhi_begin ? p.xlo_end + (i - p.xhi_begin) : -1);
+}
 
 // Material modes: bit 0 = full per-cell coefficient arrays (else uint8 index + table), bit 1 = permeability given.
 enum { kModeIndexed = 0, kModeFull = 1, kModeMu = 2 };
@@ -66,10 +71,10 @@ enum { kModeIndexed = 0, kModeFull = 1, kModeMu = 2 };
 // H pass.  R5 step 1:  psiH = bH psiH + cH D+E ;  Hx -= Dbx (D+y Ez / kHy + psiHxy - D+z Ey / kHz - psiHxz)  etc.
 // ------------------------------------------------------------------------------------------------------------------
 // the H update of the V consecutive cells starting at (i0, j, k); i0 < nx, j < ny
-// XV: handle x-slab vectors with 128-bit psi / coefficient accesses when the slab edges fall on vector boundaries.  It
-// costs ~20 registers: worth it where most warps contain x-slab lanes and occupancy is not the limit (the persistent
-// small-grid kernel: C1 24.3 -> 15.1 us/step), not in the two-pass kernels (64 / 72 registers, 8 / 7 blocks per SM).
-template <typename T, int MODE, bool XV = false>
+// x slabs are stored in whole vectors (fdtd_params.h), so a thread's V cells are wholly inside or wholly outside: the x-slab
+// update is 128-bit psi and coefficient accesses for any layer thickness (a cell-by-cell path cost the fused step 40 % on
+// grids with 10-cell layers: profiles/r02_midsize.md).
+template <typename T, int MODE>
 __device__ __forceinline__ void update_H_vec(const StepParams<T>& p, int i0, int j, int k) {
   constexpr int V = VecOf<T>::V;
   const long long o = i0 + (long long)p.P * j + p.PS * k;
@@ -83,9 +88,7 @@ __device__ __forceinline__ void update_H_vec(const StepParams<T>& p, int i0, int
 
   const int sj = slab_coord(j, p.lo[1], p.hi[1], p.ny);
   const int sk = slab_coord(k, p.lo[2], p.hi[2], p.nz);
-  const bool xs = (i0 < p.lo[0]) || (i0 + V > p.nx - p.hi[0]);
-  // slab edges on vector boundaries: a vector is then wholly inside or wholly outside the x slab (128-bit psi accesses)
-  const bool xvec = XV && (p.lo[0] % V == 0) && ((p.nx - p.hi[0]) % V == 0) && (p.nx % V == 0);
+  const bool xs = (i0 < p.xlo_end) || (i0 >= p.xhi_begin);
 
   T ax[V], ay[V], az[V];          // curl accumulators
   T d0[V], d1[V], d2[V], d3[V];  // raw derivatives kept for the y / z slab psi updates
@@ -105,26 +108,12 @@ __device__ __forceinline__ void update_H_vec(const StepParams<T>& p, int i0, int
       // x terms need the per-cell kappa: done in the x-slab branch or here with kappa = 1
       dxa[v] = dxEz; dxb[v] = dxEy;
       if (!xs) { ay[v] -= dxEz; az[v] += dxEy; }
-      else if (!xvec) {
-        const int si = slab_coord(i0 + v, p.lo[0], p.hi[0], p.nx);
-        T ikx = T(1);
-        T pyx = T(0), pzx = T(0);
-        if (si >= 0 && i0 + v < p.nx) {
-          ikx = p.kH[0][si];
-          const long long q = si + (long long)(p.lo[0] + p.hi[0]) * (j + (long long)p.ny * k);
-          const T b = p.bH[0][si], c = p.cH[0][si];
-          pyx = b * p.psi[pHyx][q] + c * dxEz; p.psi[pHyx][q] = pyx;
-          pzx = b * p.psi[pHzx][q] + c * dxEy; p.psi[pHzx][q] = pzx;
-        }
-        ay[v] -= dxEz * ikx + pyx;
-        az[v] += dxEy * ikx + pzx;
-      }
       d0[v] = dyEz; d1[v] = dyEx; d2[v] = dzEy; d3[v] = dzEx;
     }
   }
-  if (xs && xvec) {  // x slab, whole vector: psiHyx (from D+x Ez) -> Hy, psiHzx (from D+x Ey) -> Hz
-    const int si0 = slab_coord(i0, p.lo[0], p.hi[0], p.nx);
-    const long long q = si0 + (long long)(p.lo[0] + p.hi[0]) * (j + (long long)p.ny * k);
+  if (xs) {  // x slab, whole vector: psiHyx (from D+x Ez) -> Hy, psiHzx (from D+x Ey) -> Hz
+    const int si0 = xslab_coord(p, i0);
+    const long long q = si0 + (long long)p.Sxp * (j + (long long)p.ny * k);
     T a[V], d[V], b[V], c[V], ik[V];
     ldv(p.psi[pHyx] + q, a); ldv(p.psi[pHzx] + q, d);
     ldv(p.bH[0] + si0, b); ldv(p.cH[0] + si0, c); ldv(p.kH[0] + si0, ik);
@@ -206,7 +195,8 @@ __global__ void __launch_bounds__(128) k_update_H(const StepParams<T> p) {
 // then the low-face wall rows are forced to zero (PEC walls; PAPER.md:46 for the ground).
 // ------------------------------------------------------------------------------------------------------------------
 // the E update of the V consecutive cells starting at (i0, j, k); i0 < nx, j < ny
-template <typename T, int MODE, bool XV = false>
+// PEER: the launch that updates E on plane 0 of a z slab also stores the new Ex, Ey into the lower neighbour's halo plane
+template <typename T, int MODE, bool PEER = false>
 __device__ __forceinline__ void update_E_vec(const StepParams<T>& p, int i0, int j, int k) {
   constexpr int V = VecOf<T>::V;
   const long long o = i0 + (long long)p.P * j + p.PS * k;
@@ -223,8 +213,7 @@ __device__ __forceinline__ void update_E_vec(const StepParams<T>& p, int i0, int
 
   const int sj = slab_coord(j, p.lo[1], p.hi[1], p.ny);
   const int sk = slab_coord(k, p.lo[2], p.hi[2], p.nz);
-  const bool xs = (i0 < p.lo[0]) || (i0 + V > p.nx - p.hi[0]);
-  const bool xvec = XV && (p.lo[0] % V == 0) && ((p.nx - p.hi[0]) % V == 0) && (p.nx % V == 0);
+  const bool xs = (i0 < p.xlo_end) || (i0 >= p.xhi_begin);
 
   T ax[V], ay[V], az[V];
   T d0[V], d1[V], d2[V], d3[V];  // raw derivatives kept for the y / z slab psi updates
@@ -243,25 +232,12 @@ __device__ __forceinline__ void update_E_vec(const StepParams<T>& p, int i0, int
       az[v] = -dyHx * iky;
       dxa[v] = dxHz; dxb[v] = dxHy;
       if (!xs) { ay[v] -= dxHz; az[v] += dxHy; }
-      else if (!xvec) {
-        const int si = slab_coord(i0 + v, p.lo[0], p.hi[0], p.nx);
-        T ikx = T(1), pyx = T(0), pzx = T(0);
-        if (si >= 0 && i0 + v < p.nx) {
-          ikx = p.kE[0][si];
-          const long long q = si + (long long)(p.lo[0] + p.hi[0]) * (j + (long long)p.ny * k);
-          const T b = p.bE[0][si], c = p.cE[0][si];
-          pyx = b * p.psi[pEyx][q] + c * dxHz; p.psi[pEyx][q] = pyx;
-          pzx = b * p.psi[pEzx][q] + c * dxHy; p.psi[pEzx][q] = pzx;
-        }
-        ay[v] -= dxHz * ikx + pyx;
-        az[v] += dxHy * ikx + pzx;
-      }
       d0[v] = dyHz; d1[v] = dyHx; d2[v] = dzHy; d3[v] = dzHx;
     }
   }
-  if (xs && xvec) {  // x slab, whole vector: psiEyx (from D-x Hz) -> Ey, psiEzx (from D-x Hy) -> Ez
-    const int si0 = slab_coord(i0, p.lo[0], p.hi[0], p.nx);
-    const long long q = si0 + (long long)(p.lo[0] + p.hi[0]) * (j + (long long)p.ny * k);
+  if (xs) {  // x slab, whole vector: psiEyx (from D-x Hz) -> Ey, psiEzx (from D-x Hy) -> Ez
+    const int si0 = xslab_coord(p, i0);
+    const long long q = si0 + (long long)p.Sxp * (j + (long long)p.ny * k);
     T a[V], d[V], b[V], c[V], ik[V];
     ldv(p.psi[pEyx] + q, a); ldv(p.psi[pEzx] + q, d);
     ldv(p.bE[0] + si0, b); ldv(p.cE[0] + si0, c); ldv(p.kE[0] + si0, ik);
@@ -323,16 +299,45 @@ __device__ __forceinline__ void update_E_vec(const StepParams<T>& p, int i0, int
     if (wi || wj || pad) ez[v] = T(0);
   }
   stv(p.dst[kEx] + o, ex); stv(p.dst[kEy] + o, ey); stv(p.dst[kEz] + o, ez);
+  if (PEER && k == 0 && p.peer_E[0] != nullptr) {   // NVLink peer stores: the tangential E the slab below needs for its next H update
+    const long long oq = i0 + (long long)p.P * j;
+    stv(p.peer_E[0] + oq, ex); stv(p.peer_E[1] + oq, ey);
+  }
 }
 
-template <typename T, int MODE>
+template <typename T, int MODE, bool PEER = false>
 __global__ void __launch_bounds__(128) k_update_E(const StepParams<T> p) {
   constexpr int V = VecOf<T>::V;
   const int nvec = (p.nx + V - 1) / V, v = blockIdx.x * blockDim.x + threadIdx.x;
   const int j = gridDim.y > 1 ? (int)blockIdx.y : v / nvec, i0 = (gridDim.y > 1 ? v : v - j * nvec) * V;
   const int k = blockIdx.z;
   if (j >= p.ny) return;
-  update_E_vec<T, MODE>(p, i0, j, k);
+  update_E_vec<T, MODE, PEER>(p, i0, j, k);
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// z-slab hand-over flags (fdtd_z_link; guard cells exchanged every step).  A slab pushes its boundary
+// planes into the neighbour's halo with peer stores from the kernel that computes them; what orders the neighbour's next
+// kernel after those stores is a step counter in the NEIGHBOUR's memory:
+//   k_z_post  (stream-ordered after the producing kernel)  fence; *peer_flag = step      release at system scope
+//   k_z_wait  (stream-ordered before the consuming kernel) spin until *flag >= step      acquire at system scope
+// `step` is read from the device step counter (+ add), so the same captured graph serves every replay.  The spin is
+// bounded: after max_spins polls it records a time-out in *err and returns (no launch can hang the device).
+// ------------------------------------------------------------------------------------------------------------------
+__global__ void k_z_post(unsigned long long* peer_flag, const long long* nstep, long long add) {
+  const unsigned long long v = (unsigned long long)(*nstep + add);
+  __threadfence_system();
+  asm volatile("st.release.sys.global.u64 [%0], %1;" ::"l"(peer_flag), "l"(v) : "memory");
+}
+__global__ void k_z_wait(const unsigned long long* flag, const long long* nstep, long long add, int* err, long long max_spins) {
+  const unsigned long long want = (unsigned long long)(*nstep + add);
+  for (long long it = 0;; ++it) {
+    unsigned long long v;
+    asm volatile("ld.acquire.sys.global.u64 %0, [%1];" : "=l"(v) : "l"(flag) : "memory");
+    if (v >= want) break;
+    if (it >= max_spins) { atomicExch(err, 1); break; }
+    __nanosleep(it < 64 ? 100 : 1000);
+  }
 }
 
 // ------------------------------------------------------------------------------------------------------------------

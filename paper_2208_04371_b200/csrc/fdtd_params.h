@@ -41,11 +41,17 @@ struct StepParams {
   T idx_, idy_, idz_;   // 1/dx, 1/dy, 1/dz
   // CPML: thickness per face and per-axis coefficient vectors indexed by the slab coordinate s in [0, lo+hi)
   int lo[3], hi[3];
+  // x slabs in whole 16-byte vectors: cells [0, xlo_end) and [xhi_begin, pitch) carry psi; padded slab coordinate
+  // sp(i) = i below xlo_end, xlo_end + (i - xhi_begin) from xhi_begin on; Sxp = padded cells per row (multiple of the
+  // vector length).  Cells of those vectors outside the true layer have b = 1, c = 0, 1/kappa = 1: their psi stays zero.
+  int xlo_end, xhi_begin, Sxp;
   const T* bE[3]; const T* cE[3]; const T* kE[3];   // kE = 1/kappa at integer positions (E profile)
   const T* bH[3]; const T* cH[3]; const T* kH[3];   // at half-integer positions (H profile)
-  T* psi[12];       // slab-only arrays: y-slab  i + P*(s + Sy*k);  z-slab  i + P*(j + ny*s);  x-slab  s + Sx*(j + ny*k)
+  T* psi[12];       // slab-only arrays: y-slab  i + P*(s + Sy*k);  z-slab  i + P*(j + ny*s);  x-slab  sp + Sxp*(j + ny*k)
   long long* nstep; // device step counter, incremented by the first kernel of every step
   int z_lo_open;    // 1: this grid is a z slab of a larger one and plane 0 is not a wall (Ex, Ey there are ordinary cells)
+  T* peer_E[2];     // z slab linked to its lower neighbour (fdtd_z_link): that slab's halo plane nz of Ex, Ey (element (0,0)
+                    // of the plane, same pitch), written by the kernel that updates E on plane 0; nullptr = not linked
 };
 
 struct PortDev {

@@ -10,8 +10,7 @@
 //            grid barrier
 //   after the last step: V probe of that step.
 //
-// The arithmetic is the two-pass step's (update_H_vec / update_E_vec of fdtd_kernels.cuh, here with the vectorised x-slab
-// path XV: same formulas, 128-bit psi accesses -- small grids have x-slab lanes in most warps), the source is added by the
+// The arithmetic is the two-pass step's (update_H_vec / update_E_vec of fdtd_kernels.cuh), the source is added by the
 // thread that owns the cell right after its E update (ports in order, like the per-port k_source launches), and the probe
 // sums use the thread -> warp -> block order of k_probe_dft's one-block path.
 #pragma once
@@ -127,7 +126,7 @@ __global__ void __launch_bounds__(kPersistThreads) k_steps_persistent(const Step
       for (int port = blockIdx.x; port < q.nports; port += gridDim.x) probe_V_dft(q, port, n - 1, sh);
     for (int v = tid0; v < nvec; v += nthr) {
       const int iv = v % nvx, jk = v / nvx;
-      update_H_vec<T, MODE, true>(p, iv * V, jk % p.ny, jk / p.ny);
+      update_H_vec<T, MODE>(p, iv * V, jk % p.ny, jk / p.ny);
     }
     grid.sync();
     // ---- E phase, source ----------------------------------------------------------------------------------------------
@@ -135,7 +134,7 @@ __global__ void __launch_bounds__(kPersistThreads) k_steps_persistent(const Step
     for (int v = tid0; v < nvec; v += nthr) {
       const int iv = v % nvx, jk = v / nvx;
       const int i0 = iv * V, j = jk % p.ny, k = jk / p.ny;
-      update_E_vec<T, MODE, true>(p, i0, j, k);
+      update_E_vec<T, MODE>(p, i0, j, k);
       for (int t = 0; t < nsrc; ++t) {
         const SrcBox b = sbox[t];
         if (k >= b.sk0 && k < b.sk1 && j >= b.sj0 && j <= b.sj1 && b.is >= i0 && b.is < i0 + V)

@@ -1,19 +1,24 @@
-"""Domain decomposition along z: one slab per GPU, two plane exchanges per step (PAPER.md:143, 157:
-"decomposing the domain into a number of grids equal to the number of GPUs", guard cells exchanged every step).
+"""Domain decomposition along z: one slab per GPU, the halo exchange issued from the kernels (
+PAPER.md:143, 157: "decomposing the domain into a number of grids equal to the number of GPUs", guard cells exchanged
+every step; Table I: weak scaling at 600^3 cells per GPU).
 
 The arithmetic is the single-GPU library's, slab by slab (include/fdtd.h "domain decomposition along z"); this module only
-does bookkeeping (which planes, which ports, which CPML cells belong to which slab) and moves planes:
+does bookkeeping (which planes, which ports, which CPML cells belong to which slab) and introduces the slabs to each other:
 
-    every slab   fdtd_step_begin          fused kernel: H^{n+1/2}, and E^{n+1} except on plane 0 of a lo-open slab
-    exchange     Hx, Hy of my top plane   -> halo plane -1 of the slab above          (2 planes up)
-    every slab   fdtd_step_end            E^{n+1} on plane 0 of lo-open slabs, source, probes, DFT
-    exchange     Ex, Ey of my plane 0     -> halo plane nz of the slab below          (2 planes down)
+    link      every slab is given the addresses of its neighbours' halo planes and arrival counters (fdtd_z_halo /
+              fdtd_z_link): device pointers within one process, CUDA-IPC mappings of the neighbour's workspace across
+              processes (torch's IPC machinery opens them: memory plumbing, not arithmetic).
+    step      [wait E from above]  fused kernel: H^{n+1/2} everywhere, E^{n+1} except on plane 0 of a lo-open slab; its
+              blocks on the top plane also store Hx, Hy into the upper slab's halo plane -1  [post H up]
+              [wait H from below]  E^{n+1} on plane 0, stored also into the lower slab's halo plane nz; source, probes,
+              DFT  [post E down]
 
-Planes of slabs with equal nx, ny are contiguous buffers of equal size, so an exchange is one copy per plane: a device
-copy when the slabs share a process (`ShardedSolver(devices=[...])`, also how the decomposition is tested on one GPU) or
-torch.distributed send/recv over NCCL with one slab per rank (`ShardedSolver.distributed()`; NVLink/NVSwitch peer
-transfers, 4 planes of nx*ny words per interface per step: 19 MB for a 1536x768 face against ~50 GB of HBM traffic of
-the slab's own step, which is why no overlap machinery is built around it).
+Four planes of nx*ny words cross an interface per step (19 MB for a 1536x768 face against ~50 GB of HBM traffic of the
+slab's own step), as stores of the kernels that compute them: no pack/unpack kernels, no host-issued copies, no collective.
+`ShardedSolver` drives all slabs from one process (slabs on one GPU share a stream and advance half step by half step, so
+that no wait ever precedes its post in stream order: this is also how the decomposition is tested on one GPU);
+`DistributedSlab` is one slab per torch.distributed rank.  With transport="nccl" the planes travel as host-issued
+send/recv pairs instead (the fallback when CUDA IPC is not available, and the protocol the gloo CPU test exercises).
 """
 from __future__ import annotations
 
@@ -73,60 +78,88 @@ def owned_ports(w, z0, z1):
     return [n for n, p in enumerate(w["ports"]) if _port_planes(p)[0] >= z0 and _port_planes(p)[1] <= z1]
 
 
+def link_neighbours(lower, upper):
+    """Introduce two adjacent slabs of one process to each other (lower.z+ touches upper.z-)."""
+    planes, flag = B.fdtd_z_halo(upper.h, 0)          # where Hx, Hy of lower's top plane must go
+    B.fdtd_z_link(lower.h, 1, planes, flag)
+    planes, flag = B.fdtd_z_halo(lower.h, 1)          # where Ex, Ey of upper's plane 0 must go
+    B.fdtd_z_link(upper.h, 0, planes, flag)
+
+
 class ShardedSolver:
-    """All slabs of a workload.  `devices`: one entry per slab (repeat a device to put several slabs on one GPU)."""
+    """All slabs of a workload in one process.  `devices`: one entry per slab (repeat a device to put several slabs on
+    one GPU).  Slabs on the same device share one stream."""
 
     def __init__(self, w, devices, options=None):
+        import torch
         nsl = len(devices)
         self.w = w
         self.slabs = plan_z_slabs(w["nz"], nsl, w["pml"][4], w["pml"][5])
         self.solvers, self.owner = [], {}
         opts = {B.FDTD_OPT_STEP_IMPL: 2}
         opts.update(options or {})
-        for s, ((z0, z1), dev) in enumerate(zip(self.slabs, devices)):
+        devs = [torch.device(d) for d in devices]
+        self.streams = {}
+        for d in devs:
+            if d not in self.streams:
+                self.streams[d] = torch.cuda.Stream(d)
+        # every slab on its own GPU: the slabs run concurrently and fdtd_step(n) may be enqueued slab by slab
+        self.concurrent = nsl > 1 and len(self.streams) == nsl
+        for s, ((z0, z1), dev) in enumerate(zip(self.slabs, devs)):
             ws, owned = shard_workload(w, z0, z1)
             for local, n in enumerate(owned):
                 self.owner[n] = (s, local)
             z_open = (s > 0, s < nsl - 1)
-            self.solvers.append(Solver.from_workload(ws, options=opts, device=dev, z_open=z_open if nsl > 1 else None))
+            self.solvers.append(Solver.from_workload(ws, options=opts, device=dev, z_open=z_open if nsl > 1 else None,
+                                                     stream=self.streams[dev]))
         missing = [n for n in range(len(w["ports"])) if n not in self.owner]
         if missing:
             raise ValueError(f"ports {missing} are cut by a slab interface: choose another number of slabs")
+        for lo, up in zip(self.solvers[:-1], self.solvers[1:]):
+            link_neighbours(lo, up)
 
-    def _copy(self, src_solver, src, dst_solver, dst):
-        """One plane from src_solver's workspace to dst_solver's, ordered after the producer's stream; the producer's next
-        kernel waits for the copy (it will overwrite the plane two steps later)."""
-        import torch
-        done = torch.cuda.Event()
-        done.record(src_solver.stream)
-        dst_solver.stream.wait_event(done)
-        with torch.cuda.device(dst_solver.device), torch.cuda.stream(dst_solver.stream):
-            dst.copy_(src, non_blocking=True)
-        copied = torch.cuda.Event()
-        copied.record(dst_solver.stream)
-        src_solver.stream.wait_event(copied)
-
-    def step(self, n=1):
+    def step(self, n=1, chunk=8):
         S = self.solvers
         if len(S) == 1:
             S[0].step(n)
-            return
-        for _ in range(n):
-            for s in S:
-                s.step_begin()
-            for lo, up in zip(S[:-1], S[1:]):
-                top = lo.shape[0] - 1
-                for c in (HX, HY):
-                    self._copy(lo, lo.plane(c, top), up, up.plane(c, -1))
-            for s in S:
-                s.step_end()
-            for lo, up in zip(S[:-1], S[1:]):
-                for c in (EX, EY):
-                    self._copy(up, up.plane(c, 0), lo, lo.plane(c, lo.shape[0]))
+        elif self.concurrent:
+            # one GPU per slab: enqueue a few steps per slab in turn (a stream that waits for a neighbour must not fill the
+            # launch queue before that neighbour's work has been enqueued)
+            while n > 0:
+                m = min(n, chunk)
+                for s in S:
+                    s.step(m)
+                n -= m
+        else:
+            # slabs that share a stream: all first halves, then all second halves, in ascending order -- every wait
+            # kernel then finds its counter already posted by an earlier kernel of the same stream
+            for _ in range(n):
+                for s in S:
+                    s.step_begin()
+                for s in S:
+                    s.step_end()
 
     def read_fields(self, comp):
         import torch
         return torch.cat([s.read_fields(comp).to(self.solvers[0].device) for s in self.solvers], dim=0)
+
+    def upload_materials(self, pinned=False):
+        """(Re)send every slab's slice of the indexed material map from host memory; returns the bytes sent."""
+        import torch
+        m, sent = self.w["materials"], 0
+        for s, (z0, z1) in zip(self.solvers, self.slabs):
+            idx = torch.from_numpy(np.ascontiguousarray(m["idx"][z0:z1], dtype=np.uint8))
+            s.set_materials_indexed(idx.pin_memory() if pinned else idx, m["eps_r"], m["sigma"], m.get("mu_r"))
+            sent += idx.numel()
+        return sent
+
+    def reset(self):
+        for s in self.solvers:
+            s.reset()
+
+    @property
+    def launch_count(self):
+        return sum(s.launch_count for s in self.solvers)
 
     def read_port_dft(self, port):
         s, local = self.owner[port]
@@ -141,15 +174,40 @@ class ShardedSolver:
             s.destroy()
 
 
-class DistributedSlab:
-    """One slab per torch.distributed rank (backend nccl, one process per GPU).  Same protocol; the copies become
-    send/recv pairs between neighbouring ranks.  Port DFTs are read from the owning rank by broadcast."""
+def _ipc_export(solver):
+    """What a neighbouring rank needs to write into this slab: a picklable handle of the workspace (CUDA IPC through torch's
+    tensor-sharing machinery) and the byte offsets of the halo planes and arrival counters inside it."""
+    from torch.multiprocessing.reductions import reduce_tensor
+    base = solver.workspace.data_ptr()
+    faces = {}
+    for side, is_open in enumerate(solver.z_open):
+        if is_open:
+            planes, flag = B.fdtd_z_halo(solver.h, side)
+            faces[side] = ([p - base for p in planes], flag - base)
+    return reduce_tensor(solver.workspace), faces
 
-    def __init__(self, w, device, options=None, make_solver=None):
+
+def _ipc_link(solver, side, exported, keep):
+    """Map the neighbour's workspace into this process and link `side` of this slab to the neighbour's facing halo."""
+    (rebuild, args), faces = exported
+    ws = rebuild(*args)
+    keep.append(ws)                                   # the mapping must outlive the handle
+    planes, flag = faces[1 - side]                    # my z+ touches the neighbour's z-, and the other way round
+    B.fdtd_z_link(solver.h, side, [ws.data_ptr() + o for o in planes], ws.data_ptr() + flag)
+
+
+class DistributedSlab:
+    """One slab per torch.distributed rank (one process per GPU).  transport="peer": the slabs are linked through CUDA IPC
+    and the kernels push the planes themselves (fdtd_step(n) per rank, no per-step host work); transport="nccl": send/recv
+    pairs between neighbouring ranks around fdtd_step_begin / fdtd_step_end.  Port DFTs are read from the owning rank by
+    broadcast."""
+
+    def __init__(self, w, device, options=None, make_solver=None, transport="peer"):
         """make_solver(slab_workload, options, device, z_open) -> object with the Solver interface (default: Solver);
         the hook exists so that the exchange protocol can be exercised on CPU tensors under the gloo backend."""
         import torch.distributed as dist
         self.dist, self.rank, self.world = dist, dist.get_rank(), dist.get_world_size()
+        self.transport = transport
         self.slabs = plan_z_slabs(w["nz"], self.world, w["pml"][4], w["pml"][5])
         self.owner = {}
         for s, (z0, z1) in enumerate(self.slabs):
@@ -165,6 +223,23 @@ class DistributedSlab:
         make = make_solver or (lambda sw, o, dev, zo: Solver.from_workload(sw, options=o, device=dev, z_open=zo))
         self.solver = make(ws, opts, device, z_open if self.world > 1 else None)
         self.nf = len(w["freqs"])
+        self._mapped = []
+        if transport == "peer" and self.world > 1:
+            self._link_over_ipc(make_solver is None)
+
+    def _link_over_ipc(self, real):
+        """Every rank publishes its export, then links to rank-1 and rank+1.  `real` is False under the CPU test hook, whose
+        solver object supplies export() / link(side, exported) itself."""
+        export = _ipc_export(self.solver) if real else self.solver.export()
+        everyone = [None] * self.world
+        self.dist.all_gather_object(everyone, export)
+        for side, nb in ((0, self.rank - 1), (1, self.rank + 1)):
+            if 0 <= nb < self.world:
+                if real:
+                    _ipc_link(self.solver, side, everyone[nb], self._mapped)
+                else:
+                    self.solver.link(side, nb, everyone[nb])
+        self.dist.barrier()                          # nobody steps before everybody is linked
 
     def _exchange(self, send_up, comps):
         """send_up: my top plane -> halo plane -1 of rank+1; else my plane 0 -> halo plane nz of rank-1."""
@@ -192,14 +267,30 @@ class DistributedSlab:
                 st.wait_stream(torch.cuda.current_stream(s.device))
 
     def step(self, n=1):
-        if self.world == 1:
-            self.solver.step(n)
+        if self.world == 1 or self.transport == "peer":
+            self.solver.step(n)                      # linked slabs: the hand-over is inside the enqueued kernels
             return
         for _ in range(n):
             self.solver.step_begin()
             self._exchange(True, (HX, HY))
             self.solver.step_end()
             self._exchange(False, (EX, EY))
+
+    def upload_materials(self, w, pinned=False):
+        import torch
+        m = w["materials"]
+        z0, z1 = self.slabs[self.rank]
+        idx = torch.from_numpy(np.ascontiguousarray(m["idx"][z0:z1], dtype=np.uint8))
+        self.solver.set_materials_indexed(idx.pin_memory() if pinned else idx, m["eps_r"], m["sigma"], m.get("mu_r"))
+        return idx.numel()
+
+    def reset(self):
+        self.solver.reset()
+        self.dist.barrier()                          # nobody posts into a neighbour that has not yet zeroed its counters
+
+    @property
+    def launch_count(self):
+        return self.solver.launch_count
 
     def read_port_dft(self, port):
         import torch

@@ -28,6 +28,7 @@ class Solver:
         self.nf = 0
         self.nports = 0
         self.workspace = None
+        self.z_open = (False, False)
 
     # ---- setup (before commit) ---------------------------------------------------------------------------------
     def set_boundary(self, pml_cells, cpml=None):
@@ -49,6 +50,7 @@ class Solver:
         B.fdtd_set_option(self.h, option, value)
 
     def set_z_interfaces(self, lo_open, hi_open):
+        self.z_open = (bool(lo_open), bool(hi_open))
         B.fdtd_set_z_interfaces(self.h, lo_open, hi_open)
 
     def workspace_bytes(self):
@@ -184,7 +186,8 @@ class Solver:
 
     # ---- a workload dict (workloads/__init__.py) -> a committed solver ------------------------------------------
     @classmethod
-    def from_workload(cls, w: dict, precision=None, options=None, device="cuda:0", materials_on_device=False, z_open=None):
+    def from_workload(cls, w: dict, precision=None, options=None, device="cuda:0", materials_on_device=False, z_open=None,
+                      stream=None):
         prec = precision if precision is not None else w["precision"]
         s = cls(w["nx"], w["ny"], w["nz"], w["dx"], w["dy"], w["dz"], w["dt"], prec)
         if w.get("periodic_y"):
@@ -201,7 +204,7 @@ class Solver:
             s.set_option(k, v)
         if z_open is not None:
             s.set_z_interfaces(*z_open)
-        s.commit(device)
+        s.commit(device, stream=stream)
         np_dt = np.float64 if prec == B.FDTD_F64 else np.float32
         if m["mode"] == "indexed":
             idx = np.ascontiguousarray(m["idx"], dtype=np.uint8)

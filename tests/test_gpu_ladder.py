@@ -9,8 +9,8 @@
 Rung (ii) of SURVEY 8(d) -- reduced linear scale, FULL step count, S* formed (the method needs 1e5-1e6 steps,
 PAPER.md:116; SURVEY G31 flagged S*_11 at 200 k steps in fp32 as the risk):
   C2  1/4 scale (128x64x32), all 200 000 steps, inc + tot (via stub => a real S*_11), fp32 GPU in the configuration commit
-      selects and with the fused kernel forced, against the fp64 oracle: fields at 5 checkpoints, S*_11 and S*_21 over the
-      1-500 GHz band.  With FDTD_SLOW=1 also R14's yardstick: the oracle's own fp32 instantiation over the same 200 000 steps.
+      selects and with the fused kernel forced, against the fp64 oracle: fields at 6 checkpoints beside R14's yardstick (the
+      oracle's own fp32 instantiation over the same 200 000 steps), S*_11 and S*_21 over the 1-500 GHz band.
   C4  1/8 scale (128x64x32; 1/4 scale = 256x128x64 with FDTD_SLOW=1), all 50 000 steps, inc + tot, fp64 full coefficient
       arrays: fields 1e-11 at 5 checkpoints, raw DFTs 1e-11, S* column formed.
   C3  1/4 scale (384x192x192), all 2000 steps: fields at 5 checkpoints, raw DFTs, S* column.
@@ -135,17 +135,48 @@ def _s_column(inc, tot, nports, module):
     return np.array(module.s_star_column(0, list(Vi), list(Ii), list(Vt)))
 
 
+def _family_errors(sim_fields, o, emax, hmax):
+    """max|dE| / running max|E| and max|dH| / running max|H| of a six-component state against the oracle's."""
+    e = max(np.abs(sim_fields(c) - o.read_field(c)).max() for c in range(3)) / emax
+    h = max(np.abs(sim_fields(c) - o.read_field(c)).max() for c in range(3, 6)) / hmax
+    return e, h
+
+
 def test_C2_quarter_scale_full_200k_steps_sparams():
-    cps = [2000, 20000, 60000, 120000, 200000]
+    """What this rung measures (numbers in profiles/r02_ladder.md): the GAUSS pulse leaves a static charge on the copper
+    lines, so E stays at ~0.95 of its running maximum for the rest of the run, and fp32 storage of that static field has
+    a frozen rounding pattern whose discrete curl is not zero: H drifts linearly in ANY fp32 time stepping -- the
+    oracle's own fp32 instantiation (R14's yardstick, same algorithm and order on the CPU) is 0.4 of max|H| away from
+    its fp64 run after 200 000 steps, E 1e-3 of max|E|.  The 1e-4 field bar is therefore asserted while it is reachable
+    (the 500-step checkpoint) and, later, the GPU is held to the yardstick: it may not be further from the fp64 oracle
+    than a small multiple of what fp32 time stepping itself loses.  S* -- a ratio of DFTs of the same run, Eq. 1 -- is
+    graded at the full 200 000 steps against north_star's 1e-3."""
+    cps = [500, 2000, 20000, 60000, 120000, 200000]
     opts = {"auto": None, "fused": {FDTD_OPT_STEP_IMPL: 2}}
     sims = {}
     for run in ("inc", "tot"):
         w = W.interconnect_c2(run=run, div=4)
         assert (w["nx"], w["ny"], w["nz"], w["steps"], len(w["freqs"])) == (128, 64, 32, 200000, 256)
-        o, gpus, worst = _run_to_checkpoints(w, opts, cps, FDTD_F32)
-        print(f"C2/4 {run} 200k steps: field_err " + ", ".join(f"{k} ({g.impl_name}) {worst[k]:.3e}" for k, g in gpus.items()))
-        assert max(worst.values()) <= TOL[FDTD_F32], worst
-        sims[run] = (o, gpus, w)
+        o = YeeOracle.from_workload(w, track_max=True)
+        o32 = YeeOracle.from_workload(w, f32=True)
+        gpus = {name: Solver.from_workload(w, options=op) for name, op in opts.items()}
+        done = 0
+        for cp in cps:
+            o.step(cp - done); o32.step(cp - done)
+            for g in gpus.values():
+                g.step(cp - done)
+            done = cp
+            emax, hmax = o.running_max()
+            ye, yh = _family_errors(o32.read_field, o, emax, hmax)
+            line = f"C2/4 {run} step {cp}: fp32-oracle yardstick dE {ye:.2e} dH {yh:.2e};"
+            for name, g in gpus.items():
+                ge, gh = _family_errors(lambda c: g.read_fields(c).cpu().numpy().astype(np.float64), o, emax, hmax)
+                line += f" {name} ({g.impl_name}) dE {ge:.2e} dH {gh:.2e};"
+                if cp <= 500:
+                    assert max(ge, gh) <= TOL[FDTD_F32], (name, cp, ge, gh)
+                assert ge <= 5 * ye + TOL[FDTD_F32] and gh <= 5 * yh + TOL[FDTD_F32], (name, cp, ge, gh, ye, yh)
+            print(line)
+        sims[run] = (o, gpus, o32)
     So = _s_column(sims["inc"][0], sims["tot"][0], 2, osp)
     assert np.abs(So[0]).max() > 1e-2, "the via stub must reflect: S*_11 of this test is meant to be non-trivial"
     Vo, Io = _dfts(sims["tot"][0], 2)
@@ -157,17 +188,11 @@ def test_C2_quarter_scale_full_200k_steps_sparams():
         print(f"C2/4 200k steps {name}: |dS*_11| = {d11:.3e}, |dS*_21| = {d21:.3e} (max|S*_11| = {np.abs(So[0]).max():.3f}, "
               f"max|S*_21| = {np.abs(So[1]).max():.3f}); raw fp32 DFT drift (V, I) = ({raw[0]:.3e}, {raw[1]:.3e}), informational (R14)")
         assert d11 <= 1e-3 and d21 <= 1e-3
-    if SLOW:   # R14's yardstick: what fp32 time stepping itself loses over 200 000 steps (same algorithm, same order, on the CPU)
-        y = {}
-        for run in ("inc", "tot"):
-            o32 = YeeOracle.from_workload(sims[run][2], f32=True)
-            o32.step(200000)
-            y[run] = o32
-        S32 = _s_column(y["inc"], y["tot"], 2, osp)
-        V32, I32 = _dfts(y["tot"], 2)
-        print(f"C2/4 200k steps yardstick (fp32 oracle vs fp64 oracle): |dS*_11| = {np.abs(So[0] - S32[0]).max():.3e}, "
-              f"|dS*_21| = {np.abs(So[1] - S32[1]).max():.3e}, raw DFT (V, I) = ({np.abs(V32 - Vo).max() / np.abs(Vo).max():.3e}, "
-              f"{np.abs(I32 - Io).max() / np.abs(Io).max():.3e})")
+    S32 = _s_column(sims["inc"][2], sims["tot"][2], 2, osp)
+    V32, I32 = _dfts(sims["tot"][2], 2)
+    print(f"C2/4 200k steps yardstick (fp32 oracle vs fp64 oracle): |dS*_11| = {np.abs(So[0] - S32[0]).max():.3e}, "
+          f"|dS*_21| = {np.abs(So[1] - S32[1]).max():.3e}, raw DFT (V, I) = ({np.abs(V32 - Vo).max() / np.abs(Vo).max():.3e}, "
+          f"{np.abs(I32 - Io).max() / np.abs(Io).max():.3e})")
     for _, gpus, _ in sims.values():
         for g in gpus.values():
             g.destroy()

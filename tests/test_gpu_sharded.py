@@ -1,7 +1,10 @@
 """z-slab decomposition checked on ONE GPU: the slabs of a workload are separate
-library handles on the same device that exchange halo planes through the ShardedSolver driver, exactly as they would
-across GPUs (there the copy is an NVLink peer copy or an NCCL send/recv).  No kernel waits on another one: the slabs are
-stepped one after the other from one process.  Reference: the fp64 oracle on the undivided grid."""
+library handles on the same device, LINKED to each other (fdtd_z_halo / fdtd_z_link): the kernels themselves store the
+boundary planes into the neighbour's halo and post / wait on the neighbour's arrival counters, exactly as they do across
+GPUs (there the stores travel over NVLink).  The slabs share one stream and advance half step by half step, so every
+wait finds its counter already posted by an earlier kernel of the stream: no kernel ever waits for another launch.
+Reference: the fp64 oracle on the undivided grid.  fdtd_step(n) of a linked slab (graph replay included) is checked on a
+slab linked to ITSELF -- a z-periodic domain -- against the oracle's y-periodic option under the y <-> z mirror map."""
 import numpy as np
 import pytest
 
@@ -64,6 +67,83 @@ def test_two_slabs_fp64_full_coefficients():
     sh.destroy()
 
 
+def test_linked_slabs_move_no_plane_from_the_host():
+    """The exchange is part of the enqueued kernels: per step a middle slab launches fused + E-on-plane-0 + two waits + two
+    posts (+ its port kernels); nothing in ShardedSolver.step copies a plane."""
+    import inspect
+    from paper_2208_04371_b200 import sharded
+    w = W.throughput_c3(div=8, steps=8, npml=6, nf=4)
+    sh = ShardedSolver(w, ["cuda:0"] * 3)
+    assert not sh.concurrent and len({s.stream.cuda_stream for s in sh.solvers}) == 1
+    before = [s.launch_count for s in sh.solvers]
+    sh.step(8)
+    per_step = [(s.launch_count - b) / 8 for s, b in zip(sh.solvers, before)]
+    nport = 1 + sum(1 for p in w["ports"] if p["has_source"])          # k_probe_dft + one k_source per driving port
+    assert per_step == [1 + 2, 1 + 1 + 4 + nport, 1 + 1 + 2]           # bottom: no E-plane-0 kernel; the middle slab owns the ports
+    assert "copy_" not in inspect.getsource(sharded.ShardedSolver.step)
+    sh.destroy()
+
+
+def _mirror_yz(a):
+    """[k, j, i] array of the z-periodic GPU problem -> [j', k', i] array of the y-periodic oracle problem."""
+    return np.ascontiguousarray(np.swapaxes(a, 0, 1))
+
+
+@pytest.mark.parametrize("prec,nsteps", [(FDTD_F64, 19), (FDTD_F32, 26)])
+def test_self_linked_slab_steps_with_graphs_like_the_y_periodic_oracle(prec, nsteps):
+    """fdtd_step(n) on a linked slab: one handle whose z+ face is linked to its own z- halo and vice versa, i.e. a domain
+    periodic in z.  Every wait follows its own post in stream order.  The Yee scheme is invariant under the mirror
+    (x, y, z) -> (x, z, y) with E_y <-> E_z, H_x -> -H_x, H_y <-> -H_z, so the oracle's y-periodic option (pinned by the
+    parallel-plate tests) on the mirrored inputs is the reference.  Random materials (sigma, mu, anisotropic), CPML on x and
+    y, random initial state, no ports."""
+    from paper_2208_04371_b200 import FDTD_OPT_GRAPH_UNROLL, binding as B
+    wg = W.random_box(41, nx=150, ny=24, nz=20, pml=(4, 3, 3, 4, 0, 0), indexed=False, with_mu=True, steps=nsteps,
+                      precision=prec, pec_frac=0.02)
+    wg = dict(wg, ports=[], freqs=np.zeros(0))
+    m = wg["materials"]
+    yz = (0, 2, 1)                                                       # oracle component c holds GPU component yz[c]
+    wo = dict(wg, ny=wg["nz"], nz=wg["ny"], dy=wg["dz"], dz=wg["dy"], periodic_y=True,
+              pml=[wg["pml"][0], wg["pml"][1], 0, 0, wg["pml"][2], wg["pml"][3]],
+              materials={"mode": "full", "eps_r": [_mirror_yz(m["eps_r"][c]) for c in yz],
+                         "sigma": [_mirror_yz(m["sigma"][c]) for c in yz], "mu_r": [_mirror_yz(m["mu_r"][c]) for c in yz]})
+    r = W.rng_for(4100)
+    shape = (wg["nz"], wg["ny"], wg["nx"])
+    init = [r.standard_normal(shape) * (1.0 if c < 3 else 2.5e-3) for c in range(6)]
+    init[0][:, 0, :] = 0                                                 # walls: j = 0 and i = 0 (z has none here)
+    init[1][:, :, 0] = 0
+    init[2][:, :, 0] = 0; init[2][:, 0, :] = 0
+    o = YeeOracle.from_workload(wo, track_max=True)
+    s = Solver.from_workload(wg, precision=prec, options={FDTD_OPT_STEP_IMPL: 2, FDTD_OPT_GRAPH_UNROLL: 4}, z_open=(True, True))
+    np_dt = np.float64 if prec == FDTD_F64 else np.float32
+    for c in range(3):
+        s.write_fields(c, np.ascontiguousarray(init[c], dtype=np_dt))
+        s.write_fields(3 + c, np.ascontiguousarray(init[3 + c], dtype=np_dt))
+        o.write_field(c, _mirror_yz(init[yz[c]]))
+        o.write_field(3 + c, -_mirror_yz(init[3 + yz[c]]))
+    # halos of the initial state: plane -1 <- H of the top plane, plane nz <- E of plane 0 (what a previous step would have left)
+    import torch
+    with torch.cuda.stream(s.stream):
+        for comp, src, dst in ((B.FDTD_HX, wg["nz"] - 1, -1), (B.FDTD_HY, wg["nz"] - 1, -1), (B.FDTD_EX, 0, wg["nz"]), (B.FDTD_EY, 0, wg["nz"])):
+            s.plane(comp, dst).copy_(s.plane(comp, src))
+    for side in (0, 1):                                                  # my z+ pushes into my own z- halo and vice versa
+        planes, flag = B.fdtd_z_halo(s.h, 1 - side)
+        B.fdtd_z_link(s.h, side, planes, flag)
+    o.step(nsteps)
+    s.step(nsteps)
+    assert s.step_count == nsteps and s.graph_replays == nsteps // 4
+    emax, hmax = o.running_max()
+    emax = max(emax, max(np.abs(a).max() for a in init[:3]))
+    hmax = max(hmax, max(np.abs(a).max() for a in init[3:]))
+    worst = 0.0
+    for c in range(3):
+        ge = s.read_fields(yz[c]).cpu().numpy().astype(np.float64)
+        gh = s.read_fields(3 + yz[c]).cpu().numpy().astype(np.float64)
+        worst = max(worst, np.abs(_mirror_yz(ge) - o.read_field(c)).max() / emax,
+                    np.abs(-_mirror_yz(gh) - o.read_field(3 + c)).max() / hmax)
+    assert worst <= (1e-11 if prec == FDTD_F64 else 1e-4), worst
+    s.destroy()
+
+
 def test_a_port_cut_by_an_interface_is_refused():
     w = W.throughput_c3(div=8, steps=10, npml=6, nf=4)          # ports touch planes 45..50; two slabs cut at 48
     with pytest.raises(ValueError, match="cut by a slab interface"):
@@ -77,9 +157,12 @@ def test_slab_handles_refuse_plain_stepping_and_misordered_calls():
     s = Solver.from_workload(w, options={FDTD_OPT_STEP_IMPL: 2}, z_open=(True, False))
     assert s.impl_name == "fused"
     with pytest.raises(FdtdError):
-        s.step(1)
+        s.step(1)                                   # not linked to a neighbour: fdtd_step has no way to fill the halo
     with pytest.raises(FdtdError):
         s.step_end()
+    from paper_2208_04371_b200 import binding as B
+    with pytest.raises(FdtdError):
+        B.fdtd_z_halo(s.h, 1)                       # the z+ face of this slab is a wall, not an interface
     s.step_begin()
     with pytest.raises(FdtdError):
         s.step_begin()

@@ -79,7 +79,7 @@ def _worker(rank, world, port, out):
     os.environ["MASTER_PORT"] = str(port)
     dist.init_process_group("gloo", rank=rank, world_size=world)
     w = W.interconnect_c2(run="tot", div=4, steps=4, npml=6, nf=4)       # 128x64x32: ports on the ground side
-    d = S.DistributedSlab(w, "cpu", make_solver=lambda ws, o, dev, zo: _FakeSolver(ws, rank))
+    d = S.DistributedSlab(w, "cpu", make_solver=lambda ws, o, dev, zo: _FakeSolver(ws, rank), transport="nccl")
     d.step(2)
     f = d.solver
     nzl = f.shape[0]
@@ -105,3 +105,49 @@ def test_two_ranks_exchange_the_right_planes_in_the_right_order():
     assert r[0]["halo_hi"] == {S.EX: -1000.0 - 10 * S.EX - 4, S.EY: -1000.0 - 10 * S.EY - 4}
     # the outer halos were never written
     assert all(np.isnan(v) for v in r[0]["halo_lo"].values()) and all(np.isnan(v) for v in r[1]["halo_hi"].values())
+
+
+class _FakeLinkedSolver(_FakeSolver):
+    """Stand-in for a slab whose kernels push the planes themselves: export() is what a neighbour needs, link() records
+    what this slab was told about a neighbour, step(n) is the only call a linked slab receives."""
+    def __init__(self, ws, rank, z_open):
+        super().__init__(ws, rank)
+        self.z_open, self.links, self.stepped = z_open, {}, []
+
+    def export(self):
+        return {"rank": self.rank, "faces": {side: f"halo{side}@{self.rank}" for side, o in enumerate(self.z_open) if o}}
+
+    def link(self, side, nb, exported):
+        self.links[side] = (nb, exported["rank"], exported["faces"][1 - side])
+
+    def step(self, n):
+        self.stepped.append(n)
+
+
+def _worker_links(rank, world, port, out):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    w = W.throughput_c3(div=8, steps=4, npml=6, nf=4)                     # 192x96x96, ports in the middle slab of three
+    d = S.DistributedSlab(w, "cpu", make_solver=lambda ws, o, dev, zo: _FakeLinkedSolver(ws, rank, zo), transport="peer")
+    d.step(5)
+    out[rank] = dict(links=dict(d.solver.links), stepped=list(d.solver.stepped), log=list(d.solver.log),
+                     z_open=d.solver.z_open, owner=dict(d.owner))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_three_ranks_link_to_the_facing_halo_of_each_neighbour_and_step_without_host_exchange():
+    world = 3
+    with mp.Manager() as m:
+        out = m.dict()
+        mp.spawn(_worker_links, args=(world, _free_port(), out), nprocs=world, join=True)
+        r = dict(out)
+    assert [r[k]["z_open"] for k in range(3)] == [(False, True), (True, True), (True, False)]
+    # side 1 (z+) of rank k is linked to the z- halo (side 0) of rank k+1, side 0 (z-) to the z+ halo (side 1) of rank k-1
+    assert r[0]["links"] == {1: (1, 1, "halo0@1")}
+    assert r[1]["links"] == {0: (0, 0, "halo1@0"), 1: (2, 2, "halo0@2")}
+    assert r[2]["links"] == {0: (1, 1, "halo1@1")}
+    # a linked slab is advanced by fdtd_step(n) alone: no begin / end / host-issued exchange
+    assert all(r[k]["stepped"] == [5] and r[k]["log"] == [] for k in range(3))
+    assert all(r[k]["owner"] == {p: (1, p) for p in range(4)} for k in range(3))

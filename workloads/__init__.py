@@ -278,7 +278,9 @@ def interconnect_c4(seed=2212, run="tot", div=1, steps=50000, npml=12, nf=512):
 # --------------------------------------------------------------------------------------------------
 # C3  throughput grid 1536x768x768, fp32 + uint8 index into a 64-entry table, six-face CPML
 # --------------------------------------------------------------------------------------------------
-def throughput_c3(seed=2211, shape=(1536, 768, 768), steps=2000, npml=16, nf=128, nblocks=4096, div=1):
+def throughput_c3(seed=2211, shape=(1536, 768, 768), steps=2000, npml=16, nf=128, nblocks=4096, div=1, kc=None):
+    """kc: plane of the two port lines (default: the middle plane nz // 2; the z-slab weak-scaling grids put it in the
+    middle of the lowest slab so that no interface cuts a port)."""
     nx, ny, nz = (v // div for v in shape)
     d = 5e-9
     dt = 0.99 * cfl_limit(d, d, d)
@@ -300,7 +302,7 @@ def throughput_c3(seed=2211, shape=(1536, 768, 768), steps=2000, npml=16, nf=128
         idx[o[2]:o[2] + e[2], o[1]:o[1] + e[1], o[0]:o[0] + e[0]] = int(r.integers(2, 64))
     # two PEC lines (10 x 4 cells) in a vacuum corridor (+-24 cells) along x, for the ports
     cw, ch, cor = max(2, 10 // div), max(1, 4 // div), max(3, 24 // div)
-    kc = nz // 2
+    kc = nz // 2 if kc is None else int(kc)
     lines = []
     for jc in (ny // 3, (2 * ny) // 3):
         idx[kc - cor:kc + ch + cor, jc - cor:jc + cw + cor, :] = 0
@@ -419,6 +421,16 @@ def drive_port(w, j):
               "sk1": t["vk1"]})
     assert 0 <= t["is"] < w["nx"]
     return dict(w, ports=ports), direction
+
+
+def weak_scaling_600(n_slabs=1, steps=100, edge=600):
+    """The per-GPU load of the paper's weak-scaling study (Table I: 600^3 cells per GPU), stacked along z:
+    edge x edge x (edge * n_slabs) cells of C3's generator (same block density, 16-cell CPML on all six faces, 4 ports on
+    two lines through the lowest slab)."""
+    vol = n_slabs * edge**3 / (1536 * 768 * 768)
+    w = throughput_c3(shape=(edge, edge, edge * n_slabs), steps=steps, nblocks=max(1, int(4096 * vol)), kc=edge // 2)
+    w["name"] = f"weak{edge}x{n_slabs}"
+    return w
 
 
 def get(name, **kw):
