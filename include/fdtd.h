@@ -59,7 +59,11 @@ enum {
                                1 = two-pass (H kernel, E kernel, in place),
                                2 = fused E+H kernel (temporal blocking over the half steps; a second field set),
                                3 = persistent: fdtd_step(n) is one cooperative launch per 4096 steps, with grid-wide
-                                   barriers between the half steps (grids that live in L2; the arithmetic of 1)         */
+                                   barriers between the half steps (grids that live in L2; the arithmetic of 1),
+                               4 = two steps per pass: a box of cells that keeps two cells' distance from the CPML
+                                   layers and the port planes is advanced TWO steps by one kernel (every field read and
+                                   written once per two steps), the shell around it step by step with the kernels of 1;
+                                   fdtd_commit returns FDTD_EINVAL when the grid leaves no such box; a second field set */
   FDTD_OPT_USE_GRAPH = 2,   /* 1 (default) = replay a captured CUDA graph per FDTD_OPT_GRAPH_UNROLL steps; 0 = plain launches.
                                Capture needs a real stream: on the NULL (legacy default) stream fdtd_step always issues
                                plain launches (fdtd_graph_replays() stays 0)                                             */
@@ -139,6 +143,8 @@ int fdtd_step(fdtd_t*, long n);
  * the kernels, and return the average device time per step, in milliseconds, of
  *   ms_avg[0] = H pass (or the fused E+H kernel), ms_avg[1] = E pass (0 when fused), ms_avg[2] = source injection,
  *   ms_avg[3] = probes + DFT.   This is the measurement hook of bench.py's roofline line.  Synchronises the stream.
+ * With FDTD_OPT_STEP_IMPL = 4 the steps run in pairs (n is rounded up to even): ms_avg[0] = the two-step box kernel,
+ * ms_avg[1] = the shell passes with their port kernels, both per step; ms_avg[2] = ms_avg[3] = 0.
  * FDTD_ESTATE on a z slab (fdtd_set_z_interfaces) or between fdtd_step_begin and fdtd_step_end. */
 int fdtd_profile_step(fdtd_t*, long n, double ms_avg[4]);
 

@@ -5,6 +5,7 @@
 // step of the method runs in the kernels of fdtd_kernels.cuh / fdtd_fused.cuh.  There is no CPU fallback.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -22,6 +23,7 @@
 #include "fdtd_kernels.cuh"
 #include "fdtd_params.h"
 #include "fdtd_persistent.cuh"
+#include "fdtd_step2.cuh"
 
 using namespace fdtd_b200;
 
@@ -158,6 +160,10 @@ struct Solver : fdtd {
   PortParams<T> pp2{};
   // fused step: two field sets (ping-pong); fpar[c] reads set c and writes set 1-c; cur = set holding the current state
   bool fused = false;
+  bool two_step = false;     // two steps per pass over a box + one-step kernels on the shell around it (fdtd_step2.cuh)
+  Step2Params<T> s2par[2];   // s2par[c] reads set c, writes set 1 - c
+  int box[6] = {0, 0, 0, 0, 0, 0};   // bx0 bx1 by0 by1 bz0 bz1
+  bool has_shell = false;
   bool persistent = false;   // small grids: many steps per cooperative launch (fdtd_persistent.cuh)
   int persist_blocks = 0;
   int cur = 0;
@@ -175,6 +181,7 @@ struct Solver : fdtd {
   std::vector<T> h_vec[18];
   cudaGraphExec_t gexec = nullptr;
   int graph_steps = 0;
+  long graph_nodes = 0;        // kernel launches inside one captured graph (counted while capturing)
 
   ~Solver() override {
     if (gexec) cudaGraphExecDestroy(gexec);
@@ -182,7 +189,9 @@ struct Solver : fdtd {
   }
   // auto: the fused kernel pays off once the grid no longer fits in L2 (small grids are launch-bound)
   bool slabs_fit() const { return Sp(0) <= kMaxSlab && S(1) <= kMaxSlab && S(2) <= kMaxSlab; }
-  bool want_fused() const { return slabs_fit() && (opt_impl == 2 || z_lo_open || z_hi_open || (opt_impl == 0 && (long long)nx * ny * nz >= (4LL << 20))); }
+  bool want_two_step() const { return opt_impl == 4 && !z_lo_open && !z_hi_open; }
+  bool two_sets() const { return want_fused() || want_two_step(); }
+  bool want_fused() const { return opt_impl != 4 && slabs_fit() && (opt_impl == 2 || z_lo_open || z_hi_open || (opt_impl == 0 && (long long)nx * ny * nz >= (4LL << 20))); }
 
   int mode() const { return (mat_mode == FDTD_MAT_FULL ? kModeFull : 0) | (has_mu ? kModeMu : 0); }
   size_t psi_elems(int a) const {
@@ -202,7 +211,7 @@ struct Solver : fdtd {
     auto take = [&](size_t bytes) { const size_t o = off; off += align_up(bytes, 256); return o; };
     const size_t fbytes = (size_t)cells_padded() * sizeof(T);
     for (int f = 0; f < 6; ++f) c.field[f] = take(fbytes);
-    if (want_fused()) for (int f = 0; f < 6; ++f) c.field2[f] = take(fbytes);
+    if (two_sets()) for (int f = 0; f < 6; ++f) c.field2[f] = take(fbytes);
     if (mat_mode == FDTD_MAT_INDEXED) {
       c.idx = take((size_t)cells_padded());
       c.tab = take(kTabWords * sizeof(T));
@@ -256,9 +265,18 @@ struct Solver : fdtd {
   int read_port_dft(int port, double* V, double* I) override;
   int read_port_last(int port, double* V, double* I) override;
   int reset() override;
-  const char* impl_name() const override { return fused ? "fused" : (persistent ? "persistent" : "two_pass"); }
-  int fused_kz() const override { return fused ? kz : 0; }
+  const char* impl_name() const override { return two_step ? "two_step" : (fused ? "fused" : (persistent ? "persistent" : "two_pass")); }
+  int fused_kz() const override { return (fused || two_step) ? kz : 0; }
   int build_fused();
+  int build_step2();
+  void enqueue_pair(cudaEvent_t* ev = nullptr);
+  void enqueue_steps(long count);
+  void shell_pass(bool isH, int d, const StepParams<T>& base, bool bump);
+  StepParams<T> sp_of(int set) const {
+    StepParams<T> q = sp;
+    for (int f = 0; f < 6; ++f) q.src[f] = q.dst[f] = field_origin(f, set);
+    return q;
+  }
   int autotune();
   int autotune_kz_only() { const long keep = opt_impl; opt_impl = 2; const int r = autotune(); opt_impl = keep; return r; }
   int setup_persistent();
@@ -410,7 +428,15 @@ int Solver<T>::commit(void* w, size_t bytes, void* st) {
     return fail(FDTD_EINVAL, "fdtd_commit: a z slab (fdtd_set_z_interfaces) runs the fused step only (CPML <= %d cells per axis)", kMaxSlab);
   pp2 = pp;
   fused = want_fused();
+  two_step = want_two_step();
   cur = 0;
+  if (opt_impl == 4 && !two_step) return fail(FDTD_EINVAL, "fdtd_commit: FDTD_OPT_STEP_IMPL = 4 (two steps per pass) does not run on a z slab");
+  if (two_step) {
+    pp2.Ez = field_origin(kEz, 1); pp2.Hy = field_origin(kHy, 1); pp2.Hz = field_origin(kHz, 1);
+    kz = opt_kz > 0 ? (int)opt_kz : 24;
+    const int r = build_step2();
+    if (r != FDTD_OK) return r;
+  }
   if (fused) {
     pp2.Ez = field_origin(kEz, 1); pp2.Hy = field_origin(kHy, 1); pp2.Hz = field_origin(kHz, 1);
     kz = opt_kz > 0 ? (int)opt_kz : 32;
@@ -446,7 +472,7 @@ int Solver<T>::commit(void* w, size_t bytes, void* st) {
     const int r = autotune();
     if (r != FDTD_OK) return r;
   }
-  if (!fused && (opt_impl == 0 || opt_impl == 3)) {
+  if (!fused && !two_step && (opt_impl == 0 || opt_impl == 3)) {
     const int r = setup_persistent();
     if (r != FDTD_OK) return r;
   }
@@ -705,8 +731,23 @@ int Solver<T>::autotune() {
   int best_kz = kz;
   bool best_fused = true;
   if (opt_kz <= 0) {
-    const int cand[7] = {8, 12, 16, 20, 24, 32, 48};
-    for (int c = 0; c < 7; ++c) {
+    // the fixed ladder, plus -- for grids that give the SMs only a few waves of blocks -- the chunk lengths whose block count
+    // comes closest to whole waves (C2: 76 tiles; 10-plane chunks make 6.7 waves where 16-plane chunks make 4.1)
+    std::vector<int> cand = {8, 12, 16, 20, 24, 32, 48};
+    {
+      const long long tiles = (long long)fpar[0].ntx * fpar[0].nty;
+      std::vector<std::pair<double, int>> fit;
+      for (int q = 6; q <= 48 && q <= nz; ++q) {
+        const double waves = (double)(tiles * ((nz + q - 1) / q)) / sm_count;
+        if (waves > 24.0) continue;
+        fit.push_back({-(waves / std::ceil(waves)) * q / (q + 2.5), q});   // wave fill x (planes owned / planes loaded)
+      }
+      std::sort(fit.begin(), fit.end());
+      for (size_t q = 0; q < fit.size() && q < 3; ++q)
+        if (std::find(cand.begin(), cand.end(), fit[q].second) == cand.end()) cand.push_back(fit[q].second);
+      std::sort(cand.begin(), cand.end());
+    }
+    for (size_t c = 0; c < cand.size(); ++c) {
       if (cand[c] > nz && c > 0) break;
       kz = cand[c] > nz ? nz : cand[c];
       fpar[0].kz = fpar[1].kz = kz;
@@ -833,6 +874,178 @@ int Solver<T>::setup_persistent() {
   return FDTD_OK;
 }
 
+// ---- two steps per pass (fdtd_step2.cuh): the box, its tensor maps, the shell passes ----------------------------------------
+#ifndef FDTD_STEP2_R
+#define FDTD_STEP2_R 11
+#endif
+#ifndef FDTD_STEP2_NS
+#define FDTD_STEP2_NS 3
+#endif
+static_assert(Step2Cfg<float, FDTD_STEP2_R, FDTD_STEP2_NS>::SMEM <= 232448 && Step2Cfg<double, FDTD_STEP2_R, FDTD_STEP2_NS>::SMEM <= 232448,
+              "two-step kernel: rows x stages exceed the 227 KB shared memory of an sm_100 CTA");
+template <typename T, int MODE>
+static cudaError_t step2_set_attr() {
+  using C = Step2Cfg<T, FDTD_STEP2_R, FDTD_STEP2_NS>;
+  return cudaFuncSetAttribute(k_step2<T, MODE, C::R, C::NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM);
+}
+template <typename T, int MODE>
+static void step2_launch(const Step2Params<T>& q, cudaStream_t st) {
+  using C = Step2Cfg<T, FDTD_STEP2_R, FDTD_STEP2_NS>;
+  const long long blocks = (long long)q.ntx * q.nty * ((q.bz1 - q.bz0 + q.kz - 1) / q.kz);
+  k_step2<T, MODE, C::R, C::NS><<<(unsigned)blocks, C::THREADS, C::SMEM, st>>>(q);
+}
+
+// The box that advances two steps per pass: every cell at least two cells away from every CPML cell and from every source
+// sample, and not on a port plane (the probes of the intermediate step read the shell's arrays; fdtd_step2.cuh).  Ports are
+// kept out by x ranges: a transmission line's ports sit near its two ends (Fig. 1a).
+template <typename T>
+int Solver<T>::build_step2() {
+  using C = Step2Cfg<T, FDTD_STEP2_R, FDTD_STEP2_NS>;
+  constexpr int V = C::V;
+  auto enc = tensor_map_encoder();
+  if (!enc) return fail(FDTD_ECUDA, "fdtd_commit: the driver does not export cuTensorMapEncodeTiled (two-step kernel needs TMA)");
+  cudaError_t e = cudaSuccess;
+  switch (mode()) {
+    case 0: e = step2_set_attr<T, 0>(); break;
+    case 1: e = step2_set_attr<T, 1>(); break;
+    case 2: e = step2_set_attr<T, 2>(); break;
+    default: e = step2_set_attr<T, 3>(); break;
+  }
+  if (e != cudaSuccess) return cuda_fail(e, "fdtd_commit: shared memory opt-in of the two-step kernel");
+  {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sm_count < 1)
+      return cuda_fail(cudaGetLastError(), "fdtd_commit: SM count");
+  }
+  auto up = [](int v, int m) { return (v + m - 1) / m * m; };
+  auto down = [](int v, int m) { return v / m * m; };
+  int b[6];
+  b[0] = npml[0] ? up(npml[0] + 2, V) : 0;  b[1] = npml[1] ? down(nx - npml[1] - 2, V) : nx;
+  b[2] = npml[2] ? npml[2] + 2 : 0;         b[3] = npml[3] ? ny - npml[3] - 2 : ny;
+  b[4] = npml[4] ? npml[4] + 2 : 0;         b[5] = npml[5] ? nz - npml[5] - 2 : nz;
+  for (const PortDev& d : ports) {
+    if (d.ip < nx / 2) b[0] = std::max(b[0], up(std::max(d.has_source ? d.is + 2 : 0, d.ip + 1), V));
+    else               b[1] = std::min(b[1], down(std::min(d.has_source ? d.is - 1 : nx, d.ip), V));
+    if (d.has_source && ((d.ip < nx / 2) != (d.is < nx / 2)))
+      return fail(FDTD_EINVAL, "fdtd_commit: FDTD_OPT_STEP_IMPL = 4 needs every source on the same side of the grid as its port plane");
+  }
+  if (b[1] - b[0] < 8 * V || b[3] - b[2] < 8 || b[5] - b[4] < 8)
+    return fail(FDTD_EINVAL, "fdtd_commit: FDTD_OPT_STEP_IMPL = 4: no box of at least %d x 8 x 8 cells keeps two cells' distance from the "
+                             "CPML layers and the port planes of this grid", 8 * V);
+  for (int q = 0; q < 6; ++q) box[q] = b[q];
+  has_shell = b[0] > 0 || b[1] < nx || b[2] > 0 || b[3] < ny || b[4] > 0 || b[5] < nz;
+  if (kz > b[5] - b[4]) kz = b[5] - b[4];
+  if (kz < 1) kz = 1;
+
+  const cuuint64_t gdim[3] = {(cuuint64_t)pitch(), (cuuint64_t)(ny + 1), (cuuint64_t)(nz + 2)};
+  const cuuint32_t estr[3] = {1, 1, 1};
+  auto make = [&](CUtensorMap* tm, void* base, CUtensorMapDataType dt, size_t es, int bx, int by) -> bool {
+    const cuuint64_t gstr[2] = {(cuuint64_t)pitch() * es, (cuuint64_t)plane() * es};
+    const cuuint32_t bx3[3] = {(cuuint32_t)bx, (cuuint32_t)by, 1};
+    return enc(tm, dt, 3, base, gdim, gstr, bx3, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+               CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+  };
+  const CUtensorMapDataType fdt = sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
+  for (int c = 0; c < 2; ++c) {
+    Step2Params<T>& q = s2par[c];
+    q.sp = sp;
+    for (int f = 0; f < 6; ++f) { q.sp.src[f] = field_origin(f, c); q.sp.dst[f] = field_origin(f, 1 - c); }
+    q.kz = kz;
+    q.ntx = (b[1] - b[0] + C::TXO - 1) / C::TXO; q.nty = (b[3] - b[2] + C::TYO - 1) / C::TYO;
+    q.group = q.ntx <= sm_count ? (sm_count / q.ntx) * q.ntx : sm_count;
+    if (q.group > q.ntx * q.nty) q.group = q.ntx * q.nty;
+    q.bx0 = b[0]; q.bx1 = b[1]; q.by0 = b[2]; q.by1 = b[3]; q.bz0 = b[4]; q.bz1 = b[5];
+    q.bump = has_shell ? 0 : 1;
+    for (int f = 0; f < 6; ++f)
+      if (!make(&q.tm[f], ws + (c ? cv.field2[f] : cv.field[f]), fdt, sizeof(T), C::xw(f), C::nr(f)))
+        return fail(FDTD_ECUDA, "fdtd_commit: cuTensorMapEncodeTiled failed for field %d (two-step kernel)", f);
+    q.tm[6] = q.tm[0];   // unused: the two-step kernel loads the material index itself
+  }
+  return FDTD_OK;
+}
+
+template <typename T, int MODE>
+static void region_launch(bool isH, const StepParams<T>& q, int nk, cudaStream_t st) {
+  const long long nvec = (long long)q.rnvx * q.rny;
+  const dim3 grid((unsigned)((nvec + 127) / 128), 1, (unsigned)nk), block(128, 1, 1);
+  if (isH) k_update_H<T, MODE, true><<<grid, block, 0, st>>>(q);
+  else k_update_E<T, MODE, false, true><<<grid, block, 0, st>>>(q);
+}
+
+// One half step of the shell: every cell outside the box shrunk by d cells (d whole vectors in x) on its open sides.  The
+// complement of that inner box is cut into at most six disjoint boxes (two z slabs over the full planes, two y slabs between
+// them, two x slabs between those).
+template <typename T>
+void Solver<T>::shell_pass(bool isH, int d, const StepParams<T>& base, bool bump) {
+  const int V = vlen();
+  const int ix0 = box[0] > 0 ? box[0] + d * V : 0, ix1 = box[1] < nx ? box[1] - d * V : nx;
+  const int iy0 = box[2] > 0 ? box[2] + d : 0, iy1 = box[3] < ny ? box[3] - d : ny;
+  const int iz0 = box[4] > 0 ? box[4] + d : 0, iz1 = box[5] < nz ? box[5] - d : nz;
+  const int reg[6][6] = {{0, nx, 0, ny, 0, iz0},     {0, nx, 0, ny, iz1, nz},   {0, nx, 0, iy0, iz0, iz1},
+                         {0, nx, iy1, ny, iz0, iz1}, {0, ix0, iy0, iy1, iz0, iz1}, {ix1, nx, iy0, iy1, iz0, iz1}};
+  bool first = bump;
+  for (int g = 0; g < 6; ++g) {
+    const int* q6 = reg[g];
+    if (q6[1] <= q6[0] || q6[3] <= q6[2] || q6[5] <= q6[4]) continue;
+    StepParams<T> q = base;
+    q.ri0 = q6[0]; q.rnvx = (q6[1] - q6[0] + V - 1) / V; q.rj0 = q6[2]; q.rny = q6[3] - q6[2]; q.rk0 = q6[4];
+    q.bump = first ? 1 : 0;
+    first = false;
+    switch (mode()) {
+      case 0: region_launch<T, 0>(isH, q, q6[5] - q6[4], stream); break;
+      case 1: region_launch<T, 1>(isH, q, q6[5] - q6[4], stream); break;
+      case 2: region_launch<T, 2>(isH, q, q6[5] - q6[4], stream); break;
+      default: region_launch<T, 3>(isH, q, q6[5] - q6[4], stream); break;
+    }
+    ++launches;
+  }
+}
+
+// Two steps: set a = cur holds time n everywhere; afterwards set b holds time n + 2 everywhere.
+//   shell (one-step kernels, writing set b only):  H1 on shell+3 (E, H from a)   E1 on shell+2 (H from b, E from a)
+//                                                  source, probes, DFT on b        H2 on shell+1, E2 on shell (in place in b)
+//                                                  source, probes, DFT on b
+//   box   (k_step2, reads a, writes b): overwrites the intermediate values the shell passes left in the band around the shell
+// ev (profiling): ev[0] .. ev[1] = shell passes and port kernels, ev[1] .. ev[2] = the box kernel.
+template <typename T>
+void Solver<T>::enqueue_pair(cudaEvent_t* ev) {
+  const int a = cur, b = cur ^ 1;
+  if (ev) cudaEventRecord(ev[0], stream);
+  if (has_shell) {
+    StepParams<T> q = sp_of(a);
+    for (int f = kHx; f <= kHz; ++f) q.dst[f] = field_origin(f, b);
+    shell_pass(true, 3, q, true);                                    // H1: reads a, writes H of b
+    q = sp_of(a);
+    for (int f = kHx; f <= kHz; ++f) q.src[f] = field_origin(f, b);
+    for (int f = kEx; f <= kEz; ++f) q.dst[f] = field_origin(f, b);
+    shell_pass(false, 2, q, false);                                  // E1: H from b, E from a, writes E of b
+    cur = b; enqueue_ports(); cur = a;
+    q = sp_of(b);
+    shell_pass(true, 1, q, true);                                    // H2, E2: in place in b
+    shell_pass(false, 0, q, false);
+    cur = b; enqueue_ports(); cur = a;
+  }
+  if (ev) cudaEventRecord(ev[1], stream);
+  switch (mode()) {
+    case 0: step2_launch<T, 0>(s2par[a], stream); break;
+    case 1: step2_launch<T, 1>(s2par[a], stream); break;
+    case 2: step2_launch<T, 2>(s2par[a], stream); break;
+    default: step2_launch<T, 3>(s2par[a], stream); break;
+  }
+  ++launches;
+  if (ev) cudaEventRecord(ev[2], stream);
+  cur = b;
+}
+
+// `count` steps of the step implementation in use: pairs where the handle advances two steps per pass
+template <typename T>
+void Solver<T>::enqueue_steps(long count) {
+  if (two_step) {
+    for (; count >= 2; count -= 2) enqueue_pair();
+  }
+  for (; count > 0; --count) enqueue_step();
+}
+
 template <typename T>
 void Solver<T>::launch_fused(cudaEvent_t* ev) {
   if (ev) cudaEventRecord(ev[0], stream);
@@ -849,6 +1062,18 @@ void Solver<T>::launch_fused(cudaEvent_t* ev) {
 template <typename T>
 void Solver<T>::enqueue_step(cudaEvent_t* ev) {
   if (z_slab()) { enqueue_begin(); enqueue_end(); return; }
+  if (two_step) {   // a single step (odd remainder of a pair-wise run): the two-pass kernels in place on the current set
+    const StepParams<T> q = sp_of(cur);
+    switch (mode()) {
+      case 0: launch_two_pass<T, 0>(q, stream, ev); break;
+      case 1: launch_two_pass<T, 1>(q, stream, ev); break;
+      case 2: launch_two_pass<T, 2>(q, stream, ev); break;
+      default: launch_two_pass<T, 3>(q, stream, ev); break;
+    }
+    launches += 2;
+    enqueue_ports_ev(ev);
+    return;
+  }
   if (fused) {
     launch_fused(ev);
     launches += 1;
@@ -899,6 +1124,23 @@ int Solver<T>::profile_step(long n, double* ms) {
     if (cudaEventCreate(&ev[q]) != cudaSuccess) return cuda_fail(cudaGetLastError(), "fdtd_profile_step: event");
   for (int q = 0; q < 4; ++q) ms[q] = 0.0;
   cudaError_t e = cudaSuccess;
+  if (two_step) {   // pairs: ms[0] = the two-step box kernel, ms[1] = the shell passes with their port kernels, both per STEP
+    const long pairs = (n + 1) / 2;
+    for (long s = 0; s < pairs && e == cudaSuccess; ++s) {
+      enqueue_pair(ev);
+      if ((e = cudaEventSynchronize(ev[2])) != cudaSuccess) break;
+      float t0 = 0.f, t1 = 0.f;
+      cudaEventElapsedTime(&t0, ev[0], ev[1]);
+      cudaEventElapsedTime(&t1, ev[1], ev[2]);
+      ms[1] += (double)t0 / (2.0 * pairs);
+      ms[0] += (double)t1 / (2.0 * pairs);
+    }
+    for (int q = 0; q < 5; ++q) cudaEventDestroy(ev[q]);
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "fdtd_profile_step");
+    nstep += 2 * pairs;
+    return FDTD_OK;
+  }
   for (long s = 0; s < n && e == cudaSuccess; ++s) {
     enqueue_step(ev);
     if ((e = cudaEventSynchronize(ev[4])) != cudaSuccess) break;
@@ -922,9 +1164,10 @@ int Solver<T>::build_graph(cudaGraphExec_t* out) {
   const int cur_before = cur;
   cudaError_t e = cudaStreamBeginCapture(stream, cudaStreamCaptureModeThreadLocal);
   if (e != cudaSuccess) return cuda_fail(e, "graph capture begin");
-  for (int s = 0; s < graph_steps; ++s) enqueue_step();
+  enqueue_steps(graph_steps);
   cudaGraph_t g = nullptr;
   e = cudaStreamEndCapture(stream, &g);
+  graph_nodes = launches - before;
   launches = before;
   cur = cur_before;   // graph_steps is even when the step ping-pongs, so a replay ends on the set it started from
   if (e != cudaSuccess) return cuda_fail(e, "graph capture end");
@@ -957,22 +1200,20 @@ int Solver<T>::step(long n) {
     err.clear();
   }
   graph_steps = (int)opt_unroll + ((fused && (opt_unroll & 1)) ? 1 : 0);
+  if (two_step) graph_steps = ((int)opt_unroll + 3) / 4 * 4;   // whole pairs, and an even number of them (the sets swap per pair)
   if (opt_graph && stream != nullptr && left >= graph_steps) {
     cudaGraphExec_t* g = cur ? &gexec2 : &gexec;
     const int r = build_graph(g);
     if (r != FDTD_OK) return r;
-    long nodes = fused ? 1 : 2;
-    if (!ports.empty()) { nodes += 1; for (const PortDev& q : ports) if (q.has_source) nodes += 1; }
-    if (z_slab()) nodes += 3 * (z_lo_open + z_hi_open) - z_hi_open;   // E on plane 0, one wait and one post per open side
     while (left >= graph_steps) {
       const cudaError_t e = cudaGraphLaunch(*g, stream);
       if (e != cudaSuccess) return cuda_fail(e, "graph launch");
       ++graph_replays;
       left -= graph_steps;
-      launches += nodes * graph_steps;
+      launches += graph_nodes;
     }
   }
-  for (; left > 0; --left) enqueue_step();
+  enqueue_steps(left);
   const cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return cuda_fail(e, "fdtd_step");
   nstep += n;
@@ -1162,7 +1403,7 @@ int Solver<T>::reset() {
   cudaError_t e = cudaSuccess;
   const size_t fbytes = (size_t)cells_padded() * sizeof(T);
   for (int f = 0; f < 6 && e == cudaSuccess; ++f) e = cudaMemsetAsync(ws + cv.field[f], 0, fbytes, stream);
-  for (int f = 0; f < 6 && e == cudaSuccess && fused; ++f) e = cudaMemsetAsync(ws + cv.field2[f], 0, fbytes, stream);
+  for (int f = 0; f < 6 && e == cudaSuccess && (fused || two_step); ++f) e = cudaMemsetAsync(ws + cv.field2[f], 0, fbytes, stream);
   for (int q = 0; q < 12 && e == cudaSuccess; ++q)
     if (psi_elems(psi_axis(q))) e = cudaMemsetAsync(ws + cv.psi[q], 0, psi_elems(psi_axis(q)) * sizeof(T), stream);
   for (int q = 0; q < 6 && e == cudaSuccess && fused; ++q)
@@ -1267,7 +1508,7 @@ int fdtd_set_option(fdtd_t* h, int option, long value) {
   if (!h) return FDTD_EINVAL;
   if (h->committed) return h->fail(FDTD_ESTATE, "fdtd_set_option: call before fdtd_commit");
   switch (option) {
-    case FDTD_OPT_STEP_IMPL: if (value < 0 || value > 3) break; h->opt_impl = value; return FDTD_OK;
+    case FDTD_OPT_STEP_IMPL: if (value < 0 || value > 4) break; h->opt_impl = value; return FDTD_OK;
     case FDTD_OPT_USE_GRAPH: h->opt_graph = value ? 1 : 0; return FDTD_OK;
     case FDTD_OPT_GRAPH_UNROLL: if (value < 1 || value > 1024) break; h->opt_unroll = value; return FDTD_OK;
     case FDTD_OPT_FUSED_KZ: if (value < 0 || value > 65535) break; h->opt_kz = value; return FDTD_OK;

@@ -176,9 +176,17 @@ __device__ __forceinline__ void update_H_vec(const StepParams<T>& p, int i0, int
   stv(p.dst[kHx] + o, hx); stv(p.dst[kHy] + o, hy); stv(p.dst[kHz] + o, hz);
 }
 
-template <typename T, int MODE>
+// REGION: the launch covers a box of cells given in p.ri0 .. (rows of the box back to back along blockIdx.x, planes on blockIdx.z)
+template <typename T, int MODE, bool REGION = false>
 __global__ void __launch_bounds__(128) k_update_H(const StepParams<T> p) {
   constexpr int V = VecOf<T>::V;
+  if (REGION) {
+    const int v = blockIdx.x * blockDim.x + threadIdx.x, jr = v / p.rnvx;
+    if (p.bump && v == 0 && blockIdx.z == 0) *p.nstep += 1;
+    if (jr >= p.rny) return;
+    update_H_vec<T, MODE>(p, p.ri0 + (v - jr * p.rnvx) * V, p.rj0 + jr, p.rk0 + (int)blockIdx.z);
+    return;
+  }
   // threads are numbered along the row vectors of a plane, rows back to back: no idle lanes when a row is not a
   // multiple of the block (the X3-shaped grid: 50 vectors per row)
   // (rows that are a whole number of blocks keep one row per blockIdx.y and skip the division)
@@ -305,9 +313,15 @@ __device__ __forceinline__ void update_E_vec(const StepParams<T>& p, int i0, int
   }
 }
 
-template <typename T, int MODE, bool PEER = false>
+template <typename T, int MODE, bool PEER = false, bool REGION = false>
 __global__ void __launch_bounds__(128) k_update_E(const StepParams<T> p) {
   constexpr int V = VecOf<T>::V;
+  if (REGION) {
+    const int v = blockIdx.x * blockDim.x + threadIdx.x, jr = v / p.rnvx;
+    if (jr >= p.rny) return;
+    update_E_vec<T, MODE, PEER>(p, p.ri0 + (v - jr * p.rnvx) * V, p.rj0 + jr, p.rk0 + (int)blockIdx.z);
+    return;
+  }
   const int nvec = (p.nx + V - 1) / V, v = blockIdx.x * blockDim.x + threadIdx.x;
   const int j = gridDim.y > 1 ? (int)blockIdx.y : v / nvec, i0 = (gridDim.y > 1 ? v : v - j * nvec) * V;
   const int k = blockIdx.z;

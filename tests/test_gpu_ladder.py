@@ -178,7 +178,8 @@ def test_C2_quarter_scale_full_200k_steps_sparams():
             print(line)
         sims[run] = (o, gpus, o32)
     So = _s_column(sims["inc"][0], sims["tot"][0], 2, osp)
-    assert np.abs(So[0]).max() > 1e-2, "the via stub must reflect: S*_11 of this test is meant to be non-trivial"
+    # the via stub reflects: S*_11 is a non-zero entry here (about 1.3e-3 in this DC-limit band at 1/4 scale; C1's is identically 0)
+    assert np.abs(So[0]).min() > 5e-4, "S*_11 of this test is meant to be non-trivial"
     Vo, Io = _dfts(sims["tot"][0], 2)
     for name in opts:
         Sg = _s_column(sims["inc"][1][name], sims["tot"][1][name], 2, sparams)
@@ -187,7 +188,8 @@ def test_C2_quarter_scale_full_200k_steps_sparams():
         raw = (np.abs(Vg - Vo).max() / np.abs(Vo).max(), np.abs(Ig - Io).max() / np.abs(Io).max())
         print(f"C2/4 200k steps {name}: |dS*_11| = {d11:.3e}, |dS*_21| = {d21:.3e} (max|S*_11| = {np.abs(So[0]).max():.3f}, "
               f"max|S*_21| = {np.abs(So[1]).max():.3f}); raw fp32 DFT drift (V, I) = ({raw[0]:.3e}, {raw[1]:.3e}), informational (R14)")
-        assert d11 <= 1e-3 and d21 <= 1e-3
+        assert d11 <= 1e-3 and d21 <= 1e-3                      # north_star's bar, absolute
+        assert d11 <= 0.05 * np.abs(So[0]).min()                  # and S*_11 itself is resolved, not just below the bar
     S32 = _s_column(sims["inc"][2], sims["tot"][2], 2, osp)
     V32, I32 = _dfts(sims["tot"][2], 2)
     print(f"C2/4 200k steps yardstick (fp32 oracle vs fp64 oracle): |dS*_11| = {np.abs(So[0] - S32[0]).max():.3e}, "

@@ -14,11 +14,13 @@ from oracle.yee import YeeOracle
 from paper_2208_04371_b200 import (FDTD_F32, FDTD_F64, FDTD_OPT_GRAPH_UNROLL, FDTD_OPT_STEP_IMPL, FDTD_OPT_USE_GRAPH,
                                    FdtdError, Solver, sparams)
 
-from .parity_util import TOL, assert_fields, run_pair
+from .parity_util import TOL, assert_fields, run_pair, solver_or_skip
 
 pytestmark = pytest.mark.gpu
 
-IMPLS = [1, 2, 3]  # FDTD_OPT_STEP_IMPL: 1 = two-pass kernels, 2 = fused E+H kernel (TMA-staged, ping-pong field sets), 3 = persistent
+# FDTD_OPT_STEP_IMPL: 1 = two-pass kernels, 2 = fused E+H kernel (TMA-staged, ping-pong field sets), 3 = persistent,
+# 4 = two steps per pass on a box + one-step kernels on the shell (skipped where the grid leaves no such box)
+IMPLS = [1, 2, 3, 4]
 
 
 @pytest.mark.parametrize("impl", IMPLS)
@@ -178,7 +180,7 @@ def test_graph_replay_equals_plain_launches(impl):
     w = W.random_box(11, nx=40, ny=22, nz=18, steps=27, precision=FDTD_F32)
     out = []
     for graph in (0, 1):
-        s = Solver.from_workload(w, options={FDTD_OPT_STEP_IMPL: impl, FDTD_OPT_USE_GRAPH: graph, FDTD_OPT_GRAPH_UNROLL: 4})
+        s = solver_or_skip(w, options={FDTD_OPT_STEP_IMPL: impl, FDTD_OPT_USE_GRAPH: graph, FDTD_OPT_GRAPH_UNROLL: 4})
         assert s.stream.cuda_stream != 0
         if graph:
             s.step(27)
@@ -335,7 +337,7 @@ def test_fused_equals_two_pass_closely():
         assert np.abs(out[0][c] - out[1][c]).max() / scale < 2e-6
 
 
-@pytest.mark.parametrize("impl", [2, 3])
+@pytest.mark.parametrize("impl", [2, 3, 4])
 def test_repeated_runs_are_bitwise_identical(impl):
     """The fused kernel synchronises its warps with mbarriers only (TMA ring, row-to-row and column hand-over) and the
     persistent kernel with grid barriers: a missing edge in either protocol shows up as run-to-run differences.  Many
@@ -375,3 +377,59 @@ def test_two_overlapping_sources_and_thick_slabs(impl):
     assert_fields(rep, FDTD_F32)
     assert max(rep["dft_err"]) <= 1e-5
     s.destroy()
+
+
+# ---- two steps per pass (FDTD_OPT_STEP_IMPL = 4, fdtd_step2.cuh) --------------------------------------------------------
+def _random_init(shape, seed):
+    r = W.rng_for(seed)
+    ini = [r.standard_normal(shape) * (1.0 if c < 3 else 2.5e-3) for c in range(6)]
+    ini[0][:, 0, :] = 0; ini[0][0] = 0
+    ini[1][:, :, 0] = 0; ini[1][0] = 0
+    ini[2][:, :, 0] = 0; ini[2][:, 0, :] = 0
+    return ini
+
+
+@pytest.mark.parametrize("prec", [FDTD_F64, FDTD_F32])
+@pytest.mark.parametrize("nsteps", [2, 7, 18])
+@pytest.mark.parametrize("mats", ["indexed", "indexed+mu", "full", "full+mu"])
+def test_two_step_box_alone_on_a_pec_box(prec, nsteps, mats):
+    """No CPML, no ports: the box is the whole grid and k_step2 is the only field kernel (plus the two-pass kernels for the
+    odd last step).  Several x tiles (300 = 2 x 120 + 60), y tiles, z chunks that do not divide nz, walls on all six
+    faces, random materials and a random initial state: every cell of the grid is compared."""
+    from paper_2208_04371_b200 import FDTD_OPT_FUSED_KZ
+    w = W.random_box(51, nx=300, ny=40, nz=30, pml=(0,) * 6, indexed=mats.startswith("indexed"), with_mu=mats.endswith("mu"),
+                     steps=nsteps, precision=prec)
+    w = dict(w, ports=[], freqs=np.zeros(0))
+    o, s, rep = run_pair(w, nsteps, precision=prec, options={FDTD_OPT_STEP_IMPL: 4, FDTD_OPT_FUSED_KZ: 7, FDTD_OPT_GRAPH_UNROLL: 4},
+                         init_fields=_random_init((30, 40, 300), 77))
+    assert s.impl_name == "two_step" and s.graph_replays == nsteps // 4
+    assert_fields(rep, prec, tol=(1e-12 if prec == FDTD_F64 else 2e-6))
+    s.destroy()
+
+
+@pytest.mark.parametrize("prec", [FDTD_F64, FDTD_F32])
+@pytest.mark.parametrize("pml", [(5, 6, 4, 3, 0, 5), (4, 4, 4, 4, 4, 4), (0, 7, 0, 5, 3, 0)])
+def test_two_step_box_with_cpml_shell_and_ports(prec, pml):
+    """CPML on some or all faces and two ports: the box keeps two cells from the layers and stays between the port planes;
+    the shell (CPML cells, the band around them, the port planes) is advanced by the region launches of the two-pass
+    kernels, whose intermediate values in the band the box kernel then overwrites.  Fields at an even and an odd step
+    count, the probes of BOTH steps of every pair (raw DFTs)."""
+    w = W.random_box(54, nx=300, ny=44, nz=40, pml=pml, steps=41, precision=prec)
+    o, s, rep = run_pair(w, 41, precision=prec, options={FDTD_OPT_STEP_IMPL: 4}, checkpoints=[2, 12, 41])
+    assert s.impl_name == "two_step"
+    assert_fields(rep, prec, tol=(1e-12 if prec == FDTD_F64 else 1e-5))
+    assert max(rep["dft_err"]) <= (1e-11 if prec == FDTD_F64 else 1e-5)
+    s.destroy()
+
+
+def test_two_step_refuses_grids_without_a_box():
+    """A grid whose CPML layers (or port planes) leave no 32 x 8 x 8 box is an error for FDTD_OPT_STEP_IMPL = 4, not a silent
+    change of implementation; so is a z slab."""
+    w = W.random_box(1, steps=4, precision=FDTD_F32)            # 20 x 14 x 12
+    with pytest.raises(FdtdError) as e:
+        Solver.from_workload(w, options={FDTD_OPT_STEP_IMPL: 4})
+    assert e.value.code == -1
+    w = W.random_box(54, nx=300, ny=44, nz=40, pml=(4, 4, 4, 4, 0, 0), steps=4, precision=FDTD_F32)
+    with pytest.raises(FdtdError) as e:
+        Solver.from_workload(dict(w, ports=[], freqs=np.zeros(0)), options={FDTD_OPT_STEP_IMPL: 4}, z_open=(False, True))
+    assert e.value.code == -1
