@@ -296,7 +296,7 @@ def run_ours(args, rank, world, local_rank):
     import torch
     import torch.distributed as dist
 
-    from paper_2208_04371_b200 import FDTD_OPT_STEP_IMPL, Solver, binding
+    from paper_2208_04371_b200 import FDTD_OPT_FUSED_KZ, FDTD_OPT_FUSED_TILE, FDTD_OPT_STEP_IMPL, Solver, binding
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
@@ -313,7 +313,13 @@ def run_ours(args, rank, world, local_rank):
     K, Wm = args.steps, args.warmup
     w = workload(args.workload, K)
     n_cells = w["nx"] * w["ny"] * w["nz"]
-    opts = {FDTD_OPT_STEP_IMPL: args.step_impl} if args.step_impl else None
+    opts = {}
+    if args.step_impl:
+        opts[FDTD_OPT_STEP_IMPL] = args.step_impl
+    if args.fused_kz:
+        opts[FDTD_OPT_FUSED_KZ] = args.fused_kz
+    if args.fused_tile:
+        opts[FDTD_OPT_FUSED_TILE] = args.fused_tile
     s = Solver.from_workload(w, options=opts, device=str(dev))
     torch.cuda.synchronize(dev)
 
@@ -336,22 +342,47 @@ def run_ours(args, rank, world, local_rank):
     # ---- per-kernel durations (CUDA events between the kernels, on the solver's stream) ------------------------------
     ms = s.profile_step(max(3, min(20, K)))
     impl = s.impl_name
-    if impl == "fused":
+    es = 4 if w["precision"] == 32 else 8
+    peak, peak_src = measured_peak()
+    extra = {}
+    if impl == "two_step":
+        # the dominant kernel advances its box TWO steps per launch: every field of the box read once and written once (+1 B
+        # index) per two cell-updates; profile_step's figures are per STEP, a launch lasts two of them.  The shell around the
+        # box (CPML layers, port planes) is advanced step by step by the two-pass kernels on region grids (ms[1]).
+        b = s.two_step_box
+        box_cells = (b[1] - b[0]) * (b[3] - b[2]) * (b[5] - b[4])
+        full = w["materials"]["mode"] == "full"
+        kname, kms = "k_step2", 2.0 * ms[0]
+        ab = box_cells * (12 * es + (6 * es if full else 1))
+        shell_cells = n_cells - box_cells
+        # what one STEP must move under this scheme: half a box pass + the shell's two-pass traffic (73 B fp32 indexed + psi)
+        step_bytes = ab / 2 + (algorithmic_bytes(w, "two_pass", "H") + algorithmic_bytes(w, "two_pass", "E")) * shell_cells / n_cells
+        one_step_model = algorithmic_bytes(w, "fused", "H")      # the 49 B + psi model of the one-step fused kernel, for comparison
+        extra = {"box": b, "box_cells": box_cells, "shell_cells": shell_cells, "shell_ms_per_step": ms[1],
+                 "bytes_per_cell_update_box": ab / 2 / box_cells,
+                 "one_step_byte_model": {"bytes_per_cell_update": one_step_model / n_cells,
+                                         "equivalent_gbs": one_step_model * K / t_s / 1e9,
+                                         "equivalent_frac": one_step_model * K / t_s / 1e9 / peak,
+                                         "note": "throughput expressed in the one-step fused kernel's byte model (49 B + psi per "
+                                                 "cell-update): may exceed 1 because two steps per pass move fewer bytes"}}
+    elif impl == "fused":
         kname, kms = "k_step_fused", ms[0]
+        ab = algorithmic_bytes(w, impl, "H")
+        step_bytes = ab
     else:
         kname, kms = ("k_update_E", ms[1]) if ms[1] >= ms[0] else ("k_update_H", ms[0])
-    ab = algorithmic_bytes(w, impl, "E" if kname == "k_update_E" else "H")
-    peak, peak_src = measured_peak()
+        ab = algorithmic_bytes(w, impl, "E" if kname == "k_update_E" else "H")
+        step_bytes = algorithmic_bytes(w, impl, "H") + algorithmic_bytes(w, impl, "E")
     achieved = ab / (kms * 1e-3) / 1e9
-    step_bytes = algorithmic_bytes(w, impl, "H") + (algorithmic_bytes(w, impl, "E") if impl != "fused" else 0)
     # DRAM bytes of one launch from the committed `ncu --set full` capture of this workload and kernel (profiles/), else null
     traffic, traffic_src = ncu_traffic(args.workload, kname, "f32" if w["precision"] == 32 else "f64", s.fused_kz)
     roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": ab, "kernel_ms": kms,
-                "kernel_ms_all": {"H_or_fused": ms[0], "E": ms[1], "source": ms[2], "probe_dft": ms[3]},
+                "kernel_ms_all": {"H_or_fused_or_box": ms[0], "E_or_shell": ms[1], "source": ms[2], "probe_dft": ms[3]},
                 "bytes_per_cell_update_step": step_bytes / n_cells,
                 "step_achieved_gbs": step_bytes * K / t_s / 1e9, "frac_of_8000": step_bytes * K / t_s / 1e9 / 8000.0}
+    roofline.update(extra)
 
     # ---- sustained: BASELINE.json's "2000 steps timed" on C3, own clock samples ---------------------------------------
     sustained = None
@@ -396,7 +427,7 @@ def run_ours(args, rank, world, local_rank):
             "dtype": "f32" if w["precision"] == 32 else "f64", "data": "synthetic",
             "config": {"workload": args.workload, "grid": [w["nx"], w["ny"], w["nz"]], "cells": n_cells,
                        "materials": m["mode"], "cpml_cells": w["pml"], "ports": len(w["ports"]), "dft_freqs": len(w["freqs"]),
-                       "step_impl": impl, "fused_kz": s.fused_kz, "l2": "inputs larger than L2 (no flush needed)" if n_cells * 24 > 2.6e8 else
+                       "step_impl": impl, "fused_kz": s.fused_kz, "fused_tile": s.fused_tile, "l2": "inputs larger than L2 (no flush needed)" if n_cells * 24 > 2.6e8 else
                        "grid fits in L2: launch-bound case, not a roofline case",
                        "parallelism": "replicas only" if world > 1 else "1 GPU", "library": os.path.basename(binding.library_path())},
             "clocks": ck, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "sustained": sustained}
@@ -525,7 +556,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="c3")
-    ap.add_argument("--step-impl", type=int, default=0, help="FDTD_OPT_STEP_IMPL: 0 auto, 1 two-pass, 2 fused")
+    ap.add_argument("--step-impl", type=int, default=0, help="FDTD_OPT_STEP_IMPL: 0 auto, 1 two-pass, 2 fused, 3 persistent, 4 two steps per pass")
+    ap.add_argument("--fused-kz", type=int, default=0, help="FDTD_OPT_FUSED_KZ: planes per z chunk (0 = measured at commit)")
+    ap.add_argument("--fused-tile", type=int, default=0, help="FDTD_OPT_FUSED_TILE: 0 measured at commit, 1 = 14-row tiles, 2 = 6-row tiles")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--cpu-budget", type=float, default=15.0)
     ap.add_argument("--sustained-steps", type=int, default=2000,

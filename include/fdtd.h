@@ -55,21 +55,27 @@ enum { FDTD_EX = 0, FDTD_EY, FDTD_EZ, FDTD_HX, FDTD_HY, FDTD_HZ };
 /* Options for fdtd_set_option (before commit). */
 enum {
   FDTD_OPT_STEP_IMPL = 1,   /* 0 = auto: fdtd_commit measures the candidates on the committed all-zero state and keeps the
-                                   fastest (below 4 Mi cells: two-pass vs persistent; above: two-pass vs fused),
+                                   fastest (below 4 Mi cells: two-pass vs persistent; above: two-pass vs fused; from 64 Mi
+                                   cells also 4, where the grid leaves it a box),
                                1 = two-pass (H kernel, E kernel, in place),
                                2 = fused E+H kernel (temporal blocking over the half steps; a second field set),
                                3 = persistent: fdtd_step(n) is one cooperative launch per 4096 steps, with grid-wide
                                    barriers between the half steps (grids that live in L2; the arithmetic of 1),
                                4 = two steps per pass: a box of cells that keeps two cells' distance from the CPML
-                                   layers and the port planes is advanced TWO steps by one kernel (every field read and
-                                   written once per two steps), the shell around it step by step with the kernels of 1;
-                                   fdtd_commit returns FDTD_EINVAL when the grid leaves no such box; a second field set */
+                                   layers is advanced TWO steps by one kernel (every field read and written once per two
+                                   steps; the kernel adds the first step's source itself), the shell around it -- and a
+                                   band of cells around every port plane inside the box, for the probes of the first
+                                   step -- step by step with the kernels of 1; at most 4 driving ports; fdtd_commit
+                                   returns FDTD_EINVAL when the grid leaves no such box; a second field set */
   FDTD_OPT_USE_GRAPH = 2,   /* 1 (default) = replay a captured CUDA graph per FDTD_OPT_GRAPH_UNROLL steps; 0 = plain launches.
                                Capture needs a real stream: on the NULL (legacy default) stream fdtd_step always issues
                                plain launches (fdtd_graph_replays() stays 0)                                             */
   FDTD_OPT_GRAPH_UNROLL = 3,/* steps per captured graph (default 8; rounded up to even for the fused step)              */
   FDTD_OPT_FUSED_KZ = 4,    /* planes per z chunk of the fused kernel (0 = auto: measured at commit)                    */
-  FDTD_OPT_Z_SPIN = 5       /* linked z slabs: polls of a hand-over counter before a wait gives up (default 2e7, ~2 s)  */
+  FDTD_OPT_Z_SPIN = 5,      /* linked z slabs: polls of a hand-over counter before a wait gives up (default 2e7, ~2 s)  */
+  FDTD_OPT_FUSED_TILE = 6   /* tile of the fused kernel: 0 = auto (measured at commit), 1 = 128 x 14 cells (fp64: 64 x 14), one
+                               block per SM; 2 = 128 x 6 (64 x 6), two blocks per SM: twice the tiles and two z marches per
+                               SM for mid-size grids.  The results are the same cell by cell whatever the tile            */
 };
 
 /* A port (Fig. 1a): a soft E_z source on a box of the plane i = is (surface 'e'), a voltage box and
@@ -223,6 +229,14 @@ const char* fdtd_impl_name(const fdtd_t*);
  * FDTD_OPT_STEP_IMPL = 0 or FDTD_OPT_FUSED_KZ = 0, fdtd_commit times the candidates on the committed all-zero state
  * (two-pass and fused with 12..48 planes per chunk) and keeps the fastest; the state is left exactly as committed. */
 int fdtd_fused_kz(const fdtd_t*);
+/* Tile of the fused step in use after commit, numbered as FDTD_OPT_FUSED_TILE (1 or 2; 0 when another step implementation
+ * is in use), for reports. */
+int fdtd_fused_tile(const fdtd_t*);
+/* FDTD_OPT_STEP_IMPL = 4 (in use after commit): the box [box[0], box[1]) x [box[2], box[3]) x [box[4], box[5]) of cells that one
+ * kernel advances two steps per pass; every other cell belongs to the shell that the one-step kernels advance (reports:
+ * the bytes one launch of the two-step kernel must move are counted over this box).  FDTD_ESTATE when another step
+ * implementation is in use. */
+int fdtd_two_step_box(const fdtd_t*, int box[6]);
 const char* fdtd_last_error(const fdtd_t*);
 void fdtd_destroy(fdtd_t*);
 

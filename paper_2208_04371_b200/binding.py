@@ -18,7 +18,7 @@ FDTD_F32, FDTD_F64 = 32, 64
 FDTD_W_DGAUSS, FDTD_W_GAUSS, FDTD_W_GSINE = 0, 1, 2
 FDTD_MAT_INDEXED, FDTD_MAT_FULL = 0, 1
 FDTD_EX, FDTD_EY, FDTD_EZ, FDTD_HX, FDTD_HY, FDTD_HZ = range(6)
-FDTD_OPT_STEP_IMPL, FDTD_OPT_USE_GRAPH, FDTD_OPT_GRAPH_UNROLL, FDTD_OPT_FUSED_KZ, FDTD_OPT_Z_SPIN = 1, 2, 3, 4, 5
+FDTD_OPT_STEP_IMPL, FDTD_OPT_USE_GRAPH, FDTD_OPT_GRAPH_UNROLL, FDTD_OPT_FUSED_KZ, FDTD_OPT_Z_SPIN, FDTD_OPT_FUSED_TILE = 1, 2, 3, 4, 5, 6
 
 _ERRNAMES = {-1: "FDTD_EINVAL", -2: "FDTD_ECFL", -3: "FDTD_ESTATE", -4: "FDTD_ENOMEM", -5: "FDTD_ECUDA", -6: "FDTD_ERANGE"}
 
@@ -66,6 +66,8 @@ SYMBOLS = {
     "fdtd_device": (C.c_int, [_vp]),
     "fdtd_impl_name": (C.c_char_p, [_vp]),
     "fdtd_fused_kz": (C.c_int, [_vp]),
+    "fdtd_two_step_box": (C.c_int, [_vp, C.POINTER(C.c_int)]),
+    "fdtd_fused_tile": (C.c_int, [_vp]),
     "fdtd_set_z_interfaces": (C.c_int, [_vp, C.c_int, C.c_int]),
     "fdtd_step_begin": (C.c_int, [_vp]),
     "fdtd_step_end": (C.c_int, [_vp]),
@@ -268,6 +270,16 @@ def fdtd_impl_name(h) -> str:
 
 def fdtd_fused_kz(h) -> int:
     return int(lib().fdtd_fused_kz(h))
+
+
+def fdtd_fused_tile(h) -> int:
+    return int(lib().fdtd_fused_tile(h))
+
+
+def fdtd_two_step_box(h):
+    box = (C.c_int * 6)()
+    _check(h, lib().fdtd_two_step_box(h, box))
+    return [int(v) for v in box]
 
 
 def fdtd_set_z_interfaces(h, lo_open, hi_open):

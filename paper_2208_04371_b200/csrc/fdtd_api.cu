@@ -53,7 +53,7 @@ struct fdtd {
   int has_mu = 0;
   std::vector<PortDev> ports;
   std::vector<double> freqs;
-  long opt_impl = 0, opt_graph = 1, opt_unroll = 8, opt_kz = 0;
+  long opt_impl = 0, opt_graph = 1, opt_unroll = 8, opt_kz = 0, opt_tile = 0;
   int z_lo_open = 0, z_hi_open = 0;   // this grid is a z slab of a larger one (fdtd_set_z_interfaces)
   bool z_linked[2] = {false, false};  // fdtd_z_link: the kernels push my boundary planes into the neighbour on that side
   long opt_zspin = 20000000;          // polls of a hand-over flag before the wait kernel gives up (about 2 s)
@@ -116,6 +116,8 @@ struct fdtd {
   virtual int reset() = 0;
   virtual const char* impl_name() const = 0;
   virtual int fused_kz() const = 0;
+  virtual const int* two_step_box() const = 0;
+  virtual int fused_tile() const = 0;
 };
 
 namespace {
@@ -164,10 +166,13 @@ struct Solver : fdtd {
   Step2Params<T> s2par[2];   // s2par[c] reads set c, writes set 1 - c
   int box[6] = {0, 0, 0, 0, 0, 0};   // bx0 bx1 by0 by1 bz0 bz1
   bool has_shell = false;
+  struct Band { int i0, i1, j0, j1, k0, k1; };   // cells around a port plane inside the box (build_step2)
+  std::vector<Band> bands;
   bool persistent = false;   // small grids: many steps per cooperative launch (fdtd_persistent.cuh)
   int persist_blocks = 0;
   int cur = 0;
   int kz = 0;
+  int tile_shape = 0;        // fused step: 0 = FDTD_FUSED_TY-row tiles, one block per SM; 1 = 6-row tiles, two blocks per SM
   int sm_count = 148;
   unsigned probe_blocks = 1; // blocks per port of k_probe_dft: about 1024 samples of the largest V box each
   FusedParams<T> fpar[2];
@@ -267,17 +272,23 @@ struct Solver : fdtd {
   int reset() override;
   const char* impl_name() const override { return two_step ? "two_step" : (fused ? "fused" : (persistent ? "persistent" : "two_pass")); }
   int fused_kz() const override { return (fused || two_step) ? kz : 0; }
+  const int* two_step_box() const override { return two_step ? box : nullptr; }
+  int fused_tile() const override { return fused ? tile_shape + 1 : 0; }
   int build_fused();
   int build_step2();
   void enqueue_pair(cudaEvent_t* ev = nullptr);
   void enqueue_steps(long count);
-  void shell_pass(bool isH, int d, const StepParams<T>& base, bool bump);
+  int shell_pass(bool isH, int d, const StepParams<T>& base, bool bump);
+  void region_pass(bool isH, const StepParams<T>& base, const int* r, bool bump);
+  void band_pass(bool isH, const StepParams<T>& base);
   StepParams<T> sp_of(int set) const {
     StepParams<T> q = sp;
     for (int f = 0; f < 6; ++f) q.src[f] = q.dst[f] = field_origin(f, set);
     return q;
   }
   int autotune();
+  int autotune_two_step();
+  double tuned_ms = -1.0;    // device time per step of the choice autotune() made
   int autotune_kz_only() { const long keep = opt_impl; opt_impl = 2; const int r = autotune(); opt_impl = keep; return r; }
   int setup_persistent();
   int launch_persistent(const PortParams<T>& q, long n, long* done = nullptr);
@@ -440,6 +451,7 @@ int Solver<T>::commit(void* w, size_t bytes, void* st) {
   if (fused) {
     pp2.Ez = field_origin(kEz, 1); pp2.Hy = field_origin(kHy, 1); pp2.Hz = field_origin(kHz, 1);
     kz = opt_kz > 0 ? (int)opt_kz : 32;
+    tile_shape = opt_tile > 0 ? (int)opt_tile - 1 : 0;
     const int r = build_fused();
     if (r != FDTD_OK) return r;
   }
@@ -467,9 +479,16 @@ int Solver<T>::commit(void* w, size_t bytes, void* st) {
   if ((e = cudaStreamSynchronize(stream)) != cudaSuccess) return cuda_fail(e, "fdtd_commit");
   if ((e = cudaGetLastError()) != cudaSuccess) return cuda_fail(e, "fdtd_commit");
   if (fused && (z_lo_open || z_hi_open)) {
-    if (opt_kz <= 0) { const int r = autotune_kz_only(); if (r != FDTD_OK) return r; }
-  } else if (fused && (opt_impl == 0 || opt_kz <= 0)) {
+    if (opt_kz <= 0 || opt_tile <= 0) { const int r = autotune_kz_only(); if (r != FDTD_OK) return r; }
+  } else if (fused && (opt_impl == 0 || opt_kz <= 0 || opt_tile <= 0)) {
     const int r = autotune();
+    if (r != FDTD_OK) return r;
+  }
+  // two steps per pass: a candidate of the automatic choice on grids far beyond L2 (its shell passes and the priming planes
+  // of its chunks need room to pay off: measured slower than the fused step on 16 Mi cells, faster on 900 Mi); asked for by
+  // name, only its chunk length is measured
+  if ((two_step && opt_kz <= 0) || (opt_impl == 0 && fused && !z_slab() && (long long)nx * ny * nz >= (64LL << 20))) {
+    const int r = autotune_two_step();
     if (r != FDTD_OK) return r;
   }
   if (!fused && !two_step && (opt_impl == 0 || opt_impl == 3)) {
@@ -613,35 +632,49 @@ static PFN_cuTensorMapEncodeTiled_v12000 tensor_map_encoder() {
 #ifndef FDTD_FUSED_NS
 #define FDTD_FUSED_NS 3
 #endif
-template <typename T> struct FusedTile { static constexpr int TY = FDTD_FUSED_TY, NS = FDTD_FUSED_NS; };
+// two tile shapes: 0 = FDTD_FUSED_TY rows, one block per SM (large grids: the longest rows-per-halo ratio); 1 = 6 rows, two
+// blocks per SM (mid-size grids: twice the tiles, two z marches per SM).  fdtd_commit measures both (autotune()).
+constexpr int kFusedTileShapes = 2;
+template <int SHAPE> struct FusedTile { static constexpr int TY = FDTD_FUSED_TY, NS = FDTD_FUSED_NS, PER_SM = 1; };
+template <> struct FusedTile<1> { static constexpr int TY = kFusedSmallTY, NS = 3, PER_SM = 2; };
 static_assert(FusedCfg<float, FDTD_FUSED_TY, FDTD_FUSED_NS>::SMEM <= 232448 && FusedCfg<double, FDTD_FUSED_TY, FDTD_FUSED_NS>::SMEM <= 232448,
               "fused kernel: tile x stages exceed the 227 KB shared memory of an sm_100 CTA");
+static_assert(2 * (FusedCfg<float, FusedTile<1>::TY, FusedTile<1>::NS>::SMEM + 1024) <= 233472 &&
+              2 * (FusedCfg<double, FusedTile<1>::TY, FusedTile<1>::NS>::SMEM + 1024) <= 233472,
+              "fused kernel, small tile: two blocks must fit the 228 KB shared memory of an sm_100 SM");
 
-template <typename T, int MODE>
+template <typename T, int MODE, int SHAPE>
 static cudaError_t fused_set_attr() {
-  using C = FusedCfg<T, FusedTile<T>::TY, FusedTile<T>::NS>;
+  using C = FusedCfg<T, FusedTile<SHAPE>::TY, FusedTile<SHAPE>::NS>;
   return cudaFuncSetAttribute(k_step_fused<T, MODE, C::TY, C::NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM);
 }
-template <typename T, int MODE>
+template <typename T, int MODE, int SHAPE>
 static void fused_launch(const FusedParams<T>& fp, cudaStream_t st) {
-  using C = FusedCfg<T, FusedTile<T>::TY, FusedTile<T>::NS>;
+  using C = FusedCfg<T, FusedTile<SHAPE>::TY, FusedTile<SHAPE>::NS>;
   const StepParams<T>& sp = fp.sp;
   const long long blocks = (long long)fp.ntx * fp.nty * ((sp.nz + fp.kz - 1) / fp.kz);
   k_step_fused<T, MODE, C::TY, C::NS><<<(unsigned)blocks, C::THREADS, C::SMEM, st>>>(fp);
 }
+// CALL(MODE, SHAPE) for the handle's material mode and tile shape
+#define FDTD_FUSED_DISPATCH(CALL)                                                \
+  switch (tile_shape * 4 + mode()) {                                             \
+    case 0: CALL(0, 0); break; case 1: CALL(1, 0); break; case 2: CALL(2, 0); break; case 3: CALL(3, 0); break; \
+    case 4: CALL(0, 1); break; case 5: CALL(1, 1); break; case 6: CALL(2, 1); break; default: CALL(3, 1); break; \
+  }
 
 template <typename T>
 int Solver<T>::build_fused() {
-  using C = FusedCfg<T, FusedTile<T>::TY, FusedTile<T>::NS>;
+  const int TX = 32 * VecOf<T>::V;
+  const int TY = tile_shape == 1 ? FusedTile<1>::TY : FusedTile<0>::TY, per_sm = tile_shape == 1 ? FusedTile<1>::PER_SM : FusedTile<0>::PER_SM;
+  // box of field f in the tile shape in use (FusedCfg::xw, ::nr)
+  auto box_w = [&](int f) { return tile_shape == 1 ? FusedCfg<T, FusedTile<1>::TY, FusedTile<1>::NS>::xw(f) : FusedCfg<T, FusedTile<0>::TY, FusedTile<0>::NS>::xw(f); };
+  auto box_r = [&](int f) { return tile_shape == 1 ? FusedCfg<T, FusedTile<1>::TY, FusedTile<1>::NS>::nr(f) : FusedCfg<T, FusedTile<0>::TY, FusedTile<0>::NS>::nr(f); };
   auto enc = tensor_map_encoder();
   if (!enc) return fail(FDTD_ECUDA, "fdtd_commit: the driver does not export cuTensorMapEncodeTiled (fused step needs TMA)");
   cudaError_t e = cudaSuccess;
-  switch (mode()) {
-    case 0: e = fused_set_attr<T, 0>(); break;
-    case 1: e = fused_set_attr<T, 1>(); break;
-    case 2: e = fused_set_attr<T, 2>(); break;
-    default: e = fused_set_attr<T, 3>(); break;
-  }
+#define FDTD_CALL(M, S) e = fused_set_attr<T, M, S>()
+  FDTD_FUSED_DISPATCH(FDTD_CALL)
+#undef FDTD_CALL
   if (e != cudaSuccess) return cuda_fail(e, "fdtd_commit: shared memory opt-in of the fused kernel");
   // planes per z chunk: the caller set a starting value; fdtd_commit then times the candidates on the committed
   // (all-zero) state and keeps the fastest: autotune().  Why short chunks win is in fdtd_fused.cuh / DESIGN.md 6.2.
@@ -672,18 +705,19 @@ int Solver<T>::build_fused() {
       fp.sp.psi[q] = reinterpret_cast<T*>(ws + (c ? cv.psi[q] : cv.psiH2[q]));
     }
     fp.kz = kz;
-    fp.ntx = (nx + C::TX - 1) / C::TX; fp.nty = (ny + C::TY - 1) / C::TY;
+    fp.ntx = (nx + TX - 1) / TX; fp.nty = (ny + TY - 1) / TY;
     // dispatch groups: as many whole rows of x tiles as fit the SMs (C3: 12 x 12 = 144 of 148); measured on C3 against
     // chunk-major order over all 660 tiles: 7.80 vs 7.94 ms/step (profiles/r01_final.md)
-    fp.group = fp.ntx <= sm_count ? (sm_count / fp.ntx) * fp.ntx : sm_count;
+    const int slots = sm_count * per_sm;
+    fp.group = fp.ntx <= slots ? (slots / fp.ntx) * fp.ntx : slots;
     if (fp.group > fp.ntx * fp.nty) fp.group = fp.ntx * fp.nty;
     fp.cpack = reinterpret_cast<const T*>(ws + cv.vec[0]);   // stride kMaxSlab: build_fused runs only when slabs_fit()
     for (int f = 0; f < 6; ++f) {
-      if (!make(&fp.tm[f], ws + (c ? cv.field2[f] : cv.field[f]), fdt, sizeof(T), C::xw(f), C::nr(f)))
+      if (!make(&fp.tm[f], ws + (c ? cv.field2[f] : cv.field[f]), fdt, sizeof(T), box_w(f), box_r(f)))
         return fail(FDTD_ECUDA, "fdtd_commit: cuTensorMapEncodeTiled failed for field %d", f);
     }
     if (mat_mode == FDTD_MAT_INDEXED) {
-      if (!make(&fp.tm[6], ws + cv.idx, CU_TENSOR_MAP_DATA_TYPE_UINT8, 1, C::TX, C::TY))
+      if (!make(&fp.tm[6], ws + cv.idx, CU_TENSOR_MAP_DATA_TYPE_UINT8, 1, TX, TY))
         return fail(FDTD_ECUDA, "fdtd_commit: cuTensorMapEncodeTiled failed for the material index");
     } else {
       fp.tm[6] = fp.tm[0];
@@ -728,17 +762,27 @@ template <typename T>
 int Solver<T>::autotune() {
   const int reps = (long long)nx * ny * nz >= (64LL << 20) ? 2 : 4;
   double best = -1.0;
-  int best_kz = kz;
+  int best_kz = kz, best_shape = tile_shape;
   bool best_fused = true;
-  if (opt_kz <= 0) {
-    // the fixed ladder, plus -- for grids that give the SMs only a few waves of blocks -- the chunk lengths whose block count
-    // comes closest to whole waves (C2: 76 tiles; 10-plane chunks make 6.7 waves where 16-plane chunks make 4.1)
-    std::vector<int> cand = {8, 12, 16, 20, 24, 32, 48};
-    {
+  const int kz_given = kz;
+  for (int shape = 0; shape < kFusedTileShapes; ++shape) {
+    if (opt_tile > 0 && shape != (int)opt_tile - 1) continue;
+    if (shape != tile_shape) {
+      tile_shape = shape;
+      kz = kz_given;
+      const int r = build_fused();
+      if (r != FDTD_OK) return r;
+    }
+    const int per_sm = shape == 1 ? FusedTile<1>::PER_SM : FusedTile<0>::PER_SM;
+    std::vector<int> cand;
+    if (opt_kz <= 0) {
+      // the fixed ladder, plus -- for grids that give the SMs only a few waves of blocks -- the chunk lengths whose block count
+      // comes closest to whole waves (C2: 76 tiles; 10-plane chunks make 6.7 waves where 16-plane chunks make 4.1)
+      cand = {8, 12, 16, 20, 24, 32, 48};
       const long long tiles = (long long)fpar[0].ntx * fpar[0].nty;
       std::vector<std::pair<double, int>> fit;
       for (int q = 6; q <= 48 && q <= nz; ++q) {
-        const double waves = (double)(tiles * ((nz + q - 1) / q)) / sm_count;
+        const double waves = (double)(tiles * ((nz + q - 1) / q)) / (sm_count * per_sm);
         if (waves > 24.0) continue;
         fit.push_back({-(waves / std::ceil(waves)) * q / (q + 2.5), q});   // wave fill x (planes owned / planes loaded)
       }
@@ -746,6 +790,8 @@ int Solver<T>::autotune() {
       for (size_t q = 0; q < fit.size() && q < 3; ++q)
         if (std::find(cand.begin(), cand.end(), fit[q].second) == cand.end()) cand.push_back(fit[q].second);
       std::sort(cand.begin(), cand.end());
+    } else {
+      cand = {kz};
     }
     for (size_t c = 0; c < cand.size(); ++c) {
       if (cand[c] > nz && c > 0) break;
@@ -753,12 +799,10 @@ int Solver<T>::autotune() {
       fpar[0].kz = fpar[1].kz = kz;
       const double t = time_field_kernels(reps);
       if (t < 0) return fail(FDTD_ECUDA, "fdtd_commit: timing the fused kernel failed: %s", cudaGetErrorString(cudaGetLastError()));
-      if (best < 0 || t < best) { best = t; best_kz = kz; }
+      if (best < 0 || t < best) { best = t; best_kz = kz; best_shape = shape; }
     }
-  } else {
-    best = time_field_kernels(reps);
-    if (best < 0) return fail(FDTD_ECUDA, "fdtd_commit: timing the fused kernel failed: %s", cudaGetErrorString(cudaGetLastError()));
   }
+  if (best < 0) return fail(FDTD_EINVAL, "fdtd_commit: no fused tile shape to time");
   if (opt_impl == 0) {
     fused = false;
     const double t = time_field_kernels(reps);
@@ -767,11 +811,72 @@ int Solver<T>::autotune() {
   }
   fused = best_fused;
   kz = best_kz;
+  tuned_ms = best;
+  if (tile_shape != best_shape) {
+    tile_shape = best_shape;
+    const int r = build_fused();
+    if (r != FDTD_OK) return r;
+  }
   fpar[0].kz = fpar[1].kz = kz;
   cur = 0;
   cudaError_t e = cudaMemsetAsync(sp.nstep, 0, sizeof(long long), stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
   if (e != cudaSuccess) return cuda_fail(e, "fdtd_commit: autotune");
+  return FDTD_OK;
+}
+
+// The two-steps-per-pass implementation measured like the others, on the committed all-zero state with the ports switched
+// off (a source would leave the state non-zero): pairs of steps with 24, 48 and 96 planes per chunk.  Called with the fused
+// step selected (automatic choice): two_step takes over if a pair costs less than two fused steps.  A grid that leaves no
+// box is simply no candidate.
+template <typename T>
+int Solver<T>::autotune_two_step() {
+  const bool asked = two_step;
+  const int kz_before = kz;
+  if (!asked) {
+    const std::string keep_err = err;
+    kz = 24;
+    if (build_step2() != FDTD_OK) { err = keep_err; kz = kz_before; return FDTD_OK; }
+  }
+  std::vector<PortDev> no_ports;
+  no_ports.swap(ports);
+  const int nsrc = s2par[0].nsrc;
+  s2par[0].nsrc = s2par[1].nsrc = 0;
+  cudaEvent_t a, b;
+  bool ok = cudaEventCreate(&a) == cudaSuccess && cudaEventCreate(&b) == cudaSuccess;
+  double best = -1.0;
+  int best_kz = kz;
+  const int zext = box[5] - box[4], reps = (long long)nx * ny * nz >= (64LL << 20) ? 1 : 3;
+  const int cand[3] = {24, 48, 96};
+  for (int c = 0; c < 3 && ok; ++c) {
+    if (cand[c] > zext && c > 0) break;
+    kz = cand[c] > zext ? zext : cand[c];
+    s2par[0].kz = s2par[1].kz = kz;
+    enqueue_pair();
+    cudaEventRecord(a, stream);
+    for (int q = 0; q < reps; ++q) enqueue_pair();
+    cudaEventRecord(b, stream);
+    float ms = -1.f;
+    ok = cudaEventSynchronize(b) == cudaSuccess && cudaEventElapsedTime(&ms, a, b) == cudaSuccess;
+    const double per_step = (double)ms / (2.0 * reps);
+    if (ok && (best < 0 || per_step < best)) { best = per_step; best_kz = kz; }
+  }
+  if (ok) { cudaEventDestroy(a); cudaEventDestroy(b); }
+  ports.swap(no_ports);
+  s2par[0].nsrc = s2par[1].nsrc = nsrc;
+  cur = 0;
+  cudaError_t e = cudaMemsetAsync(sp.nstep, 0, sizeof(long long), stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+  if (!ok || e != cudaSuccess || best < 0) return cuda_fail(e != cudaSuccess ? e : cudaGetLastError(), "fdtd_commit: timing the two-step kernel");
+  if (asked || (tuned_ms > 0 && best < tuned_ms)) {
+    two_step = true;
+    fused = false;
+    kz = best_kz;
+    tuned_ms = best;
+  } else {
+    kz = kz_before;
+  }
+  s2par[0].kz = s2par[1].kz = two_step ? kz : s2par[0].kz;
   return FDTD_OK;
 }
 
@@ -895,9 +1000,10 @@ static void step2_launch(const Step2Params<T>& q, cudaStream_t st) {
   k_step2<T, MODE, C::R, C::NS><<<(unsigned)blocks, C::THREADS, C::SMEM, st>>>(q);
 }
 
-// The box that advances two steps per pass: every cell at least two cells away from every CPML cell and from every source
-// sample, and not on a port plane (the probes of the intermediate step read the shell's arrays; fdtd_step2.cuh).  Ports are
-// kept out by x ranges: a transmission line's ports sit near its two ends (Fig. 1a).
+// The box that advances two steps per pass: every cell at least two cells away from every CPML cell (fdtd_step2.cuh).  Ports
+// may lie anywhere: the kernel adds the first step's source itself, and for every port plane inside the box a thin band of
+// cells around the port's probe samples is advanced through the first step by the one-step kernels, only so that the
+// probes of that step find E^{n+1} (source included) and H^{n+1/2} there (the box kernel overwrites the band afterwards).
 template <typename T>
 int Solver<T>::build_step2() {
   using C = Step2Cfg<T, FDTD_STEP2_R, FDTD_STEP2_NS>;
@@ -923,19 +1029,35 @@ int Solver<T>::build_step2() {
   b[0] = npml[0] ? up(npml[0] + 2, V) : 0;  b[1] = npml[1] ? down(nx - npml[1] - 2, V) : nx;
   b[2] = npml[2] ? npml[2] + 2 : 0;         b[3] = npml[3] ? ny - npml[3] - 2 : ny;
   b[4] = npml[4] ? npml[4] + 2 : 0;         b[5] = npml[5] ? nz - npml[5] - 2 : nz;
-  for (const PortDev& d : ports) {
-    if (d.ip < nx / 2) b[0] = std::max(b[0], up(std::max(d.has_source ? d.is + 2 : 0, d.ip + 1), V));
-    else               b[1] = std::min(b[1], down(std::min(d.has_source ? d.is - 1 : nx, d.ip), V));
-    if (d.has_source && ((d.ip < nx / 2) != (d.is < nx / 2)))
-      return fail(FDTD_EINVAL, "fdtd_commit: FDTD_OPT_STEP_IMPL = 4 needs every source on the same side of the grid as its port plane");
-  }
   if (b[1] - b[0] < 8 * V || b[3] - b[2] < 8 || b[5] - b[4] < 8)
     return fail(FDTD_EINVAL, "fdtd_commit: FDTD_OPT_STEP_IMPL = 4: no box of at least %d x 8 x 8 cells keeps two cells' distance from the "
-                             "CPML layers and the port planes of this grid", 8 * V);
+                             "CPML layers of this grid", 8 * V);
   for (int q = 0; q < 6; ++q) box[q] = b[q];
   has_shell = b[0] > 0 || b[1] < nx || b[2] > 0 || b[3] < ny || b[4] > 0 || b[5] < nz;
   if (kz > b[5] - b[4]) kz = b[5] - b[4];
   if (kz < 1) kz = 1;
+  // sources: carried in the kernel parameters
+  int nsrc = 0;
+  typename Step2Params<T>::Src srcs[kStep2MaxSrc];
+  for (const PortDev& d : ports) {
+    if (!d.has_source) continue;
+    if (nsrc == kStep2MaxSrc)
+      return fail(FDTD_EINVAL, "fdtd_commit: FDTD_OPT_STEP_IMPL = 4 carries at most %d driving ports", kStep2MaxSrc);
+    srcs[nsrc++] = {d.is, d.sj0, d.sj1, d.sk0, d.sk1, d.waveform, d.amp, d.t0, d.sigma, d.f0};
+  }
+  // bands: bounding box of the probe samples of every port whose plane lies inside the box, one vector wide in x (two where
+  // the cell ip - 1, whose H the E update on the plane needs, falls into the vector before)
+  bands.clear();
+  for (const PortDev& d : ports) {
+    if (d.ip < b[0] || d.ip >= b[1]) continue;     // on a shell plane: the shell passes cover every cell of that plane
+    Band g;
+    g.j0 = std::max(0, std::min(d.vj0, d.lj0 - 1)); g.j1 = std::min(ny, std::max(d.vj1, d.lj1) + 1);
+    g.k0 = std::max(0, std::min(d.vk0, d.lk0 - 1)); g.k1 = std::min(nz, std::max(d.vk1 - 1, d.lk1) + 1);
+    g.i0 = down(d.ip, V); g.i1 = g.i0 + V;
+    bool dup = false;
+    for (const Band& o : bands) dup = dup || (o.i0 == g.i0 && o.j0 == g.j0 && o.j1 == g.j1 && o.k0 == g.k0 && o.k1 == g.k1);
+    if (!dup) bands.push_back(g);
+  }
 
   const cuuint64_t gdim[3] = {(cuuint64_t)pitch(), (cuuint64_t)(ny + 1), (cuuint64_t)(nz + 2)};
   const cuuint32_t estr[3] = {1, 1, 1};
@@ -955,7 +1077,9 @@ int Solver<T>::build_step2() {
     q.group = q.ntx <= sm_count ? (sm_count / q.ntx) * q.ntx : sm_count;
     if (q.group > q.ntx * q.nty) q.group = q.ntx * q.nty;
     q.bx0 = b[0]; q.bx1 = b[1]; q.by0 = b[2]; q.by1 = b[3]; q.bz0 = b[4]; q.bz1 = b[5];
-    q.bump = has_shell ? 0 : 1;
+    q.nsrc = nsrc;
+    for (int n = 0; n < nsrc; ++n) q.src[n] = srcs[n];
+    q.dt = dt;
     for (int f = 0; f < 6; ++f)
       if (!make(&q.tm[f], ws + (c ? cv.field2[f] : cv.field[f]), fdt, sizeof(T), C::xw(f), C::nr(f)))
         return fail(FDTD_ECUDA, "fdtd_commit: cuTensorMapEncodeTiled failed for field %d (two-step kernel)", f);
@@ -974,57 +1098,86 @@ static void region_launch(bool isH, const StepParams<T>& q, int nk, cudaStream_t
 
 // One half step of the shell: every cell outside the box shrunk by d cells (d whole vectors in x) on its open sides.  The
 // complement of that inner box is cut into at most six disjoint boxes (two z slabs over the full planes, two y slabs between
-// them, two x slabs between those).
+// them, two x slabs between those).  Returns the number of launches (the first one carries the step-counter bump if asked).
 template <typename T>
-void Solver<T>::shell_pass(bool isH, int d, const StepParams<T>& base, bool bump) {
+int Solver<T>::shell_pass(bool isH, int d, const StepParams<T>& base, bool bump) {
   const int V = vlen();
   const int ix0 = box[0] > 0 ? box[0] + d * V : 0, ix1 = box[1] < nx ? box[1] - d * V : nx;
   const int iy0 = box[2] > 0 ? box[2] + d : 0, iy1 = box[3] < ny ? box[3] - d : ny;
   const int iz0 = box[4] > 0 ? box[4] + d : 0, iz1 = box[5] < nz ? box[5] - d : nz;
   const int reg[6][6] = {{0, nx, 0, ny, 0, iz0},     {0, nx, 0, ny, iz1, nz},   {0, nx, 0, iy0, iz0, iz1},
                          {0, nx, iy1, ny, iz0, iz1}, {0, ix0, iy0, iy1, iz0, iz1}, {ix1, nx, iy0, iy1, iz0, iz1}};
-  bool first = bump;
+  int launched = 0;
   for (int g = 0; g < 6; ++g) {
     const int* q6 = reg[g];
     if (q6[1] <= q6[0] || q6[3] <= q6[2] || q6[5] <= q6[4]) continue;
-    StepParams<T> q = base;
-    q.ri0 = q6[0]; q.rnvx = (q6[1] - q6[0] + V - 1) / V; q.rj0 = q6[2]; q.rny = q6[3] - q6[2]; q.rk0 = q6[4];
-    q.bump = first ? 1 : 0;
-    first = false;
-    switch (mode()) {
-      case 0: region_launch<T, 0>(isH, q, q6[5] - q6[4], stream); break;
-      case 1: region_launch<T, 1>(isH, q, q6[5] - q6[4], stream); break;
-      case 2: region_launch<T, 2>(isH, q, q6[5] - q6[4], stream); break;
-      default: region_launch<T, 3>(isH, q, q6[5] - q6[4], stream); break;
-    }
-    ++launches;
+    region_pass(isH, base, q6, bump && launched == 0);
+    ++launched;
+  }
+  return launched;
+}
+
+// the one-step H or E kernel on the cells [r[0], r[1]) x [r[2], r[3]) x [r[4], r[5])  (r[0] a multiple of the vector length)
+template <typename T>
+void Solver<T>::region_pass(bool isH, const StepParams<T>& base, const int* r, bool bump) {
+  const int V = vlen();
+  StepParams<T> q = base;
+  q.ri0 = r[0]; q.rnvx = (r[1] - r[0] + V - 1) / V; q.rj0 = r[2]; q.rny = r[3] - r[2]; q.rk0 = r[4];
+  q.bump = bump ? 1 : 0;
+  switch (mode()) {
+    case 0: region_launch<T, 0>(isH, q, r[5] - r[4], stream); break;
+    case 1: region_launch<T, 1>(isH, q, r[5] - r[4], stream); break;
+    case 2: region_launch<T, 2>(isH, q, r[5] - r[4], stream); break;
+    default: region_launch<T, 3>(isH, q, r[5] - r[4], stream); break;
+  }
+  ++launches;
+}
+
+// The first step on the bands around the port planes inside the box: H^{n+1/2} on the probe samples' bounding box grown by one
+// cell on its low sides (the backward differences of the E update reach there), then E^{n+1} on the bounding box itself.
+// A band is clipped to the cells the shell pass of the same half step (d = 3 for H, 2 for E) leaves out: what that pass covers
+// it has already advanced -- a second update would advance the psi of a CPML cell twice.
+template <typename T>
+void Solver<T>::band_pass(bool isH, const StepParams<T>& base) {
+  const int V = vlen(), d = isH ? 3 : 2, grow = isH ? 1 : 0;
+  const int ix0 = box[0] > 0 ? box[0] + d * V : 0, ix1 = box[1] < nx ? box[1] - d * V : nx;
+  const int iy0 = box[2] > 0 ? box[2] + d : 0, iy1 = box[3] < ny ? box[3] - d : ny;
+  const int iz0 = box[4] > 0 ? box[4] + d : 0, iz1 = box[5] < nz ? box[5] - d : nz;
+  for (const Band& g : bands) {
+    const int i0 = (isH && g.i0 > 0) ? g.i0 - V : g.i0;   // cell ip - 1 may sit in the vector before: take it along
+    const int r[6] = {std::max(i0, ix0), std::min(g.i1, ix1), std::max(g.j0 - grow, iy0), std::min(g.j1, iy1),
+                      std::max(g.k0 - grow, iz0), std::min(g.k1, iz1)};
+    if (r[1] <= r[0] || r[3] <= r[2] || r[5] <= r[4]) continue;
+    region_pass(isH, base, r, false);
   }
 }
 
 // Two steps: set a = cur holds time n everywhere; afterwards set b holds time n + 2 everywhere.
-//   shell (one-step kernels, writing set b only):  H1 on shell+3 (E, H from a)   E1 on shell+2 (H from b, E from a)
-//                                                  source, probes, DFT on b        H2 on shell+1, E2 on shell (in place in b)
-//                                                  source, probes, DFT on b
-//   box   (k_step2, reads a, writes b): overwrites the intermediate values the shell passes left in the band around the shell
-// ev (profiling): ev[0] .. ev[1] = shell passes and port kernels, ev[1] .. ev[2] = the box kernel.
+//   shell + bands (one-step kernels, writing set b only):  H1 on shell+3 (E, H from a)   E1 on shell+2 (H from b, E from a)
+//                                                  source, probes, DFT of step n+1 on b
+//   shell                                          H2 on shell+1, E2 on shell (in place in b)
+//   box   (k_step2, reads a, writes b): overwrites the intermediate values the passes above left in the band around the
+//                                       shell and around the port planes; adds the source of step n+1 to its E1 itself
+//   source, probes, DFT of step n+2 on b
+// The device step counter is advanced by the first launch of each step's H pass, or by k_bump where no such launch exists.
+// ev (profiling): ev[0] .. ev[1] = shell passes and port kernels of the first step, ev[1] .. ev[2] = the box kernel.
 template <typename T>
 void Solver<T>::enqueue_pair(cudaEvent_t* ev) {
   const int a = cur, b = cur ^ 1;
   if (ev) cudaEventRecord(ev[0], stream);
-  if (has_shell) {
-    StepParams<T> q = sp_of(a);
-    for (int f = kHx; f <= kHz; ++f) q.dst[f] = field_origin(f, b);
-    shell_pass(true, 3, q, true);                                    // H1: reads a, writes H of b
-    q = sp_of(a);
-    for (int f = kHx; f <= kHz; ++f) q.src[f] = field_origin(f, b);
-    for (int f = kEx; f <= kEz; ++f) q.dst[f] = field_origin(f, b);
-    shell_pass(false, 2, q, false);                                  // E1: H from b, E from a, writes E of b
-    cur = b; enqueue_ports(); cur = a;
-    q = sp_of(b);
-    shell_pass(true, 1, q, true);                                    // H2, E2: in place in b
-    shell_pass(false, 0, q, false);
-    cur = b; enqueue_ports(); cur = a;
-  }
+  StepParams<T> q = sp_of(a);
+  for (int f = kHx; f <= kHz; ++f) q.dst[f] = field_origin(f, b);
+  if (shell_pass(true, 3, q, true) == 0) { k_bump<<<1, 1, 0, stream>>>(sp.nstep, 1); ++launches; }   // H1: reads a, writes H of b
+  band_pass(true, q);
+  q = sp_of(a);
+  for (int f = kHx; f <= kHz; ++f) q.src[f] = field_origin(f, b);
+  for (int f = kEx; f <= kEz; ++f) q.dst[f] = field_origin(f, b);
+  shell_pass(false, 2, q, false);                                    // E1: H from b, E from a, writes E of b
+  band_pass(false, q);
+  cur = b; enqueue_ports(); cur = a;
+  q = sp_of(b);
+  if (shell_pass(true, 1, q, true) == 0) { k_bump<<<1, 1, 0, stream>>>(sp.nstep, 1); ++launches; }   // H2, E2: in place in b
+  shell_pass(false, 0, q, false);
   if (ev) cudaEventRecord(ev[1], stream);
   switch (mode()) {
     case 0: step2_launch<T, 0>(s2par[a], stream); break;
@@ -1035,6 +1188,7 @@ void Solver<T>::enqueue_pair(cudaEvent_t* ev) {
   ++launches;
   if (ev) cudaEventRecord(ev[2], stream);
   cur = b;
+  enqueue_ports();
 }
 
 // `count` steps of the step implementation in use: pairs where the handle advances two steps per pass
@@ -1049,12 +1203,9 @@ void Solver<T>::enqueue_steps(long count) {
 template <typename T>
 void Solver<T>::launch_fused(cudaEvent_t* ev) {
   if (ev) cudaEventRecord(ev[0], stream);
-  switch (mode()) {
-    case 0: fused_launch<T, 0>(fpar[cur], stream); break;
-    case 1: fused_launch<T, 1>(fpar[cur], stream); break;
-    case 2: fused_launch<T, 2>(fpar[cur], stream); break;
-    default: fused_launch<T, 3>(fpar[cur], stream); break;
-  }
+#define FDTD_CALL(M, S) fused_launch<T, M, S>(fpar[cur], stream)
+  FDTD_FUSED_DISPATCH(FDTD_CALL)
+#undef FDTD_CALL
   if (ev) { cudaEventRecord(ev[1], stream); cudaEventRecord(ev[2], stream); }
   cur ^= 1;
 }
@@ -1513,6 +1664,7 @@ int fdtd_set_option(fdtd_t* h, int option, long value) {
     case FDTD_OPT_GRAPH_UNROLL: if (value < 1 || value > 1024) break; h->opt_unroll = value; return FDTD_OK;
     case FDTD_OPT_FUSED_KZ: if (value < 0 || value > 65535) break; h->opt_kz = value; return FDTD_OK;
     case FDTD_OPT_Z_SPIN: if (value < 1) break; h->opt_zspin = value; return FDTD_OK;
+    case FDTD_OPT_FUSED_TILE: if (value < 0 || value > kFusedTileShapes) break; h->opt_tile = value; return FDTD_OK;
   }
   return h->fail(FDTD_EINVAL, "fdtd_set_option: unknown option %d or bad value %ld", option, value);
 }
@@ -1552,6 +1704,14 @@ long fdtd_graph_replays(const fdtd_t* h) { return h ? h->graph_replays : -1; }
 int fdtd_device(const fdtd_t* h) { return h ? h->device : -1; }
 const char* fdtd_impl_name(const fdtd_t* h) { return h && h->committed ? h->impl_name() : ""; }
 int fdtd_fused_kz(const fdtd_t* h) { return h && h->committed ? h->fused_kz() : 0; }
+int fdtd_fused_tile(const fdtd_t* h) { return h && h->committed ? h->fused_tile() : 0; }
+int fdtd_two_step_box(const fdtd_t* h, int box[6]) {
+  if (!h || !box) return FDTD_EINVAL;
+  const int* b = h->committed ? h->two_step_box() : nullptr;
+  if (!b) return FDTD_ESTATE;
+  for (int q = 0; q < 6; ++q) box[q] = b[q];
+  return FDTD_OK;
+}
 const char* fdtd_last_error(const fdtd_t* h) { return h ? h->err.c_str() : "null handle"; }
 void fdtd_destroy(fdtd_t* h) {
   if (!h) return;

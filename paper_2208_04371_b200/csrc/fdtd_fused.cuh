@@ -199,8 +199,12 @@ __device__ __forceinline__ void psi_update2(T (&a)[V], T (&d)[V], const T (&da)[
   }
 }
 
+// Tiles of at most kFusedSmallTY rows are the small-tile build: two blocks per SM (their shared memory and 128 registers per
+// thread allow it), so that two independent z marches hide each other's latencies on grids whose tiles are mostly CPML
+// rows / columns or too few to fill the SMs with one block each (DESIGN.md 6.2 "mid-size grids").
+constexpr int kFusedSmallTY = 6;
 template <typename T, int MODE, int TY, int NS>
-__global__ void __launch_bounds__((TY + 2) * 32, 1) k_step_fused(const __grid_constant__ FusedParams<T> fp) {
+__global__ void __launch_bounds__((TY + 2) * 32, (TY <= kFusedSmallTY ? 2 : 1)) k_step_fused(const __grid_constant__ FusedParams<T> fp) {
   using C = FusedCfg<T, TY, NS>;
   using O = VOps<T, C::V>;
   constexpr int V = C::V, TX = C::TX;

@@ -490,6 +490,9 @@ __global__ void k_coef_H(T* db, long long n, double dt, double mu0) {
   const double mr = (double)db[q];
   db[q] = mr == 0.0 ? T(0) : (T)(dt / (mu0 * mr));
 }
+// the device step counter, advanced on the stream where no field kernel of the step does it
+__global__ void k_bump(long long* nstep, long long add) { *nstep += add; }
+
 template <typename T>
 __global__ void k_fill(T* a, long long n, T v) {
   const long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x;

@@ -7,10 +7,14 @@
 // What it computes, for every cell c of the box [bx0,bx1) x [by0,by1) x [bz0,bz1):
 //     H^{n+1/2} = H^{n-1/2} - Db curl E^n          (H1)      E^{n+1} = Ca E^n     + Cb curl H^{n+1/2}   (E1)
 //     H^{n+3/2} = H^{n+1/2} - Db curl E^{n+1}      (H2)      E^{n+2} = Ca E^{n+1} + Cb curl H^{n+3/2}   (E2)
-// R5 steps 1-2 twice, plain Yee arithmetic: the box must keep two cells' distance from every CPML cell and from every
-// source sample (nothing inside the dependency cone of the box then carries a psi term or a source term between the two
-// steps); the host plan (fdtd_api.cu) advances what is outside the box -- the CPML shell and the port planes -- step by step
-// with the one-step kernels, and the intermediate fields of the box never reach HBM.
+// R5 steps 1-2 twice, plain Yee arithmetic: the box must keep two cells' distance from every CPML cell (nothing inside the
+// dependency cone of the box then carries a psi term); the host plan (fdtd_api.cu) advances what is outside the box -- the
+// CPML shell -- step by step with the one-step kernels, and the intermediate fields of the box never reach HBM.
+// Ports inside the box: the soft source of the first step (R5 step 3: E_z += A g((n+1) dt) between E1 and H2) is added by
+// this kernel to E1 on every source sample it computes, as owner or as halo -- the same value k_source adds, by the same
+// expression; the source of the second step and its probes run after the kernel on the stored E2, H2.  The probes of the
+// first step need E1, H1 on the port planes, which never leave the chip: the host plan recomputes them on a thin band of
+// cells around each port plane with the one-step kernels (fdtd_api.cu, enqueue_pair).
 //
 // How: like the fused step, a block marches along z over a chunk of planes of an (x,y) tile with TMA-staged input planes,
 // one warp per tile row.  Instead of special halo warps, every row warp computes all four half steps on the full 32-lane
@@ -25,11 +29,15 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 
+#include <type_traits>
+
 #include "fdtd_fused.cuh"
 #include "fdtd_kernels.cuh"
 #include "fdtd_params.h"
 
 namespace fdtd_b200 {
+
+constexpr int kStep2MaxSrc = 4;   // driving ports per handle the two-step kernel carries in its parameters
 
 template <typename T>
 struct Step2Params {
@@ -38,7 +46,11 @@ struct Step2Params {
   int kz;                // owned planes per z chunk
   int ntx, nty, group;   // tiles in x, y and dispatch group (as in FusedParams)
   int bx0, bx1, by0, by1, bz0, bz1;   // the box; bx0, bx1 multiples of the vector length
-  int bump;              // 1: this launch increments the device step counter by 2 (no one-step kernel runs beside it)
+  // soft sources whose samples the kernel may compute (any port with a source: the test is per cell).  The device step
+  // counter already stands at n + 2 when the kernel runs (the host plan bumps it before): E1 is at time (counter - 1) dt.
+  int nsrc;
+  struct Src { int is, sj0, sj1, sk0, sk1, waveform; double amp, t0, sigma, f0; } src[kStep2MaxSrc];
+  double dt;
 };
 
 template <typename T, int R_, int NS_>
@@ -102,8 +114,6 @@ __global__ void __launch_bounds__((R + 1) * 32, 1) k_step2(const __grid_constant
   const int k0 = fp.bz0 + chunk * fp.kz, k1 = min(k0 + fp.kz, fp.bz1);
   const int nIt = k1 - k0 + 4;   // it = 0: Ex, Ey of plane k0-2 only; it >= 1: plane k = k0 - 3 + it
 
-  if (fp.bump && blockIdx.x == 0 && threadIdx.x == 0) *p.nstep += 2;
-
   auto issue = [&](int it, int s) {
     const int k = k0 - 3 + it;
     unsigned char* st = smem + s * C::STAGE;
@@ -165,6 +175,11 @@ __global__ void __launch_bounds__((R + 1) * 32, 1) k_step2(const __grid_constant
   bool xin[V];
 #pragma unroll
   for (int v = 0; v < V; ++v) xin[v] = (i0 + v >= 0) && (i0 + v < p.nx);
+  const bool clean_xy = j >= 1 && j < p.ny && i0 >= 1 && i0 + V <= p.nx;   // no wall row / column, no cell outside the grid
+  // sources with a sample in this thread's cells (bit q = fp.src[q]); the plane range is tested per iteration
+  unsigned srcmask = 0;
+  for (int q = 0; q < fp.nsrc; ++q)
+    if (j >= fp.src[q].sj0 && j <= fp.src[q].sj1 && fp.src[q].is >= i0 && fp.src[q].is < i0 + V) srcmask |= 1u << q;
 
   const int oEx = r * WEx + lane * V, oEy = r * WEy + lane * V, oEz = r * WEz + lane * V, oH = r * TX + lane * V;
 
@@ -205,13 +220,16 @@ __global__ void __launch_bounds__((R + 1) * 32, 1) k_step2(const __grid_constant
         ez[v] = fma(b.b, az[v], a.c * ez[v]);
       }
     }
-    const bool kin = k >= 0 && k < p.nz, wk = (k == 0) && !p.z_lo_open;
+    // walls and cells outside the grid -> 0; vectors wholly inside the grid and off the wall rows / columns / plane skip this
+    if (!(clean_xy && k >= 1 && k < p.nz)) {
+      const bool kin = k >= 0 && k < p.nz, wk = (k == 0) && !p.z_lo_open;
 #pragma unroll
-    for (int v = 0; v < V; ++v) {
-      const bool in = jin && kin && xin[v], wi = (i0 + v == 0);
-      if (!in || wj || wk) ex[v] = T(0);
-      if (!in || wi || wk) ey[v] = T(0);
-      if (!in || wi || wj) ez[v] = T(0);
+      for (int v = 0; v < V; ++v) {
+        const bool in = jin && kin && xin[v], wi = (i0 + v == 0);
+        if (!in || wj || wk) ex[v] = T(0);
+        if (!in || wi || wk) ey[v] = T(0);
+        if (!in || wi || wj) ez[v] = T(0);
+      }
     }
   };
   // per-cell Db of plane offset o (permeability given), zero outside the grid
@@ -234,7 +252,12 @@ __global__ void __launch_bounds__((R + 1) * 32, 1) k_step2(const __grid_constant
   unsigned ph = 0, phprev = 0;
   long long o = orow + p.PS * (long long)(k0 - 3);
 
-  for (int it = 0; it < nIt; ++it, o += p.PS) {
+  // One plane iteration.  ST (steady state) = every half step of this row runs in this iteration: the row owns cells
+  // (rowE2) and it >= 4.  The priming iterations and the rows at the rim of the computed region (which skip the half steps
+  // their results are not valid for) take the general form, which tests each half step and zero-fills what it skips; the
+  // steady form carries no such tests and no fills (36 % of the instructions of the first version of this loop).
+  auto plane = [&](auto steady, const int it) {
+    constexpr bool ST = decltype(steady)::value;
     const int k = k0 - 3 + it, kb = k - 1;
     const unsigned char* st = smem + s * C::STAGE;
     const T* sEx = reinterpret_cast<const T*>(st + C::off(kEx));
@@ -263,9 +286,11 @@ __global__ void __launch_bounds__((R + 1) * 32, 1) k_step2(const __grid_constant
     if (lane == 31) eyi1 = sEy[oEy + V];
     T hx[V], hy[V], hz[V], ez[V];
     T nex[V], ney[V], nez[V];                    // E1 of plane k
+    if (!ST) {
 #pragma unroll
-    for (int v = 0; v < V; ++v) { hx[v] = hy[v] = hz[v] = ez[v] = nex[v] = ney[v] = nez[v] = T(0); mi[v] = 0; }
-    if (it >= 1) {
+      for (int v = 0; v < V; ++v) { hx[v] = hy[v] = hz[v] = ez[v] = nex[v] = ney[v] = nez[v] = T(0); mi[v] = 0; }
+    }
+    if (ST || it >= 1) {
       // ---------------- H1(k) = H^{n-1/2}(k) - Db curl E^n ------------------------------------------------------------------
       T ezj[V];
       ldv(sEz + oEz, ez); ldv(sEz + oEz + WEz, ezj);
@@ -301,7 +326,7 @@ __global__ void __launch_bounds__((R + 1) * 32, 1) k_step2(const __grid_constant
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(&rdy1[s * R + r]);
-    if (it >= 2 && r >= 1) {
+    if (ST || (it >= 2 && r >= 1)) {
       // ---------------- E1(k) = Ca E^n(k) + Cb curl H1 ----------------------------------------------------------------------
       mbar_wait(&rdy1[s * R + r - 1], ph);
 #pragma unroll
@@ -324,14 +349,25 @@ __global__ void __launch_bounds__((R + 1) * 32, 1) k_step2(const __grid_constant
 #pragma unroll
       for (int v = 0; v < V; ++v) { nex[v] = ex0[v]; ney[v] = ey0[v]; nez[v] = ez[v]; }
       e_update(nex, ney, nez, ax, ay, az, mi, o, k);
+      if (srcmask != 0) {   // R5 step 3 of the first step, in port order (overlapping source boxes add up as k_source adds them)
+        const double t = (double)(*p.nstep - 1) * fp.dt;
+        for (int q = 0; q < fp.nsrc; ++q) {
+          if (!((srcmask >> q) & 1u) || k < fp.src[q].sk0 || k >= fp.src[q].sk1) continue;
+          const T g = (T)(fp.src[q].amp * waveform_dev(fp.src[q].waveform, t, fp.src[q].t0, fp.src[q].sigma, fp.src[q].f0));
+#pragma unroll
+          for (int v = 0; v < V; ++v) if (i0 + v == fp.src[q].is) nez[v] += g;
+        }
+      }
       stv(xeb + oH, nex); stv(xeb + R * TX + oH, nez);
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(&rdyE[s * R + r]);
     T g2x[V], g2y[V], g2z[V];                    // H2 of plane k-1
+    if (!ST) {
 #pragma unroll
-    for (int v = 0; v < V; ++v) { g2x[v] = g2y[v] = g2z[v] = T(0); }
-    if (it >= 3 && rowB) {
+      for (int v = 0; v < V; ++v) { g2x[v] = g2y[v] = g2z[v] = T(0); }
+    }
+    if (ST || (it >= 3 && rowB)) {
       // ---------------- H2(k-1) = H1(k-1) - Db curl E1 ---------------------------------------------------------------------
       mbar_wait(&rdyE[sprev * R + r + 1], phprev);
       T exj[V], ezj[V];
@@ -361,14 +397,14 @@ __global__ void __launch_bounds__((R + 1) * 32, 1) k_step2(const __grid_constant
         }
       }
       stv(x2b + oH, g2x); stv(x2b + R * TX + oH, g2z);
-      if (own_xy && it >= 4) {
+      if (own_xy && (ST || it >= 4)) {
         const long long ob = o - p.PS;
         stv_stream(p.dst[kHx] + ob, g2x); stv_stream(p.dst[kHy] + ob, g2y); stv_stream(p.dst[kHz] + ob, g2z);
       }
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(&rdy2[s * R + r]);
-    if (it >= 4 && rowE2) {
+    if (ST || (it >= 4 && rowE2)) {
       // ---------------- E2(k-1) = Ca E1(k-1) + Cb curl H2 -------------------------------------------------------------------
       mbar_wait(&rdy2[s * R + r - 1], ph);
       T hxj[V], hzj[V];
@@ -410,7 +446,14 @@ __global__ void __launch_bounds__((R + 1) * 32, 1) k_step2(const __grid_constant
     eyi0 = eyi1;
     sprev = s; phprev = ph;
     if (++s == NS) { s = 0; ph ^= 1u; }
-  }
+    o += p.PS;
+  };
+
+  int it = 0;
+  const int n_general = rowE2 ? min(4, nIt) : nIt;
+  for (; it < n_general; ++it) plane(std::false_type{}, it);
+#pragma unroll 2
+  for (; it < nIt; ++it) plane(std::true_type{}, it);
 }
 
 }  // namespace fdtd_b200

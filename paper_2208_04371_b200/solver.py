@@ -154,6 +154,14 @@ class Solver:
     def fused_kz(self):
         return B.fdtd_fused_kz(self.h)
 
+    @property
+    def fused_tile(self):
+        return B.fdtd_fused_tile(self.h)
+
+    @property
+    def two_step_box(self):
+        return B.fdtd_two_step_box(self.h)
+
     # ---- z-slab stepping (include/fdtd.h "domain decomposition along z") ------------------------------------------
     def step_begin(self):
         B.fdtd_step_begin(self.h)

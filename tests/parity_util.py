@@ -9,9 +9,23 @@ import numpy as np
 import pytest
 
 from oracle.yee import YeeOracle
-from paper_2208_04371_b200 import FDTD_F64, FDTD_OPT_STEP_IMPL, FdtdError, Solver
+from paper_2208_04371_b200 import FDTD_F64, FDTD_OPT_FUSED_TILE, FDTD_OPT_STEP_IMPL, FdtdError, Solver
 
 TOL = {32: 1e-4, 64: 1e-11}
+
+# Step implementations the parity tests run through: FDTD_OPT_STEP_IMPL 1 = two-pass kernels, 2 = fused E+H kernel (TMA-staged,
+# ping-pong field sets) on its 14-row tile, 3 = persistent, 4 = two steps per pass on a box + one-step kernels on the shell
+# (skipped where the grid leaves no such box); 26 = the fused kernel on its 6-row tile (FDTD_OPT_FUSED_TILE = 2: two blocks
+# per SM, the mid-size-grid build).
+IMPLS = [1, 2, 3, 4, 26]
+
+
+def impl_opts(impl, more=None):
+    """fdtd_set_option dictionary of a test's step implementation id (IMPLS) plus further options."""
+    o = {FDTD_OPT_STEP_IMPL: 2, FDTD_OPT_FUSED_TILE: 2} if impl == 26 else \
+        {FDTD_OPT_STEP_IMPL: 2, FDTD_OPT_FUSED_TILE: 1} if impl == 2 else {FDTD_OPT_STEP_IMPL: impl}
+    o.update(more or {})
+    return o
 
 
 def solver_or_skip(w, precision=None, options=None, **kw):

@@ -5,7 +5,7 @@ import numpy as np
 import pytest
 
 import workloads as W
-from paper_2208_04371_b200 import FDTD_F32, FDTD_F64, FDTD_OPT_FUSED_KZ, FDTD_OPT_STEP_IMPL, FdtdError, Solver
+from paper_2208_04371_b200 import FDTD_F32, FDTD_F64, FDTD_OPT_FUSED_KZ, FDTD_OPT_FUSED_TILE, FDTD_OPT_STEP_IMPL, FdtdError, Solver
 from tests.parity_util import TOL, run_pair
 
 pytestmark = pytest.mark.gpu
@@ -35,6 +35,7 @@ def test_random_configurations_against_the_oracle(seed):
         opts = {FDTD_OPT_STEP_IMPL: c["impl"]}
         if c["impl"] == 2:
             opts[FDTD_OPT_FUSED_KZ] = c["kz"]
+            opts[FDTD_OPT_FUSED_TILE] = 1 + (c["case"] + seed) % 2      # both tile shapes of the fused kernel
         o, s, rep = run_pair(w, c["steps"], precision=c["prec"], options=opts, checkpoints=[max(1, c["steps"] // 2), c["steps"]])
         assert rep["emax"] > 0, c
         assert rep["field_err"].max() <= TOL[c["prec"]], (c, rep["field_err"])

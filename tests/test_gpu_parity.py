@@ -14,13 +14,12 @@ from oracle.yee import YeeOracle
 from paper_2208_04371_b200 import (FDTD_F32, FDTD_F64, FDTD_OPT_GRAPH_UNROLL, FDTD_OPT_STEP_IMPL, FDTD_OPT_USE_GRAPH,
                                    FdtdError, Solver, sparams)
 
-from .parity_util import TOL, assert_fields, run_pair, solver_or_skip
+from .parity_util import IMPLS, TOL, assert_fields, impl_opts, run_pair, solver_or_skip
 
 pytestmark = pytest.mark.gpu
 
-# FDTD_OPT_STEP_IMPL: 1 = two-pass kernels, 2 = fused E+H kernel (TMA-staged, ping-pong field sets), 3 = persistent,
+# IMPLS (parity_util): 1 = two-pass kernels, 2 / 26 = fused E+H kernel on its 14-row / 6-row tile, 3 = persistent,
 # 4 = two steps per pass on a box + one-step kernels on the shell (skipped where the grid leaves no such box)
-IMPLS = [1, 2, 3, 4]
 
 
 @pytest.mark.parametrize("impl", IMPLS)
@@ -34,7 +33,7 @@ IMPLS = [1, 2, 3, 4]
 def test_random_box_every_term(seed, indexed, with_mu, pml, prec, impl):
     """Random eps / sigma / mu blocks, PEC cells, kappa != 1, alpha != 0, mixed CPML faces, driven + passive port."""
     w = W.random_box(seed, indexed=indexed, with_mu=with_mu, pml=pml, steps=60, precision=prec)
-    o, s, rep = run_pair(w, 60, precision=prec, options={FDTD_OPT_STEP_IMPL: impl}, checkpoints=[1, 2, 17, 60])
+    o, s, rep = run_pair(w, 60, precision=prec, options=impl_opts(impl), checkpoints=[1, 2, 17, 60])
     assert_fields(rep, prec)
     dv, di = rep["dft_err"]
     assert max(dv, di) <= (1e-11 if prec == FDTD_F64 else 1e-4)
@@ -66,10 +65,10 @@ def test_ragged_shapes(shape, prec, impl):
         init[0][:, 0, :] = 0; init[0][0] = 0
         init[1][:, :, 0] = 0; init[1][0] = 0
         init[2][:, :, 0] = 0; init[2][:, 0, :] = 0
-        o, s, rep = run_pair(w, 30, precision=prec, options={FDTD_OPT_STEP_IMPL: impl}, init_fields=init)
+        o, s, rep = run_pair(w, 30, precision=prec, options=impl_opts(impl), init_fields=init)
     else:
         w = W.random_box(7, nx=nx, ny=ny, nz=nz, pml=pml, steps=50, precision=prec)
-        o, s, rep = run_pair(w, 50, precision=prec, options={FDTD_OPT_STEP_IMPL: impl}, checkpoints=[3, 50])
+        o, s, rep = run_pair(w, 50, precision=prec, options=impl_opts(impl), checkpoints=[3, 50])
     assert_fields(rep, prec)
 
 
@@ -96,7 +95,8 @@ def test_P2_exact_discrete_eigenmode_on_gpu(impl):
     f = dt / (2 * mu0)
     s = Solver(nx, ny, nz, dx, dy, dz, dt, FDTD_F64)
     s.set_material_mode(1)
-    s.set_option(FDTD_OPT_STEP_IMPL, impl)
+    for opt, val in impl_opts(impl).items():
+        s.set_option(opt, val)
     s.commit()
     for c, a in enumerate([Ex, Ey, Ez, f * Hx, f * Hy, f * Hz]):
         s.write_fields(c, np.ascontiguousarray(a))
@@ -113,7 +113,7 @@ def test_P2_exact_discrete_eigenmode_on_gpu(impl):
 def test_C0_cavity_full(impl):
     """Config C0 as written: 32^3 fp64 PEC cavity, 2000 steps, fields <= 1e-11 of the running maximum."""
     w = W.cavity_c0()
-    o, s, rep = run_pair(w, 2000, options={FDTD_OPT_STEP_IMPL: impl}, checkpoints=[100, 500, 1000, 2000])
+    o, s, rep = run_pair(w, 2000, options=impl_opts(impl), checkpoints=[100, 500, 1000, 2000])
     assert_fields(rep, FDTD_F64)
 
 
@@ -130,7 +130,7 @@ def _sstar(sim_inc, sim_tot, nports, module):
 def test_C1_microstrip_fields_and_sparams(impl):
     """Config C1 geometry at full size, first 1500 steps: fp32 fields, raw DFTs and S* (C1: tot == inc, R22)."""
     w = W.microstrip_c1(steps=1500)
-    o, s, rep = run_pair(w, 1500, options={FDTD_OPT_STEP_IMPL: impl}, checkpoints=[100, 700, 1500])
+    o, s, rep = run_pair(w, 1500, options=impl_opts(impl), checkpoints=[100, 700, 1500])
     assert_fields(rep, FDTD_F32)
     So = _sstar(o, o, 2, osp)
     Sg = _sstar(s, s, 2, sparams)
@@ -144,7 +144,7 @@ def test_C2_quarter_scale_inc_tot_sparams(impl):
     sims = {}
     for run in ("inc", "tot"):
         w = W.interconnect_c2(run=run, div=4, steps=1200, npml=6, nf=32)
-        o, s, rep = run_pair(w, 1200, options={FDTD_OPT_STEP_IMPL: impl}, checkpoints=[300, 1200])
+        o, s, rep = run_pair(w, 1200, options=impl_opts(impl), checkpoints=[300, 1200])
         assert_fields(rep, FDTD_F32)
         sims[run] = (o, s)
     So = _sstar(sims["inc"][0], sims["tot"][0], 2, osp)
@@ -156,7 +156,7 @@ def test_C2_quarter_scale_inc_tot_sparams(impl):
 def test_C4_eighth_scale_fp64_full_coefficients(impl):
     """Config C4 at 1/8 linear scale (128x64x32), fp64, full anisotropic arrays, 4 ports: 1e-11."""
     w = W.interconnect_c4(run="tot", div=8, steps=400, npml=5, nf=16)
-    o, s, rep = run_pair(w, 400, options={FDTD_OPT_STEP_IMPL: impl}, checkpoints=[50, 400])
+    o, s, rep = run_pair(w, 400, options=impl_opts(impl), checkpoints=[50, 400])
     assert_fields(rep, FDTD_F64)
     assert max(rep["dft_err"]) <= 1e-11
 
@@ -165,7 +165,7 @@ def test_C4_eighth_scale_fp64_full_coefficients(impl):
 def test_C3_small_scale_indexed_six_face_cpml(impl):
     """Config C3's generator at 1/8 linear scale (192x96x96): 64-entry table, six CPML faces, 4 ports, fp32."""
     w = W.throughput_c3(div=8, steps=300, npml=6, nf=16)
-    o, s, rep = run_pair(w, 300, options={FDTD_OPT_STEP_IMPL: impl}, checkpoints=[20, 300])
+    o, s, rep = run_pair(w, 300, options=impl_opts(impl), checkpoints=[20, 300])
     assert_fields(rep, FDTD_F32)
     # the S* column of port 1 over the four ports (one structure: tot == inc, so S*_11 = 0 and the rest are transfer ratios)
     So, Sg = _sstar(o, o, 4, osp), _sstar(s, s, 4, sparams)
@@ -180,7 +180,7 @@ def test_graph_replay_equals_plain_launches(impl):
     w = W.random_box(11, nx=40, ny=22, nz=18, steps=27, precision=FDTD_F32)
     out = []
     for graph in (0, 1):
-        s = solver_or_skip(w, options={FDTD_OPT_STEP_IMPL: impl, FDTD_OPT_USE_GRAPH: graph, FDTD_OPT_GRAPH_UNROLL: 4})
+        s = solver_or_skip(w, options=impl_opts(impl, {FDTD_OPT_USE_GRAPH: graph, FDTD_OPT_GRAPH_UNROLL: 4}))
         assert s.stream.cuda_stream != 0
         if graph:
             s.step(27)
@@ -328,7 +328,7 @@ def test_fused_equals_two_pass_closely():
     w = W.throughput_c3(div=8, steps=100, npml=6, nf=8)
     out = []
     for impl in (1, 2):
-        s = Solver.from_workload(w, options={FDTD_OPT_STEP_IMPL: impl})
+        s = Solver.from_workload(w, options=impl_opts(impl))
         s.step(100)
         out.append([s.read_fields(c).cpu().numpy().astype(np.float64) for c in range(6)])
         s.destroy()
@@ -337,7 +337,31 @@ def test_fused_equals_two_pass_closely():
         assert np.abs(out[0][c] - out[1][c]).max() / scale < 2e-6
 
 
-@pytest.mark.parametrize("impl", [2, 3, 4])
+def test_fused_result_does_not_depend_on_tile_chunk_or_what_commit_selected():
+    """Every cell is advanced by the same operations in the same order whatever tile owns it and whichever block recomputes
+    it as halo, so the fused step's result is bit-identical across tile shapes (FDTD_OPT_FUSED_TILE), chunk lengths
+    (FDTD_OPT_FUSED_KZ) and the configuration fdtd_commit selects by measurement (which may differ from run to run): the
+    auto-selected configuration is reproducible in its RESULT even where its choice is not."""
+    from paper_2208_04371_b200 import FDTD_OPT_FUSED_KZ, FDTD_OPT_FUSED_TILE
+    w = W.throughput_c3(div=4, steps=40, npml=8, nf=8)
+    outs, names = [], []
+    for opts in ({FDTD_OPT_FUSED_TILE: 1, FDTD_OPT_FUSED_KZ: 12}, {FDTD_OPT_FUSED_TILE: 2, FDTD_OPT_FUSED_KZ: 7},
+                 {FDTD_OPT_FUSED_TILE: 2, FDTD_OPT_FUSED_KZ: 32}, {}, {}):
+        s = Solver.from_workload(w, options={FDTD_OPT_STEP_IMPL: 2, **opts})
+        assert s.impl_name == "fused" and s.fused_tile in (1, 2)
+        if FDTD_OPT_FUSED_TILE in opts:
+            assert (s.fused_tile, s.fused_kz) == (opts[FDTD_OPT_FUSED_TILE], opts[FDTD_OPT_FUSED_KZ])
+        names.append((s.fused_tile, s.fused_kz))
+        s.step(40)
+        outs.append([s.read_fields(c).clone() for c in range(6)] + [torch_dft(s)])
+        s.destroy()
+    for name, other in zip(names[1:], outs[1:]):
+        for a, b in zip(outs[0][:6], other[:6]):
+            assert bool((a == b).all()), name
+        assert np.array_equal(outs[0][6], other[6]), name
+
+
+@pytest.mark.parametrize("impl", [2, 26, 3, 4])
 def test_repeated_runs_are_bitwise_identical(impl):
     """The fused kernel synchronises its warps with mbarriers only (TMA ring, row-to-row and column hand-over) and the
     persistent kernel with grid barriers: a missing edge in either protocol shows up as run-to-run differences.  Many
@@ -347,7 +371,7 @@ def test_repeated_runs_are_bitwise_identical(impl):
     w = W.throughput_c3(div=4, steps=60, npml=8, nf=8)          # 384x192x192: 3 x 14 x 16 blocks of the fused kernel
     outs = []
     for _ in range(3):
-        s = Solver.from_workload(w, options={FDTD_OPT_STEP_IMPL: impl, FDTD_OPT_FUSED_KZ: 12})
+        s = Solver.from_workload(w, options=impl_opts(impl, {FDTD_OPT_FUSED_KZ: 12}))
         s.step(60)
         outs.append([s.read_fields(c).clone() for c in range(6)] + [torch_dft(s)])
         s.destroy()
@@ -373,7 +397,7 @@ def test_two_overlapping_sources_and_thick_slabs(impl):
     extra.update({"is": p0["is"], "sj0": p0["sj0"] - 1, "sj1": p0["sj1"], "sk0": p0["sk0"], "sk1": p0["sk1"] + 1,
                   "waveform": 2, "f0": 3.0 / (80 * w["dt"]), "amp": -0.7, "ip": p0["ip"] + 3})
     w = dict(w, ports=[p0, w["ports"][1], extra])
-    o, s, rep = run_pair(w, 80, options={FDTD_OPT_STEP_IMPL: impl}, checkpoints=[1, 40, 80])
+    o, s, rep = run_pair(w, 80, options=impl_opts(impl), checkpoints=[1, 40, 80])
     assert_fields(rep, FDTD_F32)
     assert max(rep["dft_err"]) <= 1e-5
     s.destroy()
@@ -408,22 +432,38 @@ def test_two_step_box_alone_on_a_pec_box(prec, nsteps, mats):
 
 
 @pytest.mark.parametrize("prec", [FDTD_F64, FDTD_F32])
+@pytest.mark.parametrize("shift", [0, 57])
 @pytest.mark.parametrize("pml", [(5, 6, 4, 3, 0, 5), (4, 4, 4, 4, 4, 4), (0, 7, 0, 5, 3, 0)])
-def test_two_step_box_with_cpml_shell_and_ports(prec, pml):
-    """CPML on some or all faces and two ports: the box keeps two cells from the layers and stays between the port planes;
-    the shell (CPML cells, the band around them, the port planes) is advanced by the region launches of the two-pass
-    kernels, whose intermediate values in the band the box kernel then overwrites.  Fields at an even and an odd step
-    count, the probes of BOTH steps of every pair (raw DFTs)."""
+def test_two_step_box_with_cpml_shell_and_ports(prec, pml, shift):
+    """CPML on some or all faces and ports: the box keeps two cells from the layers; the shell (CPML cells and the band
+    around them) is advanced by the region launches of the two-pass kernels, whose intermediate values in the band the box
+    kernel then overwrites.  shift = 0: the generator's ports next to the x- layer (source plane on the last shell plane or,
+    without a layer there, inside the box; probe plane inside the box).  shift = 57: source and probe planes deep inside the
+    box (the kernel adds the first step's source itself, the probes of that step read the recomputed band around the port
+    plane), a second driving port whose source box overlaps the first one with another waveform, and its probe plane in a
+    different vector of the row.  Fields at an even and an odd step count, the probes of BOTH steps of every pair (raw DFTs)."""
     w = W.random_box(54, nx=300, ny=44, nz=40, pml=pml, steps=41, precision=prec)
+    if shift:
+        ports = [dict(q) for q in w["ports"]]
+        ports[0]["is"] += shift
+        ports[0]["ip"] += shift + 2
+        extra = dict(ports[0])
+        extra.update({"sj0": extra["sj0"] - 1, "sk1": extra["sk1"] + 1, "waveform": 2, "f0": 2.0 / (41 * w["dt"]), "amp": -0.6,
+                      "ip": extra["ip"] + 3})
+        w = dict(w, ports=ports + [extra])
     o, s, rep = run_pair(w, 41, precision=prec, options={FDTD_OPT_STEP_IMPL: 4}, checkpoints=[2, 12, 41])
     assert s.impl_name == "two_step"
+    b = s.two_step_box
+    V = 4 if prec == FDTD_F32 else 2
+    assert b[0] == (-(-(pml[0] + 2) // V) * V if pml[0] else 0)                  # the box is set by the CPML layers alone:
+    assert b[2] == (pml[2] + 2 if pml[2] else 0) and b[4] == (pml[4] + 2 if pml[4] else 0)   # ports do not shrink it
     assert_fields(rep, prec, tol=(1e-12 if prec == FDTD_F64 else 1e-5))
     assert max(rep["dft_err"]) <= (1e-11 if prec == FDTD_F64 else 1e-5)
     s.destroy()
 
 
 def test_two_step_refuses_grids_without_a_box():
-    """A grid whose CPML layers (or port planes) leave no 32 x 8 x 8 box is an error for FDTD_OPT_STEP_IMPL = 4, not a silent
+    """A grid whose CPML layers leave no 32 x 8 x 8 box is an error for FDTD_OPT_STEP_IMPL = 4, not a silent
     change of implementation; so is a z slab."""
     w = W.random_box(1, steps=4, precision=FDTD_F32)            # 20 x 14 x 12
     with pytest.raises(FdtdError) as e:
