@@ -1096,13 +1096,15 @@ static void region_launch(bool isH, const StepParams<T>& q, int nk, cudaStream_t
   else k_update_E<T, MODE, false, true><<<grid, block, 0, st>>>(q);
 }
 
-// One half step of the shell: every cell outside the box shrunk by d cells (d whole vectors in x) on its open sides.  The
+// One half step of the shell: every cell outside the box shrunk by d cells (in x: by the whole vectors that hold d cells) on
+// its open sides.  Half step d of the sequence 3, 2, 1, 0 needs the results of the one before on the cells up to d + 1 deep
+// only; what a whole vector computes beyond that is overwritten by the box kernel before anybody reads it.  The
 // complement of that inner box is cut into at most six disjoint boxes (two z slabs over the full planes, two y slabs between
 // them, two x slabs between those).  Returns the number of launches (the first one carries the step-counter bump if asked).
 template <typename T>
 int Solver<T>::shell_pass(bool isH, int d, const StepParams<T>& base, bool bump) {
-  const int V = vlen();
-  const int ix0 = box[0] > 0 ? box[0] + d * V : 0, ix1 = box[1] < nx ? box[1] - d * V : nx;
+  const int V = vlen(), dx_ = (d + V - 1) / V * V;   // x in whole vectors: the cells beyond d hold values nobody reads
+  const int ix0 = box[0] > 0 ? box[0] + dx_ : 0, ix1 = box[1] < nx ? box[1] - dx_ : nx;
   const int iy0 = box[2] > 0 ? box[2] + d : 0, iy1 = box[3] < ny ? box[3] - d : ny;
   const int iz0 = box[4] > 0 ? box[4] + d : 0, iz1 = box[5] < nz ? box[5] - d : nz;
   const int reg[6][6] = {{0, nx, 0, ny, 0, iz0},     {0, nx, 0, ny, iz1, nz},   {0, nx, 0, iy0, iz0, iz1},
@@ -1139,8 +1141,8 @@ void Solver<T>::region_pass(bool isH, const StepParams<T>& base, const int* r, b
 // it has already advanced -- a second update would advance the psi of a CPML cell twice.
 template <typename T>
 void Solver<T>::band_pass(bool isH, const StepParams<T>& base) {
-  const int V = vlen(), d = isH ? 3 : 2, grow = isH ? 1 : 0;
-  const int ix0 = box[0] > 0 ? box[0] + d * V : 0, ix1 = box[1] < nx ? box[1] - d * V : nx;
+  const int V = vlen(), d = isH ? 3 : 2, grow = isH ? 1 : 0, dx_ = (d + V - 1) / V * V;
+  const int ix0 = box[0] > 0 ? box[0] + dx_ : 0, ix1 = box[1] < nx ? box[1] - dx_ : nx;
   const int iy0 = box[2] > 0 ? box[2] + d : 0, iy1 = box[3] < ny ? box[3] - d : ny;
   const int iz0 = box[4] > 0 ? box[4] + d : 0, iz1 = box[5] < nz ? box[5] - d : nz;
   for (const Band& g : bands) {
