@@ -1,6 +1,6 @@
 """bench.py -- throughput of the Yee FDTD hot path on config C3 (BASELINE.json: "Mcell-updates/s per Yee E+H step").
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload c3|c3s|c2|c4|x3]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload c3|c3s|c0|c1|c2|c4|x3|w600]
 
 One "step" is one full leapfrog step of the whole hot path (psi_H, H, psi_E, E, walls, source,
 probes, running DFT) over the whole grid.  One cell-update = all six components of one cell advanced one step (R27);
@@ -12,6 +12,8 @@ N counts the CPML cells.  Prints ONE JSON line (rank 0).
                 host->device (fdtd_set_materials_indexed), fdtd_reset, K steps, every port's DFT device->host
   roofline      dominant kernel: algorithmic bytes per launch / its average duration from CUDA events
                 (fdtd_profile_step) vs MEASURED_PEAKS.json hbm_gbs
+  fused_step    c3 only, when fdtd_commit selected two steps per pass: the one-step fused E+H kernel on the same workload and
+                step count, with its own roofline object (north_star's 70 % target is stated for that kernel's byte model)
   sustained     BASELINE.json's "2000 steps timed" on C3, with its own clock samples, whatever --steps says (c3 only;
                 --sustained-steps 0 switches it off)
   cpu_baseline  the fp64 oracle, as it stands, on the host cores (all cores, and one thread), on the z-cropped
@@ -87,6 +89,12 @@ def workload(name, steps):
         return W.interconnect_c2(steps=steps)
     if name == "c4":
         return W.interconnect_c4(steps=steps)
+    if name == "c0":
+        return W.cavity_c0(steps=steps)
+    if name == "c1":
+        return W.microstrip_c1(steps=steps)
+    if name == "w600":  # the paper's per-GPU load of its weak-scaling study (Table I): 600^3 cells, C3's generator
+        return W.weak_scaling_600(n_slabs=1, steps=steps)
     if name == "x3":  # the paper's CMOS-line grid shape, 200x120x800 cells of (20, 50, 5) nm
         return W.cmos_line_x3(steps=steps)
     raise SystemExit(f"unknown workload {name}")
@@ -434,6 +442,30 @@ def run_ours(args, rank, world, local_rank):
     s.destroy()
     del s
     torch.cuda.empty_cache()
+    # ---- the one-step fused kernel beside a two-step headline (c3): north_star's ">= 70 % of HBM bandwidth for the fused E+H step" is
+    # a statement about THAT kernel's 49 B + psi per cell-update; the same K steps, timed the same way, on a second handle
+    if impl == "two_step" and args.workload == "c3" and not args.step_impl and not args.no_fused_leg:
+        s1 = Solver.from_workload(w, options={FDTD_OPT_STEP_IMPL: 2}, device=str(dev))
+        s1.step(Wm)
+        barrier()
+        e0.record(s1.stream)
+        s1.step(K)
+        e1.record(s1.stream)
+        barrier()
+        t1 = max_over_ranks(e0.elapsed_time(e1) * 1e-3, world, dev)
+        m1 = s1.profile_step(max(3, min(20, K)))
+        ab1 = algorithmic_bytes(w, "fused", "H")
+        tr1, tr1_src = ncu_traffic(args.workload, "k_step_fused", "f32" if w["precision"] == 32 else "f64", s1.fused_kz)
+        line["fused_step"] = {"what": "FDTD_OPT_STEP_IMPL = 2 (one step per pass), same workload, same K steps",
+                              "ms_per_step": t1 / K * 1e3, "value": job_throughput(n_cells, K, world, t1), "unit": UNIT,
+                              "fused_kz": s1.fused_kz, "fused_tile": s1.fused_tile,
+                              "roofline": {"bound": "hbm", "kernel": "k_step_fused", "achieved": ab1 / (m1[0] * 1e-3) / 1e9, "peak": peak,
+                                           "unit": "GB/s", "frac": ab1 / (m1[0] * 1e-3) / 1e9 / peak, "traffic": tr1,
+                                           "traffic_source": tr1_src, "algorithmic_bytes_per_launch": ab1, "kernel_ms": m1[0],
+                                           "frac_of_8000": ab1 / (m1[0] * 1e-3) / 1e9 / 8000.0}}
+        s1.destroy()
+        del s1
+        torch.cuda.empty_cache()
     if rank == 0 and world == 1 and not args.no_cpu:
         r = oracle_sample(budget_s=args.cpu_budget, one_thread=True)
         line["cpu_baseline"] = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"],
@@ -559,6 +591,7 @@ def main():
     ap.add_argument("--step-impl", type=int, default=0, help="FDTD_OPT_STEP_IMPL: 0 auto, 1 two-pass, 2 fused, 3 persistent, 4 two steps per pass")
     ap.add_argument("--fused-kz", type=int, default=0, help="FDTD_OPT_FUSED_KZ: planes per z chunk (0 = measured at commit)")
     ap.add_argument("--fused-tile", type=int, default=0, help="FDTD_OPT_FUSED_TILE: 0 measured at commit, 1 = 14-row tiles, 2 = 6-row tiles")
+    ap.add_argument("--no-fused-leg", action="store_true", help="c3, two steps per pass selected: skip the one-step fused kernel's leg")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--cpu-budget", type=float, default=15.0)
     ap.add_argument("--sustained-steps", type=int, default=2000,

@@ -984,7 +984,7 @@ int Solver<T>::setup_persistent() {
 #define FDTD_STEP2_R 11
 #endif
 #ifndef FDTD_STEP2_NS
-#define FDTD_STEP2_NS 3
+#define FDTD_STEP2_NS 4
 #endif
 static_assert(Step2Cfg<float, FDTD_STEP2_R, FDTD_STEP2_NS>::SMEM <= 232448 && Step2Cfg<double, FDTD_STEP2_R, FDTD_STEP2_NS>::SMEM <= 232448,
               "two-step kernel: rows x stages exceed the 227 KB shared memory of an sm_100 CTA");

@@ -23,8 +23,11 @@
 //     H2 valid for 1 <= r <= R-2, 1 <= c <= 126,                                  E2 valid for 2 <= r <= R-2, 2 <= c <= 126.
 // A tile of R computed rows x 32 lanes therefore OWNS rows 2..R-2 and lanes 1..30 (vector granularity): (R-3) x 30 V cells.
 // In z the same cone costs three priming planes per chunk.  Hand-over between neighbouring rows goes through three
-// shared-memory rings (new Hx,Hz of H1; new Ex,Ez of E1; new Hx,Hz of H2) with one mbarrier per (slot, row); x neighbours
-// come from warp shuffles; the planes k-1 a row needs are carried in registers.
+// shared-memory buffers (new Hx,Hz of H1; new Ex,Ez of E1; new Hx,Hz of H2), two slots each (plane parity), with one
+// mbarrier per (slot, row); x neighbours come from warp shuffles; the planes k-1 a row needs are carried in registers.
+// Two slots are enough because a row cannot start plane k+2 before the row above has finished plane k: its H2 waits for
+// that row's E1 of the plane before (row 0, which computes no H2, takes the same wait for that reason alone).  The shared
+// memory this leaves holds a fourth TMA stage (C3: 4.36 -> 4.27 ms per step of the box).
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>
@@ -67,9 +70,9 @@ struct Step2Cfg {
   static constexpr int STAGE = off(6);
   static constexpr int XSLOT = 2 * R * TX * (int)sizeof(T);   // one hand-over slot: [2 fields][R rows][TX]
   static constexpr int TAB_B = kTabH * (int)sizeof(T);
-  static constexpr int NBAR = 2 * NS + 3 * NS * R;
+  static constexpr int NX = 2, NBAR = 2 * NS + 3 * NX * R;
   static constexpr int BAR_B = round128(NBAR * 8);
-  static constexpr int O_X1 = NS * STAGE, O_XE = O_X1 + NS * XSLOT, O_X2 = O_XE + NS * XSLOT, O_TAB = O_X2 + NS * XSLOT,
+  static constexpr int O_X1 = NS * STAGE, O_XE = O_X1 + NX * XSLOT, O_X2 = O_XE + NX * XSLOT, O_TAB = O_X2 + NX * XSLOT,
                        O_BAR = O_TAB + TAB_B;
   static constexpr int SMEM = O_BAR + BAR_B;
   static constexpr int THREADS = (R + 1) * 32;
@@ -95,8 +98,8 @@ __global__ void __launch_bounds__((R + 1) * 32, 1) k_step2(const __grid_constant
   uint64_t* const full = reinterpret_cast<uint64_t*>(smem + C::O_BAR);
   uint64_t* const empty = full + NS;
   uint64_t* const rdy1 = full + 2 * NS;            // [NS][R] H1 row in x1
-  uint64_t* const rdyE = rdy1 + NS * R;            // [NS][R] E1 row in xe
-  uint64_t* const rdy2 = rdyE + NS * R;            // [NS][R] H2 row in x2
+  uint64_t* const rdyE = rdy1 + C::NX * R;            // [NS][R] E1 row in xe
+  uint64_t* const rdy2 = rdyE + C::NX * R;            // [NS][R] H2 row in x2
   constexpr int XS = C::XSLOT / (int)sizeof(T);
 
   const StepParams<T>& p = fp.sp;
@@ -135,8 +138,9 @@ __global__ void __launch_bounds__((R + 1) * 32, 1) k_step2(const __grid_constant
     for (int s = 0; s < NS; ++s) {
       mbar_init(&full[s], 1);
       mbar_init(&empty[s], R);
-      for (int r = 0; r < R; ++r) { mbar_init(&rdy1[s * R + r], 1); mbar_init(&rdyE[s * R + r], 1); mbar_init(&rdy2[s * R + r], 1); }
     }
+    for (int s = 0; s < C::NX; ++s)
+      for (int r = 0; r < R; ++r) { mbar_init(&rdy1[s * R + r], 1); mbar_init(&rdyE[s * R + r], 1); mbar_init(&rdy2[s * R + r], 1); }
     mbar_fence_init();
     for (int it = 0; it < NS && it < nIt; ++it) issue(it, it);
   }
@@ -266,10 +270,12 @@ __global__ void __launch_bounds__((R + 1) * 32, 1) k_step2(const __grid_constant
     const T* sHx = reinterpret_cast<const T*>(st + C::off(kHx));
     const T* sHy = reinterpret_cast<const T*>(st + C::off(kHy));
     const T* sHz = reinterpret_cast<const T*>(st + C::off(kHz));
-    T* const x1b = x1 + s * XS;
-    T* const xeb = xe + s * XS;
-    T* const x2b = x2 + s * XS;
-    const T* const xep = xe + sprev * XS;       // E1 of plane k-1, written during the previous iteration
+    const int xs = it & 1, xsp = xs ^ 1;
+    const unsigned xph = (it >> 1) & 1, xphp = ((it - 1) >> 1) & 1;
+    T* const x1b = x1 + xs * XS;
+    T* const xeb = xe + xs * XS;
+    T* const x2b = x2 + xs * XS;
+    const T* const xep = xe + xsp * XS;       // E1 of plane k-1, written during the previous iteration
 
     // material index of the thread's V cells, as ONE packed word: plane k was requested an iteration ago, plane k + 1 is
     // requested now and stays packed until its use (unpacking at once makes the thread wait for the load right here:
@@ -325,10 +331,10 @@ __global__ void __launch_bounds__((R + 1) * 32, 1) k_step2(const __grid_constant
       stv(x1b + oH, hx); stv(x1b + R * TX + oH, hz);
     }
     __syncwarp();
-    if (lane == 0) mbar_arrive(&rdy1[s * R + r]);
+    if (lane == 0) mbar_arrive(&rdy1[xs * R + r]);
     if (ST || (it >= 2 && r >= 1)) {
       // ---------------- E1(k) = Ca E^n(k) + Cb curl H1 ----------------------------------------------------------------------
-      mbar_wait(&rdy1[s * R + r - 1], ph);
+      mbar_wait(&rdy1[xs * R + r - 1], xph);
 #pragma unroll
       for (int v = 0; v < V; ++v) mi[v] = (unsigned char)((mw >> (8 * v)) & 0xffu);
       T hxj[V], hzj[V];
@@ -361,15 +367,16 @@ __global__ void __launch_bounds__((R + 1) * 32, 1) k_step2(const __grid_constant
       stv(xeb + oH, nex); stv(xeb + R * TX + oH, nez);
     }
     __syncwarp();
-    if (lane == 0) mbar_arrive(&rdyE[s * R + r]);
+    if (lane == 0) mbar_arrive(&rdyE[xs * R + r]);
     T g2x[V], g2y[V], g2z[V];                    // H2 of plane k-1
     if (!ST) {
 #pragma unroll
       for (int v = 0; v < V; ++v) { g2x[v] = g2y[v] = g2z[v] = T(0); }
     }
+    if (!ST && r == 0 && it >= 3) mbar_wait(&rdyE[xsp * R + 1], xphp);
     if (ST || (it >= 3 && rowB)) {
       // ---------------- H2(k-1) = H1(k-1) - Db curl E1 ---------------------------------------------------------------------
-      mbar_wait(&rdyE[sprev * R + r + 1], phprev);
+      mbar_wait(&rdyE[xsp * R + r + 1], xphp);
       T exj[V], ezj[V];
       ldv(xep + oH + TX, exj); ldv(xep + R * TX + oH + TX, ezj);
       T ezi = __shfl_down_sync(0xffffffffu, e1z[0], 1), eyi = __shfl_down_sync(0xffffffffu, e1y[0], 1);
@@ -403,10 +410,10 @@ __global__ void __launch_bounds__((R + 1) * 32, 1) k_step2(const __grid_constant
       }
     }
     __syncwarp();
-    if (lane == 0) mbar_arrive(&rdy2[s * R + r]);
+    if (lane == 0) mbar_arrive(&rdy2[xs * R + r]);
     if (ST || (it >= 4 && rowE2)) {
       // ---------------- E2(k-1) = Ca E1(k-1) + Cb curl H2 -------------------------------------------------------------------
-      mbar_wait(&rdy2[s * R + r - 1], ph);
+      mbar_wait(&rdy2[xs * R + r - 1], xph);
       T hxj[V], hzj[V];
       ldv(x2b + oH - TX, hxj); ldv(x2b + R * TX + oH - TX, hzj);
       T hyi = __shfl_up_sync(0xffffffffu, g2y[V - 1], 1), hzi = __shfl_up_sync(0xffffffffu, g2z[V - 1], 1);

@@ -53,3 +53,14 @@ def test_two_port_protocol_matches_the_oracle_protocol():
     tau_o = np.array(orn.phase_delay(list(So[1, 0]), list(res["freqs"])))
     assert np.abs(res["tau"][1, 0] - tau_o).max() <= 1e-3 * np.abs(tau_o).max() + 1e-18
     assert np.isnan(res["tau"][0, 0]).all()
+
+
+def test_runs_dealt_to_several_devices_give_the_same_matrix():
+    """nport.extract(devices=[...]): the 2 N independent runs spread over worker threads, one per listed device (the same GPU
+    listed twice here, or two GPUs where the box has them) -- the S* matrix is the one the single-device path returns."""
+    import torch
+    devs = ["cuda:0", "cuda:1" if torch.cuda.device_count() > 1 else "cuda:0"]
+    a = nport.extract(_wl, W.drive_port, steps=300)
+    b = nport.extract(_wl, W.drive_port, steps=300, devices=devs)
+    # (not bit for bit: fdtd_commit may select another step implementation for a run, whose probe sums add in another order)
+    assert np.abs(a["S_star"] - b["S_star"]).max() <= 1e-6 and np.abs(a["Z_r"] - b["Z_r"]).max() <= 1e-6 * np.abs(a["Z_r"]).max()
