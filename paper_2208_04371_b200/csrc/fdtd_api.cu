@@ -6,6 +6,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <array>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -278,9 +279,7 @@ struct Solver : fdtd {
   int build_step2();
   void enqueue_pair(cudaEvent_t* ev = nullptr);
   void enqueue_steps(long count);
-  int shell_pass(bool isH, int d, const StepParams<T>& base, bool bump);
-  void region_pass(bool isH, const StepParams<T>& base, const int* r, bool bump);
-  void band_pass(bool isH, const StepParams<T>& base);
+  int shell_pass(bool isH, int d, const StepParams<T>& base, bool bump, bool with_bands);
   StepParams<T> sp_of(int set) const {
     StepParams<T> q = sp;
     for (int f = 0; f < 6; ++f) q.src[f] = q.dst[f] = field_origin(f, set);
@@ -1089,69 +1088,70 @@ int Solver<T>::build_step2() {
 }
 
 template <typename T, int MODE>
-static void region_launch(bool isH, const StepParams<T>& q, int nk, cudaStream_t st) {
-  const long long nvec = (long long)q.rnvx * q.rny;
-  const dim3 grid((unsigned)((nvec + 127) / 128), 1, (unsigned)nk), block(128, 1, 1);
-  if (isH) k_update_H<T, MODE, true><<<grid, block, 0, st>>>(q);
-  else k_update_E<T, MODE, false, true><<<grid, block, 0, st>>>(q);
+static void region_launch(bool isH, const StepParams<T>& q, unsigned blocks, cudaStream_t st) {
+  if (isH) k_update_H<T, MODE, true><<<blocks, 128, 0, st>>>(q);
+  else k_update_E<T, MODE, false, true><<<blocks, 128, 0, st>>>(q);
 }
 
 // One half step of the shell: every cell outside the box shrunk by d cells (in x: by the whole vectors that hold d cells) on
 // its open sides.  Half step d of the sequence 3, 2, 1, 0 needs the results of the one before on the cells up to d + 1 deep
 // only; what a whole vector computes beyond that is overwritten by the box kernel before anybody reads it.  The
 // complement of that inner box is cut into at most six disjoint boxes (two z slabs over the full planes, two y slabs between
-// them, two x slabs between those).  Returns the number of launches (the first one carries the step-counter bump if asked).
+// them, two x slabs between those); with_bands adds the bands around the port planes inside the box (first step only).  All
+// of it is ONE launch (region table in the kernel parameters): the small boxes run beside the large ones instead of after
+// them.  Returns the number of launches (the first one carries the step-counter bump if asked).
 template <typename T>
-int Solver<T>::shell_pass(bool isH, int d, const StepParams<T>& base, bool bump) {
+int Solver<T>::shell_pass(bool isH, int d, const StepParams<T>& base, bool bump, bool with_bands) {
   const int V = vlen(), dx_ = (d + V - 1) / V * V;   // x in whole vectors: the cells beyond d hold values nobody reads
   const int ix0 = box[0] > 0 ? box[0] + dx_ : 0, ix1 = box[1] < nx ? box[1] - dx_ : nx;
   const int iy0 = box[2] > 0 ? box[2] + d : 0, iy1 = box[3] < ny ? box[3] - d : ny;
   const int iz0 = box[4] > 0 ? box[4] + d : 0, iz1 = box[5] < nz ? box[5] - d : nz;
   const int reg[6][6] = {{0, nx, 0, ny, 0, iz0},     {0, nx, 0, ny, iz1, nz},   {0, nx, 0, iy0, iz0, iz1},
                          {0, nx, iy1, ny, iz0, iz1}, {0, ix0, iy0, iy1, iz0, iz1}, {ix1, nx, iy0, iy1, iz0, iz1}};
-  int launched = 0;
+  std::vector<std::array<int, 6>> list;
   for (int g = 0; g < 6; ++g) {
     const int* q6 = reg[g];
     if (q6[1] <= q6[0] || q6[3] <= q6[2] || q6[5] <= q6[4]) continue;
-    region_pass(isH, base, q6, bump && launched == 0);
+    list.push_back({q6[0], q6[1], q6[2], q6[3], q6[4], q6[5]});
+  }
+  if (with_bands) {
+    // H^{n+1/2} on the probe samples' bounding box grown by one cell on its low sides (the backward differences of the E update
+    // reach there), E^{n+1} on the bounding box itself; clipped to the cells the six boxes above leave out: what they cover is
+    // advanced already -- a second update would advance the psi of a CPML cell twice
+    const int grow = isH ? 1 : 0;
+    for (const Band& g : bands) {
+      const int i0 = (isH && g.i0 > 0) ? g.i0 - V : g.i0;   // cell ip - 1 may sit in the vector before: take it along
+      const std::array<int, 6> r = {std::max(i0, ix0), std::min(g.i1, ix1), std::max(g.j0 - grow, iy0), std::min(g.j1, iy1),
+                                    std::max(g.k0 - grow, iz0), std::min(g.k1, iz1)};
+      if (r[1] <= r[0] || r[3] <= r[2] || r[5] <= r[4]) continue;
+      list.push_back(r);
+    }
+  }
+  int launched = 0;
+  for (size_t first = 0; first < list.size(); first += StepParams<T>::kMaxRegions) {
+    StepParams<T> q = base;
+    unsigned blocks = 0;
+    q.nreg = 0;
+    for (size_t g = first; g < list.size() && q.nreg < StepParams<T>::kMaxRegions; ++g) {
+      const std::array<int, 6>& r = list[g];
+      typename StepParams<T>::Region& o = q.reg[q.nreg++];
+      o.i0 = r[0]; o.j0 = r[2]; o.k0 = r[4];
+      o.nvx = (r[1] - r[0] + V - 1) / V; o.ny = r[3] - r[2];
+      o.bpp = (int)(((long long)o.nvx * o.ny + 127) / 128);
+      o.blk0 = blocks;
+      blocks += (unsigned)o.bpp * (unsigned)(r[5] - r[4]);
+    }
+    q.bump = (bump && launched == 0) ? 1 : 0;
+    switch (mode()) {
+      case 0: region_launch<T, 0>(isH, q, blocks, stream); break;
+      case 1: region_launch<T, 1>(isH, q, blocks, stream); break;
+      case 2: region_launch<T, 2>(isH, q, blocks, stream); break;
+      default: region_launch<T, 3>(isH, q, blocks, stream); break;
+    }
+    ++launches;
     ++launched;
   }
   return launched;
-}
-
-// the one-step H or E kernel on the cells [r[0], r[1]) x [r[2], r[3]) x [r[4], r[5])  (r[0] a multiple of the vector length)
-template <typename T>
-void Solver<T>::region_pass(bool isH, const StepParams<T>& base, const int* r, bool bump) {
-  const int V = vlen();
-  StepParams<T> q = base;
-  q.ri0 = r[0]; q.rnvx = (r[1] - r[0] + V - 1) / V; q.rj0 = r[2]; q.rny = r[3] - r[2]; q.rk0 = r[4];
-  q.bump = bump ? 1 : 0;
-  switch (mode()) {
-    case 0: region_launch<T, 0>(isH, q, r[5] - r[4], stream); break;
-    case 1: region_launch<T, 1>(isH, q, r[5] - r[4], stream); break;
-    case 2: region_launch<T, 2>(isH, q, r[5] - r[4], stream); break;
-    default: region_launch<T, 3>(isH, q, r[5] - r[4], stream); break;
-  }
-  ++launches;
-}
-
-// The first step on the bands around the port planes inside the box: H^{n+1/2} on the probe samples' bounding box grown by one
-// cell on its low sides (the backward differences of the E update reach there), then E^{n+1} on the bounding box itself.
-// A band is clipped to the cells the shell pass of the same half step (d = 3 for H, 2 for E) leaves out: what that pass covers
-// it has already advanced -- a second update would advance the psi of a CPML cell twice.
-template <typename T>
-void Solver<T>::band_pass(bool isH, const StepParams<T>& base) {
-  const int V = vlen(), d = isH ? 3 : 2, grow = isH ? 1 : 0, dx_ = (d + V - 1) / V * V;
-  const int ix0 = box[0] > 0 ? box[0] + dx_ : 0, ix1 = box[1] < nx ? box[1] - dx_ : nx;
-  const int iy0 = box[2] > 0 ? box[2] + d : 0, iy1 = box[3] < ny ? box[3] - d : ny;
-  const int iz0 = box[4] > 0 ? box[4] + d : 0, iz1 = box[5] < nz ? box[5] - d : nz;
-  for (const Band& g : bands) {
-    const int i0 = (isH && g.i0 > 0) ? g.i0 - V : g.i0;   // cell ip - 1 may sit in the vector before: take it along
-    const int r[6] = {std::max(i0, ix0), std::min(g.i1, ix1), std::max(g.j0 - grow, iy0), std::min(g.j1, iy1),
-                      std::max(g.k0 - grow, iz0), std::min(g.k1, iz1)};
-    if (r[1] <= r[0] || r[3] <= r[2] || r[5] <= r[4]) continue;
-    region_pass(isH, base, r, false);
-  }
 }
 
 // Two steps: set a = cur holds time n everywhere; afterwards set b holds time n + 2 everywhere.
@@ -1169,17 +1169,15 @@ void Solver<T>::enqueue_pair(cudaEvent_t* ev) {
   if (ev) cudaEventRecord(ev[0], stream);
   StepParams<T> q = sp_of(a);
   for (int f = kHx; f <= kHz; ++f) q.dst[f] = field_origin(f, b);
-  if (shell_pass(true, 3, q, true) == 0) { k_bump<<<1, 1, 0, stream>>>(sp.nstep, 1); ++launches; }   // H1: reads a, writes H of b
-  band_pass(true, q);
+  if (shell_pass(true, 3, q, true, true) == 0) { k_bump<<<1, 1, 0, stream>>>(sp.nstep, 1); ++launches; }   // H1: reads a, writes H of b
   q = sp_of(a);
   for (int f = kHx; f <= kHz; ++f) q.src[f] = field_origin(f, b);
   for (int f = kEx; f <= kEz; ++f) q.dst[f] = field_origin(f, b);
-  shell_pass(false, 2, q, false);                                    // E1: H from b, E from a, writes E of b
-  band_pass(false, q);
+  shell_pass(false, 2, q, false, true);                              // E1: H from b, E from a, writes E of b
   cur = b; enqueue_ports(); cur = a;
   q = sp_of(b);
-  if (shell_pass(true, 1, q, true) == 0) { k_bump<<<1, 1, 0, stream>>>(sp.nstep, 1); ++launches; }   // H2, E2: in place in b
-  shell_pass(false, 0, q, false);
+  if (shell_pass(true, 1, q, true, false) == 0) { k_bump<<<1, 1, 0, stream>>>(sp.nstep, 1); ++launches; }   // H2, E2: in place in b
+  shell_pass(false, 0, q, false, false);
   if (ev) cudaEventRecord(ev[1], stream);
   switch (mode()) {
     case 0: step2_launch<T, 0>(s2par[a], stream); break;

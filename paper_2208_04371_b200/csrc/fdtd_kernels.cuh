@@ -176,15 +176,26 @@ __device__ __forceinline__ void update_H_vec(const StepParams<T>& p, int i0, int
   stv(p.dst[kHx] + o, hx); stv(p.dst[kHy] + o, hy); stv(p.dst[kHz] + o, hz);
 }
 
-// REGION: the launch covers a box of cells given in p.ri0 .. (rows of the box back to back along blockIdx.x, planes on blockIdx.z)
+// REGION launches (fdtd_params.h): the block's region, and the first cell, row and plane of this thread in it (false = none)
+template <typename T>
+__device__ __forceinline__ bool region_cell(const StepParams<T>& p, int& i0, int& j, int& k) {
+  int g = 0;
+  for (int q = 1; q < p.nreg; ++q) g = blockIdx.x >= p.reg[q].blk0 ? q : g;
+  const typename StepParams<T>::Region r = p.reg[g];
+  const unsigned b = blockIdx.x - r.blk0;
+  const int kk = (int)(b / (unsigned)r.bpp), v = (int)(b - (unsigned)kk * (unsigned)r.bpp) * (int)blockDim.x + (int)threadIdx.x, jr = v / r.nvx;
+  i0 = r.i0 + (v - jr * r.nvx) * VecOf<T>::V; j = r.j0 + jr; k = r.k0 + kk;
+  return jr < r.ny;
+}
+
+// REGION: the launch covers the boxes of cells listed in p.reg (one launch per half step of the shell)
 template <typename T, int MODE, bool REGION = false>
 __global__ void __launch_bounds__(128) k_update_H(const StepParams<T> p) {
   constexpr int V = VecOf<T>::V;
   if (REGION) {
-    const int v = blockIdx.x * blockDim.x + threadIdx.x, jr = v / p.rnvx;
-    if (p.bump && v == 0 && blockIdx.z == 0) *p.nstep += 1;
-    if (jr >= p.rny) return;
-    update_H_vec<T, MODE>(p, p.ri0 + (v - jr * p.rnvx) * V, p.rj0 + jr, p.rk0 + (int)blockIdx.z);
+    if (p.bump && blockIdx.x == 0 && threadIdx.x == 0) *p.nstep += 1;
+    int i0, j, k;
+    if (region_cell(p, i0, j, k)) update_H_vec<T, MODE>(p, i0, j, k);
     return;
   }
   // threads are numbered along the row vectors of a plane, rows back to back: no idle lanes when a row is not a
@@ -317,9 +328,8 @@ template <typename T, int MODE, bool PEER = false, bool REGION = false>
 __global__ void __launch_bounds__(128) k_update_E(const StepParams<T> p) {
   constexpr int V = VecOf<T>::V;
   if (REGION) {
-    const int v = blockIdx.x * blockDim.x + threadIdx.x, jr = v / p.rnvx;
-    if (jr >= p.rny) return;
-    update_E_vec<T, MODE, PEER>(p, p.ri0 + (v - jr * p.rnvx) * V, p.rj0 + jr, p.rk0 + (int)blockIdx.z);
+    int i0, j, k;
+    if (region_cell(p, i0, j, k)) update_E_vec<T, MODE, PEER>(p, i0, j, k);
     return;
   }
   const int nvec = (p.nx + V - 1) / V, v = blockIdx.x * blockDim.x + threadIdx.x;

@@ -50,9 +50,14 @@ struct StepParams {
   T* psi[12];       // slab-only arrays: y-slab  i + P*(s + Sy*k);  z-slab  i + P*(j + ny*s);  x-slab  sp + Sxp*(j + ny*k)
   long long* nstep; // device step counter, incremented by the first kernel of every step
   int z_lo_open;    // 1: this grid is a z slab of a larger one and plane 0 is not a wall (Ex, Ey there are ordinary cells)
-  // region launches of the two-pass kernels (the shell around a two-step box, fdtd_step2.cuh): cells
-  // [ri0, ri0 + rnvx * V) x [rj0, rj0 + rny) x [rk0, rk0 + gridDim.z); bump = this launch increments the step counter
-  int ri0, rj0, rk0, rnvx, rny, bump;
+  // region launches of the two-pass kernels (the shell around a two-step box, fdtd_step2.cuh): ONE launch covers up to
+  // kMaxRegions disjoint boxes of cells [i0, i0 + nvx * V) x [j0, j0 + ny) x [k0, k0 + nk); its 1-D grid numbers, region after
+  // region, the planes of a box and within a plane the blocks over its row vectors (rows back to back: bpp blocks per plane);
+  // blk0 = first block of the region.  bump = this launch increments the step counter.
+  struct Region { int i0, j0, k0, nvx, ny, bpp; unsigned blk0; };
+  static constexpr int kMaxRegions = 10;
+  int nreg, bump;
+  Region reg[kMaxRegions];
   T* peer_E[2];     // z slab linked to its lower neighbour (fdtd_z_link): that slab's halo plane nz of Ex, Ey (element (0,0)
                     // of the plane, same pitch), written by the kernel that updates E on plane 0; nullptr = not linked
 };
