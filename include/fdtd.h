@@ -55,7 +55,7 @@ enum { FDTD_EX = 0, FDTD_EY, FDTD_EZ, FDTD_HX, FDTD_HY, FDTD_HZ };
 /* Options for fdtd_set_option (before commit). */
 enum {
   FDTD_OPT_STEP_IMPL = 1,   /* 0 = auto: fdtd_commit measures the candidates on the committed all-zero state and keeps the
-                                   fastest (below 4 Mi cells: two-pass vs persistent; above: two-pass vs fused; from 64 Mi
+                                   fastest (below 4 Mi cells: two-pass vs persistent; above: two-pass vs fused; from 8 Mi
                                    cells also 4, where the grid leaves it a box),
                                1 = two-pass (H kernel, E kernel, in place),
                                2 = fused E+H kernel (temporal blocking over the half steps; a second field set),

@@ -170,7 +170,8 @@ struct Solver : fdtd {
   struct Band { int i0, i1, j0, j1, k0, k1; };   // cells around a port plane inside the box (build_step2)
   std::vector<Band> bands;
   bool persistent = false;   // small grids: many steps per cooperative launch (fdtd_persistent.cuh)
-  int persist_blocks = 0;
+  int persist_blocks = 0;    // blocks of the persistent kernel that update cells ...
+  int persist_probe = 0;     // ... and blocks that only take the port probes (0: blocks 0..ports-1 do both)
   int cur = 0;
   int kz = 0;
   int tile_shape = 0;        // fused step: 0 = FDTD_FUSED_TY-row tiles, one block per SM; 1 = 6-row tiles, two blocks per SM
@@ -486,7 +487,7 @@ int Solver<T>::commit(void* w, size_t bytes, void* st) {
   // two steps per pass: a candidate of the automatic choice on grids far beyond L2 (its shell passes and the priming planes
   // of its chunks need room to pay off: measured slower than the fused step on 16 Mi cells, faster on 900 Mi); asked for by
   // name, only its chunk length is measured
-  if ((two_step && opt_kz <= 0) || (opt_impl == 0 && fused && !z_slab() && (long long)nx * ny * nz >= (64LL << 20))) {
+  if ((two_step && opt_kz <= 0) || (opt_impl == 0 && fused && !z_slab() && (long long)nx * ny * nz >= (8LL << 20))) {
     const int r = autotune_two_step();
     if (r != FDTD_OK) return r;
   }
@@ -881,11 +882,11 @@ int Solver<T>::autotune_two_step() {
 
 // ---- persistent multi-step kernel for small grids ---------------------------------------------------------------------
 template <typename T, int MODE>
-static cudaError_t persistent_launch(const StepParams<T>& sp, const PortParams<T>& q, int n, int blocks, cudaStream_t st) {
+static cudaError_t persistent_launch(const StepParams<T>& sp, const PortParams<T>& q, int n, int blocks, int probe_blocks, cudaStream_t st) {
   StepParams<T> a = sp;
   PortParams<T> b = q;
-  void* args[3] = {&a, &b, &n};
-  return cudaLaunchCooperativeKernel(reinterpret_cast<void*>(k_steps_persistent<T, MODE>), dim3(blocks), dim3(kPersistThreads), args, 0, st);
+  void* args[4] = {&a, &b, &n, &probe_blocks};
+  return cudaLaunchCooperativeKernel(reinterpret_cast<void*>(k_steps_persistent<T, MODE>), dim3(blocks + probe_blocks), dim3(kPersistThreads), args, 0, st);
 }
 template <typename T, int MODE>
 static cudaError_t persistent_occupancy(int* per_sm) {
@@ -899,10 +900,10 @@ int Solver<T>::launch_persistent(const PortParams<T>& q, long n, long* done) {
   while (n > 0 && e == cudaSuccess) {
     const int m = (int)(n > 4096 ? 4096 : n);   // a launch stays well under a second even on the largest eligible grid
     switch (mode()) {
-      case 0: e = persistent_launch<T, 0>(sp, q, m, persist_blocks, stream); break;
-      case 1: e = persistent_launch<T, 1>(sp, q, m, persist_blocks, stream); break;
-      case 2: e = persistent_launch<T, 2>(sp, q, m, persist_blocks, stream); break;
-      default: e = persistent_launch<T, 3>(sp, q, m, persist_blocks, stream); break;
+      case 0: e = persistent_launch<T, 0>(sp, q, m, persist_blocks, persist_probe, stream); break;
+      case 1: e = persistent_launch<T, 1>(sp, q, m, persist_blocks, persist_probe, stream); break;
+      case 2: e = persistent_launch<T, 2>(sp, q, m, persist_blocks, persist_probe, stream); break;
+      default: e = persistent_launch<T, 3>(sp, q, m, persist_blocks, persist_probe, stream); break;
     }
     n -= m;
     if (e == cudaSuccess && done) *done += m;
@@ -942,6 +943,8 @@ int Solver<T>::setup_persistent() {
   long long want = (nvec + kPersistThreads - 1) / kPersistThreads;           // no more blocks than there is work
   const long long cap = (long long)sms * (per_sm > 4 ? 4 : per_sm);
   persist_blocks = (int)(want < cap ? (want < 1 ? 1 : want) : cap);
+  // one more resident block per port for the probes and their DFT terms, where the device has room for them
+  persist_probe = (!ports.empty() && persist_blocks + (long long)ports.size() <= cap) ? (int)ports.size() : 0;
   if (opt_impl == 3) { persistent = true; return FDTD_OK; }
   // measure: 16 steps either way
   const int reps = 16;

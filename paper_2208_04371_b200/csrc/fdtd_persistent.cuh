@@ -4,11 +4,14 @@
 // (about 4 us each inside a CUDA graph: 16 us for C0's 32^3 cells).  Here one resident grid of blocks walks the whole
 // grid with a grid-stride loop and separates the half steps with grid-wide barriers instead of kernel boundaries:
 //
-//   step n:  [H phase: H^{n+1/2} from E^n            | blocks 0..ports-1 first probe V of step n-1 (E is read-only here)]
+//   step n:  [H phase: H^{n+1/2} from E^n            | probe blocks: V of step n-1 (E is read-only here)]
 //            grid barrier
-//            [E phase: E^{n+1} from H^{n+1/2}, source | blocks 0..ports-1 first probe I of step n   (H is read-only here)]
+//            [E phase: E^{n+1} from H^{n+1/2}, source | probe blocks: I of step n   (H is read-only here)]
 //            grid barrier
 //   after the last step: V probe of that step.
+// The probes of port p are taken by a block of their own (the last `probe_blocks` blocks of the grid do nothing else) where
+// the resident grid has room for it: a block that sums a port, evaluates its 2 x nf sines in fp64 AND updates its share of
+// the cells would be the last one at every barrier.  Without room (probe_blocks = 0) blocks 0..ports-1 do both.
 //
 // The arithmetic is the two-pass step's (update_H_vec / update_E_vec of fdtd_kernels.cuh), the source is added by the
 // thread that owns the cell right after its E update (ports in order, like the per-port k_source launches), and the probe
@@ -91,7 +94,8 @@ __device__ __forceinline__ void probe_I_dft(const PortParams<T>& p, int port, lo
 struct SrcBox { int is, sj0, sj1, sk0, sk1, port; };
 
 template <typename T, int MODE>
-__global__ void __launch_bounds__(kPersistThreads) k_steps_persistent(const StepParams<T> p, const PortParams<T> q, int nsteps) {
+__global__ void __launch_bounds__(kPersistThreads) k_steps_persistent(const StepParams<T> p, const PortParams<T> q, int nsteps,
+                                                                      int probe_blocks) {
   namespace cg = cooperative_groups;
   cg::grid_group grid = cg::this_grid();
   constexpr int V = VecOf<T>::V;
@@ -112,7 +116,11 @@ __global__ void __launch_bounds__(kPersistThreads) k_steps_persistent(const Step
   const int nsrc = nsrc_s;
   const int nvx = (p.nx + V - 1) / V;
   const int nvec = nvx * p.ny * p.nz;                       // the host uses this kernel below 2^31 vectors only
-  const int tid0 = blockIdx.x * kPersistThreads + threadIdx.x, nthr = gridDim.x * kPersistThreads;
+  const int nfb = (int)gridDim.x - probe_blocks;            // blocks that update cells
+  const bool field_block = (int)blockIdx.x < nfb;
+  // ports this block probes: block b of the probe blocks takes ports b, b + probe_blocks, ...; shared duty: b, b + gridDim.x, ...
+  const int port0 = probe_blocks > 0 ? (int)blockIdx.x - nfb : (int)blockIdx.x, port_step = probe_blocks > 0 ? probe_blocks : (int)gridDim.x;
+  const int tid0 = field_block ? blockIdx.x * kPersistThreads + threadIdx.x : 0x7fffffff, nthr = nfb * kPersistThreads;
   const long long n0 = *p.nstep;                            // written again only after the last grid barrier
 
   for (int s = 0; s < nsteps; ++s) {
@@ -122,15 +130,16 @@ __global__ void __launch_bounds__(kPersistThreads) k_steps_persistent(const Step
       const PortDev d = q.ports[sbox[threadIdx.x].port];
       sg[threadIdx.x] = (T)(d.amp * waveform_dev(d.waveform, (double)n * q.dt, d.t0, d.sigma, d.f0));
     }
-    if (s > 0)
-      for (int port = blockIdx.x; port < q.nports; port += gridDim.x) probe_V_dft(q, port, n - 1, sh);
+    if (s > 0 && port0 >= 0)
+      for (int port = port0; port < q.nports; port += port_step) probe_V_dft(q, port, n - 1, sh);
     for (int v = tid0; v < nvec; v += nthr) {
       const int iv = v % nvx, jk = v / nvx;
       update_H_vec<T, MODE>(p, iv * V, jk % p.ny, jk / p.ny);
     }
     grid.sync();
     // ---- E phase, source ----------------------------------------------------------------------------------------------
-    for (int port = blockIdx.x; port < q.nports; port += gridDim.x) probe_I_dft(q, port, n, sh);
+    if (port0 >= 0)
+      for (int port = port0; port < q.nports; port += port_step) probe_I_dft(q, port, n, sh);
     for (int v = tid0; v < nvec; v += nthr) {
       const int iv = v % nvx, jk = v / nvx;
       const int i0 = iv * V, j = jk % p.ny, k = jk / p.ny;
@@ -143,7 +152,8 @@ __global__ void __launch_bounds__(kPersistThreads) k_steps_persistent(const Step
     }
     grid.sync();
   }
-  for (int port = blockIdx.x; port < q.nports; port += gridDim.x) probe_V_dft(q, port, n0 + nsteps, sh);
+  if (port0 >= 0)
+    for (int port = port0; port < q.nports; port += port_step) probe_V_dft(q, port, n0 + nsteps, sh);
   if (blockIdx.x == 0 && threadIdx.x == 0) *p.nstep = n0 + nsteps;
 }
 
