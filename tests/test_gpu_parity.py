@@ -473,3 +473,25 @@ def test_two_step_refuses_grids_without_a_box():
     with pytest.raises(FdtdError) as e:
         Solver.from_workload(dict(w, ports=[], freqs=np.zeros(0)), options={FDTD_OPT_STEP_IMPL: 4}, z_open=(False, True))
     assert e.value.code == -1
+
+
+def test_five_driving_ports_two_step_by_name_is_refused_and_the_automatic_choice_steps_on():
+    """The two-step kernel carries at most four driving ports in its parameters.  Asked for by name with five it is an error;
+    under the automatic choice (a grid of 8 Mi cells, where two steps per pass is a candidate) the handle simply keeps one of
+    the other implementations and matches the oracle."""
+    w = W.random_box(61, nx=256, ny=256, nz=128, pml=(4, 4, 4, 4, 4, 4), steps=6, precision=FDTD_F32)
+    src = dict(w["ports"][0])
+    ports = [dict(src) for _ in range(5)]
+    for n, q in enumerate(ports):
+        q["is"] = src["is"] + 9 * n
+        q["ip"] = src["ip"] + 9 * n
+        q["amp"] = 1.0 - 0.1 * n
+    w = dict(w, ports=ports)
+    with pytest.raises(FdtdError) as e:
+        Solver.from_workload(w, options={FDTD_OPT_STEP_IMPL: 4})
+    assert e.value.code == -1
+    o, s, rep = run_pair(w, 6, checkpoints=[2, 6])
+    assert s.impl_name in ("fused", "two_pass")
+    assert_fields(rep, FDTD_F32)
+    assert max(rep["dft_err"]) <= 1e-4
+    s.destroy()
