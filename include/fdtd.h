@@ -240,6 +240,39 @@ int fdtd_two_step_box(const fdtd_t*, int box[6]);
 const char* fdtd_last_error(const fdtd_t*);
 void fdtd_destroy(fdtd_t*);
 
+/* ---- port probes for callers that cannot allocate device memory ------------------------------------------------------------
+ * V and I of Eq. 4 (reading R7; the formulas stand above fdtd_port) of `nports` ports, from field arrays the
+ * caller already holds, without a handle and without a workspace.  Meant for code that has no way to obtain device memory when
+ * it wants a probe: a monitor looking at a run in flight (an allocation would synchronise the GPU under the time stepping), a
+ * plug-in whose host program took the whole GPU for its own pool at start-up (an allocation fails there), a hook that runs
+ * where allocator calls are forbidden.  The reduction is spread over several thread blocks per port and needs a little memory
+ * for the hand-over between them; this entry point keeps it in a fixed array inside the library image
+ * (FDTD_NOALLOC_SCRATCH_BYTES per GPU, resident on every GPU that loads the library until the process exits) and calls no
+ * allocation routine of any kind.
+ *   Ez, Hy, Hz   DEVICE arrays of nx*ny*nz elements of `precision` (FDTD_F32 | FDTD_F64), index i + nx*(j + ny*k), all on one
+ *                GPU; read only.  E.g. what fdtd_read_fields wrote, or another solver's fields.
+ *   ports        HOST array; only ip, v* and l* are read (the source part is ignored).  Same range rules as fdtd_add_port.
+ *   VI           DEVICE array of 2*nports doubles on the same GPU: VI[2p] = V, VI[2p+1] = I of port p.  Written by the kernel;
+ *                valid once the stream has reached that point.  The reduction is carried out in fp64 whatever the precision.
+ *   cuda_stream  a cudaStream_t of that GPU as void* (NULL = the legacy default stream).  One memset and one kernel are
+ *                enqueued; nothing is synchronised.
+ *   errbuf       optional HOST buffer for a message on failure (there is no handle to ask); may be NULL.
+ * Limits and sharing -- all of them consequences of the one built-in array:
+ *   - at most FDTD_NOALLOC_MAX_PORTS ports per call; a longer list returns FDTD_ERANGE and enqueues nothing (split it);
+ *   - every call on a GPU uses the same array, which still holds the previous call's contents; the call clears the arrival
+ *     counters (the only part that must start at zero) on the stream before its kernel;
+ *   - calls whose kernels may run at the same time on one GPU (two streams, two threads) race on that array and give wrong
+ *     answers; calls on one stream are ordered and fine, and different GPUs have different copies;
+ *   - the first call on each GPU looks up where that GPU's copy of the array lives (cudaGetSymbolAddress, with that GPU made
+ *     current) and caches the address: make this first call before any stream capture begins.
+ * Returns FDTD_OK, FDTD_EINVAL (bad precision / sizes / null or non-device pointers / arrays on different GPUs), FDTD_ERANGE
+ * (too many ports, a port outside the grid, ny*nz above 2^31-1) or FDTD_ECUDA.  The caller's current device is restored. */
+enum { FDTD_NOALLOC_MAX_PORTS = 16, FDTD_NOALLOC_MAX_BLOCKS = 64,
+       FDTD_NOALLOC_SCRATCH_BYTES = 2 * 8 * FDTD_NOALLOC_MAX_BLOCKS * FDTD_NOALLOC_MAX_PORTS + 256 };
+int fdtd_port_probe_noalloc(const void* Ez, const void* Hy, const void* Hz, int precision, int nx, int ny, int nz,
+                            double dy, double dz, const fdtd_port* ports, int nports, double* VI, void* cuda_stream,
+                            char* errbuf, size_t errbuf_len);
+
 #ifdef __cplusplus
 }
 #endif

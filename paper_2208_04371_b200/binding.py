@@ -76,7 +76,10 @@ SYMBOLS = {
     "fdtd_z_link": (C.c_int, [_vp, C.c_int, C.POINTER(C.c_void_p), C.c_void_p]),
     "fdtd_last_error": (C.c_char_p, [_vp]),
     "fdtd_destroy": (None, [_vp]),
+    "fdtd_port_probe_noalloc": (C.c_int, [_vp, _vp, _vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double,
+                                          C.POINTER(fdtd_port), C.c_int, _vp, _vp, C.c_char_p, C.c_size_t]),
 }
+FDTD_NOALLOC_MAX_PORTS = 16
 
 _lib = None
 
@@ -319,3 +322,27 @@ def fdtd_last_error(h) -> str:
 
 def fdtd_destroy(h):
     lib().fdtd_destroy(h)
+
+
+def fdtd_port_probe_noalloc(Ez, Hy, Hz, precision, nx, ny, nz, dy, dz, ports, VI, cuda_stream):
+    """V and I (Eq. 4) of `ports` from three CUDA field tensors of nx*ny*nz elements, written into the CUDA float64 tensor
+    VI (2 per port: V, I) on the given stream.  This is the entry point for callers that cannot allocate device memory (a
+    monitor beside a running solver, a plug-in in a host that owns all GPU memory, a no-allocation region): the hand-over
+    memory of the reduction is a fixed array inside the library, shared by every call on a GPU -- so at most
+    FDTD_NOALLOC_MAX_PORTS ports per call, and calls that overlap on one GPU race.  Nothing is allocated here either: the
+    tensors are the caller's, the port list is marshalled into host memory."""
+    n_cells = int(nx) * int(ny) * int(nz)
+    for name, t in (("Ez", Ez), ("Hy", Hy), ("Hz", Hz)):
+        _check_cell_array(t, n_cells, 8 if precision == FDTD_F64 else 4, f"fdtd_port_probe_noalloc {name}")
+    _check_cell_array(VI, 2 * len(ports), 8, "fdtd_port_probe_noalloc VI")
+    arr = (fdtd_port * max(len(ports), 1))()
+    for q, port in zip(arr, ports):
+        for name, _ in fdtd_port._fields_:
+            key = "is" if name == "is_" else name
+            if key in port:
+                setattr(q, name, port[key])
+    err = C.create_string_buffer(256)
+    code = lib().fdtd_port_probe_noalloc(_ptr(Ez), _ptr(Hy), _ptr(Hz), int(precision), int(nx), int(ny), int(nz), float(dy),
+                                         float(dz), arr, len(ports), _ptr(VI), int(cuda_stream), err, len(err))
+    if code != FDTD_OK:
+        raise FdtdError(code, err.value.decode())
