@@ -72,7 +72,8 @@ enum {
                                plain launches (fdtd_graph_replays() stays 0)                                             */
   FDTD_OPT_GRAPH_UNROLL = 3,/* steps per captured graph (default 8; rounded up to even for the fused step)              */
   FDTD_OPT_FUSED_KZ = 4,    /* planes per z chunk of the fused kernel (0 = auto: measured at commit)                    */
-  FDTD_OPT_Z_SPIN = 5,      /* linked z slabs: polls of a hand-over counter before a wait gives up (default 2e7, ~2 s)  */
+  FDTD_OPT_Z_SPIN = 5,      /* linked z slabs: polls of a hand-over counter before a wait gives up (default 2e7; a poll sleeps
+                               about 1 us, so about 20 s).  After the first time-out the slab's later waits return at once    */
   FDTD_OPT_FUSED_TILE = 6   /* tile of the fused kernel: 0 = auto (measured at commit), 1 = 128 x 14 cells (fp64: 64 x 14), one
                                block per SM; 2 = 128 x 6 (64 x 6), two blocks per SM: twice the tiles and two z marches per
                                SM for mid-size grids.  The results are the same cell by cell whatever the tile            */
@@ -212,6 +213,10 @@ int fdtd_plane(fdtd_t*, int comp, int k, void** dev_ptr, size_t* bytes);
  * fdtd_step_end stay available and do the same per half step: slabs that share ONE stream must be advanced that way
  * (all begins, then all ends, in ascending slab order), so that no wait ever precedes its post in stream order; slabs on
  * their own GPUs run fdtd_step(n) concurrently.  A wait that gives up makes the next synchronising read return FDTD_ECUDA.
+ * fdtd_reset of a linked slab clears its own halo planes and counters on its own stream only, while the neighbours' kernels
+ * store into them: the CALLER must let every linked slab finish (synchronise all their streams, and a barrier between
+ * processes) before the first fdtd_reset, and let every reset finish the same way before the next step -- otherwise a late
+ * post survives the clear and satisfies the waits of the next run.
  * Errors: FDTD_ESTATE before commit / for a face that is not an interface; FDTD_ECUDA without a peer path. */
 int fdtd_z_halo(fdtd_t*, int side, void* planes[4], void** flag);
 int fdtd_z_link(fdtd_t*, int side, void* const peer_planes[4], void* peer_flag);

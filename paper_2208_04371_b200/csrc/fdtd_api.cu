@@ -57,7 +57,7 @@ struct fdtd {
   long opt_impl = 0, opt_graph = 1, opt_unroll = 8, opt_kz = 0, opt_tile = 0;
   int z_lo_open = 0, z_hi_open = 0;   // this grid is a z slab of a larger one (fdtd_set_z_interfaces)
   bool z_linked[2] = {false, false};  // fdtd_z_link: the kernels push my boundary planes into the neighbour on that side
-  long opt_zspin = 20000000;          // polls of a hand-over flag before the wait kernel gives up (about 2 s)
+  long opt_zspin = 20000000;          // polls of a hand-over flag before the wait kernel gives up (>= 1 us each: about 20 s)
   bool mid_step = false;              // between fdtd_step_begin and fdtd_step_end
   bool committed = false;
   long nstep = 0;
@@ -842,7 +842,7 @@ int Solver<T>::autotune_two_step() {
   no_ports.swap(ports);
   const int nsrc = s2par[0].nsrc;
   s2par[0].nsrc = s2par[1].nsrc = 0;
-  cudaEvent_t a, b;
+  cudaEvent_t a = nullptr, b = nullptr;
   bool ok = cudaEventCreate(&a) == cudaSuccess && cudaEventCreate(&b) == cudaSuccess;
   double best = -1.0;
   int best_kz = kz;
@@ -861,7 +861,8 @@ int Solver<T>::autotune_two_step() {
     const double per_step = (double)ms / (2.0 * reps);
     if (ok && (best < 0 || per_step < best)) { best = per_step; best_kz = kz; }
   }
-  if (ok) { cudaEventDestroy(a); cudaEventDestroy(b); }
+  if (a) cudaEventDestroy(a);
+  if (b) cudaEventDestroy(b);
   ports.swap(no_ports);
   s2par[0].nsrc = s2par[1].nsrc = nsrc;
   cur = 0;

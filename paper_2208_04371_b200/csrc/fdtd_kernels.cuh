@@ -346,7 +346,9 @@ __global__ void __launch_bounds__(128) k_update_E(const StepParams<T> p) {
 //   k_z_post  (stream-ordered after the producing kernel)  fence; *peer_flag = step      release at system scope
 //   k_z_wait  (stream-ordered before the consuming kernel) spin until *flag >= step      acquire at system scope
 // `step` is read from the device step counter (+ add), so the same captured graph serves every replay.  The spin is
-// bounded: after max_spins polls it records a time-out in *err and returns (no launch can hang the device).
+// bounded: after max_spins polls it records a time-out in *err and returns (no launch can hang the device); once *err is set
+// every later wait of the slab returns at once (the run is lost anyway; the next synchronising read reports it) instead of
+// spinning the full time-out again per step.
 // ------------------------------------------------------------------------------------------------------------------
 __global__ void k_z_post(unsigned long long* peer_flag, const long long* nstep, long long add) {
   const unsigned long long v = (unsigned long long)(*nstep + add);
@@ -355,6 +357,7 @@ __global__ void k_z_post(unsigned long long* peer_flag, const long long* nstep, 
 }
 __global__ void k_z_wait(const unsigned long long* flag, const long long* nstep, long long add, int* err, long long max_spins) {
   const unsigned long long want = (unsigned long long)(*nstep + add);
+  if (*reinterpret_cast<volatile int*>(err)) return;
   for (long long it = 0;; ++it) {
     unsigned long long v;
     asm volatile("ld.acquire.sys.global.u64 %0, [%1];" : "=l"(v) : "l"(flag) : "memory");

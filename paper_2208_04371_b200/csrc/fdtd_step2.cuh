@@ -205,6 +205,9 @@ __global__ void __launch_bounds__((R + 1) * 32, 1) k_step2(const __grid_constant
   auto e_update = [&](T (&ex)[V], T (&ey)[V], T (&ez)[V], const T (&ax)[V], const T (&ay)[V], const T (&az)[V],
                       const unsigned char (&m)[V], long long o, int k) {
     if (kFull) {
+      // rows / columns / planes outside the grid (the halo of the computed region) have no coefficient cells: nothing is loaded
+      // there and the mask below zeroes the result (same test as load_db)
+      if (jin && k >= 0 && k < p.nz && i0 >= 0 && i0 < p.nx) {
       T ca[V], cb[V];
       ldv(p.Ca[0] + o, ca); ldv(p.Cb[0] + o, cb);
 #pragma unroll
@@ -215,6 +218,7 @@ __global__ void __launch_bounds__((R + 1) * 32, 1) k_step2(const __grid_constant
       ldv(p.Ca[2] + o, ca); ldv(p.Cb[2] + o, cb);
 #pragma unroll
       for (int v = 0; v < V; ++v) ez[v] = fma(cb[v], az[v], ca[v] * ez[v]);
+      }
     } else {
 #pragma unroll
       for (int v = 0; v < V; ++v) {   // (one look-up for vectors under a single material measured slower: 5.21 against 4.80 ms)

@@ -154,8 +154,13 @@ class ShardedSolver:
         return sent
 
     def reset(self):
+        """Zero every slab.  Linked slabs write into each other (halo planes, arrival counters), and one slab may be a step
+        ahead of its neighbour: all of them must have drained before the first one clears its counters, and all clears must
+        have landed before anyone steps again (include/fdtd.h, fdtd_z_link)."""
+        self.synchronize()
         for s in self.solvers:
             s.reset()
+        self.synchronize()
 
     @property
     def launch_count(self):
@@ -285,7 +290,15 @@ class DistributedSlab:
         return idx.numel()
 
     def reset(self):
+        """Quiesce, clear, quiesce: a neighbour's last kernels store into my halo planes and post my counters, so every rank
+        drains its stream before anyone clears, and every clear has landed on the device before anyone steps again."""
+        sync = getattr(self.solver, "synchronize", None)   # the CPU test hook's solver has no stream
+        if sync:
+            sync()
+        self.dist.barrier()                          # everybody's kernels (and their stores into my halo) are done
         self.solver.reset()
+        if sync:
+            sync()
         self.dist.barrier()                          # nobody posts into a neighbour that has not yet zeroed its counters
 
     @property

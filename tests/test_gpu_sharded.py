@@ -171,3 +171,53 @@ def test_slab_handles_refuse_plain_stepping_and_misordered_calls():
     p0, p1 = s.plane(0, -1), s.plane(0, w["nz"])
     assert p0.numel() == p1.numel() > 0
     s.destroy()
+
+
+def test_linked_slabs_reset_and_run_again_like_a_fresh_run():
+    """fdtd_reset of linked slabs (ShardedSolver.reset drains every slab before the first clear and after the last one: a late
+    post into a neighbour's counter would satisfy the waits of the next run).  Step, reset, step again: fields and port DFTs
+    must be those of a run that never saw the first one, bit for bit."""
+    w = W.throughput_c3(div=8, steps=60, npml=6, nf=8)
+    sh = ShardedSolver(w, ["cuda:0"] * 3)
+    sh.step(37)                                      # an odd count: the ping-pong field sets end up swapped
+    sh.reset()
+    sh.step(60)
+    fresh = ShardedSolver(w, ["cuda:0"] * 3)
+    fresh.step(60)
+    for c in range(6):
+        a, b = sh.read_fields(c), fresh.read_fields(c)
+        assert float(b.abs().max()) > 0
+        assert bool((a == b).all()), c
+    for p in range(len(w["ports"])):
+        for x, y in zip(sh.read_port_dft(p), fresh.read_port_dft(p)):
+            assert np.array_equal(x, y)
+    sh.destroy(); fresh.destroy()
+
+
+def test_a_wait_that_times_out_is_reported_and_later_waits_return_at_once():
+    """A hi-open slab linked to a neighbour that never posts (a scratch buffer stands in for its halo planes and counter), with
+    FDTD_OPT_Z_SPIN = 1: the first step's wait is satisfied by the zeroed counter, the second one gives up after one poll and
+    sets the slab's time-out flag, every later wait sees the flag and returns without polling; the next synchronising read
+    returns FDTD_ECUDA and fdtd_reset clears the condition."""
+    import time
+    import torch
+    from paper_2208_04371_b200 import FdtdError
+    from paper_2208_04371_b200 import binding as B
+    w = W.random_box(5, nx=40, ny=20, nz=24, pml=(3, 3, 3, 3, 0, 0), steps=4, precision=FDTD_F32)
+    w = dict(w, ports=[], freqs=np.zeros(0))
+    s = Solver.from_workload(w, options={FDTD_OPT_STEP_IMPL: 2, B.FDTD_OPT_Z_SPIN: 1}, z_open=(False, True))
+    _, nbytes = B.fdtd_plane(s.h, 0, 0)
+    dummy = torch.zeros(4 * nbytes + 256, dtype=torch.uint8, device=s.device)    # four planes and a counter nobody posts
+    torch.cuda.synchronize()
+    base = dummy.data_ptr()
+    B.fdtd_z_link(s.h, 1, [base + q * nbytes for q in range(4)], base + 4 * nbytes)
+    t0 = time.time()
+    s.step(200)
+    with pytest.raises(FdtdError) as e:
+        s.read_fields(0)
+    assert e.value.code == B.FDTD_ECUDA and "timed out" in str(e.value)
+    assert time.time() - t0 < 5.0
+    s.reset()
+    s.step(1)                                        # step 1 waits for "0 steps delivered": satisfied
+    s.read_fields(0)
+    s.destroy()
