@@ -17,8 +17,9 @@ from paper_2208_04371_b200 import FDTD_OPT_STEP_IMPL, Solver
 
 pytestmark = pytest.mark.gpu
 
-NSTEP = 6
+NSTEP = 24                 # 12 passes of the two-steps-per-pass kernel
 MARGIN = NSTEP + 1
+EDGE = 2 * MARGIN + 16     # crop edge: a compared interior of 16 cells where both faces of an axis are artificial
 
 
 def _crop_workload(w, lo, hi, keep_ports=()):
@@ -46,18 +47,77 @@ def _crop_workload(w, lo, hi, keep_ports=()):
                 freqs=w["freqs"] if ports else np.zeros(0))
 
 
-def _crops(w):
-    nx, ny, nz = w["nx"], w["ny"], w["nz"]
-    e = 40  # crop edge; compared interior = e - 2*MARGIN where both faces are artificial
+def _seams(s, w):
+    """Per axis (x, y, z): (origin, period) of the tile / chunk seams of the step implementation in use, and the faces of the
+    two-step box (None for the other implementations).  Two steps per pass: owned tiles of 120 x 8 cells (fp32: 30 of 32 lanes
+    x 4 cells, rows 2..R-2 of R = 11) counted from the box origin, chunks of fdtd_fused_kz() planes from the box's first plane.
+    Fused step: tiles of 128 x 14 (tile 1) or 128 x 6 (tile 2) cells and chunks of fdtd_fused_kz() planes, from cell 0.  The
+    two-pass kernels have no seams (None)."""
+    if s.impl_name == "two_step":
+        b = s.two_step_box
+        return [(b[0], 120), (b[2], 8), (b[4], s.fused_kz)], b
+    if s.impl_name == "fused":
+        return [(0, 128), (0, 14 if s.fused_tile == 1 else 6), (0, s.fused_kz)], None
+    return [None, None, None], None
+
+
+def _place(center, n, plo, phi):
+    """Start of a crop of EDGE cells around `center` on an axis of n cells.  A crop never cuts a CPML slab: one that would reach
+    into a slab is moved flush to that real face instead (it then contains the whole slab and the wall)."""
+    lo = center - EDGE // 2
+    if lo < plo:
+        return 0
+    if lo + EDGE > n - phi:
+        return n - EDGE
+    return int(lo)
+
+
+def _crops(w, s):
+    """Crops whose COMPARED interior (MARGIN cells off every artificial face) holds, for the implementation in use: an x-tile, a
+    y-tile and a z-chunk seam at once (two places), each face of the two-step box on each axis (the two corners hold the three
+    low / three high faces together with the CPML slabs and walls; three more crops put one high or low face mid-face next to
+    seams of the other two axes), the band of one-step cells around a port plane, plus three random interior crops."""
+    n = (w["nx"], w["ny"], w["nz"])
+    pml = w["pml"]
+    seams, box = _seams(s, w)
     r = W.rng_for(990)
-    out = [((0, 0, 0), (e, e, e)),                                     # corner: three low CPML slabs + walls
-           ((nx - e, ny - e, nz - e), (nx, ny, nz)),                   # opposite corner: three high slabs
-           ((108, 0, 300), (148, e, 340)),                             # x-tile boundary at i = 128, y-low slab
-           ((nx - e, 360, 0), (nx, 400, e)),                           # x-high and z-low slabs, y-tile boundaries
-           ((620, 376, 108), (660, 416, 148))]                         # interior: z-chunk boundary at k = 128
-    for _ in range(3):                                                 # random interior crops
-        o = [int(r.integers(16, n - 16 - e)) for n in (nx, ny, nz)]
-        out.append((tuple(o), tuple(v + e for v in o)))
+
+    def seam_near(a, frac):
+        """a seam of axis a close to frac * n (falls back to that position where the implementation has no seams)"""
+        c = int(frac * n[a])
+        if seams[a] is None:
+            return c
+        o, per = seams[a]
+        return o + per * max(1, round((c - o) / per))
+
+    def around(cx, cy, cz):
+        lo = tuple(_place(c, n[a], pml[2 * a], pml[2 * a + 1]) for a, c in enumerate((cx, cy, cz)))
+        return lo, tuple(v + EDGE for v in lo)
+
+    out = [((0, 0, 0), (EDGE,) * 3),                                          # corner: three low CPML slabs + walls (+ box faces)
+           (tuple(v - EDGE for v in n), n),                                   # opposite corner: three high slabs
+           around(seam_near(0, 0.09), seam_near(1, 0.5), seam_near(2, 0.15)),   # x, y and z seams in one interior (first seams)
+           around(seam_near(0, 0.6), seam_near(1, 0.3), seam_near(2, 0.7))]     # ... and deep inside the grid
+    seam_checks = [2, 3]
+    if box is not None:                                                       # one box face mid-face, seams on the other axes
+        out += [around(box[1], seam_near(1, 0.4), seam_near(2, 0.5)),
+                around(seam_near(0, 0.4), box[2], seam_near(2, 0.3)),
+                around(seam_near(0, 0.7), seam_near(1, 0.6), box[5])]
+    else:
+        out += [((n[0] - EDGE, 360, 0), (n[0], 360 + EDGE, EDGE))]            # x-high and z-low slabs
+    p0 = w["ports"][0]                                                        # the port plane and its band of one-step cells
+    out.append(around(p0["ip"], (p0["vj0"] + p0["vj1"]) // 2, (p0["vk0"] + p0["vk1"]) // 2))
+    for _ in range(3):                                                        # random interior crops
+        o = [int(r.integers(16, m - 16 - EDGE)) for m in n]
+        out.append((tuple(o), tuple(v + EDGE for v in o)))
+    # the promised seams really lie inside the compared interior
+    for q in seam_checks:
+        lo, hi = out[q]
+        for a in range(3):
+            if seams[a] is not None:
+                o, per = seams[a]
+                inner = range(lo[a] + (MARGIN if lo[a] > 0 else 0) + 1, hi[a] - (MARGIN if hi[a] < n[a] else 0))
+                assert any((c - o) % per == 0 for c in inner), (q, a, lo, hi, seams[a])
     return out
 
 
@@ -83,13 +143,13 @@ def test_C3_full_size_sampled_subboxes(impl, shape):
         if c == 2: a[:, :, 0] = 0; a[:, 0, :] = 0
         s.write_fields(c, a)
         init.append(a)
-    crops = _crops(w)
+    crops = _crops(w, s)
     init_crops = [[init[c][k0:k1, j0:j1, i0:i1].cpu().numpy().astype(np.float64) for c in range(6)]
                   for (i0, j0, k0), (i1, j1, k1) in crops]
     del init, a
     torch.cuda.empty_cache()
     s.step(NSTEP)
-    worst = 0.0
+    refs = []
     for (lo, hi), ic in zip(crops, init_crops):
         wc = _crop_workload(w, lo, hi)
         o = YeeOracle.from_workload(wc, track_max=True)
@@ -103,10 +163,16 @@ def test_C3_full_size_sampled_subboxes(impl, shape):
         # interior of the crop: MARGIN cells away from every artificial face
         sl = tuple(slice(MARGIN if l > 0 else 0, (h - l) - (MARGIN if h < n else 0))
                    for l, h, n in ((k0, k1, nz), (j0, j1, ny), (i0, i1, nx)))
-        for c in range(6):
-            gpu = s.read_fields(c)[k0:k1, j0:j1, i0:i1].cpu().numpy().astype(np.float64)
-            d = np.abs(gpu[sl] - o.read_field(c)[sl]).max() / (emax if c < 3 else hmax)
-            worst = max(worst, d)
+        refs.append(([o.read_field(c)[sl] for c in range(6)], sl, emax, hmax))
+    worst = 0.0
+    for c in range(6):
+        full = s.read_fields(c)
+        for ((i0, j0, k0), (i1, j1, k1)), (ref, sl, emax, hmax) in zip(crops, refs):
+            gpu = full[k0:k1, j0:j1, i0:i1].cpu().numpy().astype(np.float64)
+            worst = max(worst, np.abs(gpu[sl] - ref[c]).max() / (emax if c < 3 else hmax))
+        del full
+    print(f"C3 full size impl={s.impl_name} kz={s.fused_kz} box={s.two_step_box if s.impl_name == 'two_step' else None}: "
+          f"{len(crops)} crops of {EDGE}^3, {NSTEP} steps, worst field err {worst:.3e}")
     assert worst <= 1e-4, worst
     s.destroy()
 

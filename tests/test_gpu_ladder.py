@@ -62,27 +62,34 @@ def test_C1_full_length_sparams():
     y_i = max(np.abs(o32.read_port_dft(p)[1] - o.read_port_dft(p)[1]).max() for p in range(2)) / imax
     S32 = _sstar(o32, 2, osp)
     print(f"C1 40k steps, yardstick: fp32 oracle vs fp64 oracle raw dft (V, I) = ({y_v:.3e}, {y_i:.3e}), dS = {np.abs(S32 - So).max():.3e}")
-    assert rep["dft_err"][0] <= 4 * y_v + 1e-6 and rep["dft_err"][1] <= 4 * y_i + 1e-6
+    assert rep["dft_err"][0] <= 2 * y_v + 1e-6 and rep["dft_err"][1] <= 2 * y_i + 1e-6
 
 
 @pytest.mark.parametrize("impl", [0, 2])
 def test_C2_full_grid_first_steps(impl):
-    w = W.interconnect_c2(run="tot", steps=300)
+    """SURVEY 8(d) rung (i): the full grid, first 500 steps, fields at {100, 250, 500} and the raw port DFTs."""
+    w = W.interconnect_c2(run="tot", steps=500)
     assert (w["nx"], w["ny"], w["nz"]) == (512, 256, 128)
-    o, s, rep = run_pair(w, 300, options={FDTD_OPT_STEP_IMPL: impl}, checkpoints=[100, 300])
-    print(f"C2 full grid impl={s.impl_name} kz={s.fused_kz}: field_err={rep['field_err'].max():.3e} dft={rep['dft_err']}")
+    o, s, rep = run_pair(w, 500, options={FDTD_OPT_STEP_IMPL: impl}, checkpoints=[100, 250, 500])
+    print(f"C2 full grid 500 steps impl={s.impl_name} kz={s.fused_kz}: field_err={rep['field_err'].max():.3e} dft={rep['dft_err']}")
     assert_fields(rep, FDTD_F32)
-    assert max(rep["dft_err"]) <= 1e-4      # 300 steps: far below the drift regime of R14
+    assert max(rep["dft_err"]) <= 1e-4      # 500 steps: far below the drift regime of R14
     s.destroy()
 
 
-@pytest.mark.parametrize("impl", [0, 2])
-def test_C4_full_grid_first_steps(impl):
-    """impl 0: what fdtd_commit selects at this size (the fused step or two steps per pass, by measurement); 2: the fused step."""
-    w = W.interconnect_c4(run="tot", steps=40)
+_SLOW = os.environ.get("FDTD_SLOW") == "1"
+
+
+@pytest.mark.parametrize("impl,steps", [(0, 40), (2, 40)] + ([(0, 500)] if _SLOW else []))
+def test_C4_full_grid_first_steps(impl, steps):
+    """impl 0: what fdtd_commit selects at this size (the fused step or two steps per pass, by measurement); 2: the fused step.
+    40 steps in the default run; rung (i)'s full 500 steps (fields at {100, 250, 500}; about two minutes of fp64 oracle on 134 M
+    cells) with FDTD_SLOW=1 -- run once per round through gpurun, its line is kept in profiles/r03_ladder.md."""
+    w = W.interconnect_c4(run="tot", steps=steps)
     assert (w["nx"], w["ny"], w["nz"]) == (1024, 512, 256) and w["precision"] == FDTD_F64
-    o, s, rep = run_pair(w, 40, options={FDTD_OPT_STEP_IMPL: impl}, checkpoints=[10, 40])
-    print(f"C4 full grid impl={s.impl_name} kz={s.fused_kz}: field_err={rep['field_err'].max():.3e} dft={rep['dft_err']}")
+    cps = [10, 40] if steps == 40 else [100, 250, 500]
+    o, s, rep = run_pair(w, steps, options={FDTD_OPT_STEP_IMPL: impl}, checkpoints=cps)
+    print(f"C4 full grid {steps} steps impl={s.impl_name} kz={s.fused_kz}: field_err={rep['field_err'].max():.3e} dft={rep['dft_err']}")
     assert s.impl_name in (("fused", "two_step") if impl == 0 else ("fused",))
     assert_fields(rep, FDTD_F64)
     assert max(rep["dft_err"]) <= 1e-11
@@ -154,7 +161,9 @@ def test_C2_quarter_scale_full_200k_steps_sparams():
     than a small multiple of what fp32 time stepping itself loses.  S* -- a ratio of DFTs of the same run, Eq. 1 -- is
     graded at the full 200 000 steps against north_star's 1e-3."""
     cps = [500, 2000, 20000, 60000, 120000, 200000]
-    opts = {"auto": None, "fused": {FDTD_OPT_STEP_IMPL: 2}}
+    opts = {"auto": None}
+    if _SLOW:     # the fused step by name as well (the same 200 000 steps again: FDTD_SLOW=1 only; r02_ladder.md has its numbers)
+        opts["fused"] = {FDTD_OPT_STEP_IMPL: 2}
     sims = {}
     for run in ("inc", "tot"):
         w = W.interconnect_c2(run=run, div=4)
@@ -176,7 +185,7 @@ def test_C2_quarter_scale_full_200k_steps_sparams():
                 line += f" {name} ({g.impl_name}) dE {ge:.2e} dH {gh:.2e};"
                 if cp <= 500:
                     assert max(ge, gh) <= TOL[FDTD_F32], (name, cp, ge, gh)
-                assert ge <= 5 * ye + TOL[FDTD_F32] and gh <= 5 * yh + TOL[FDTD_F32], (name, cp, ge, gh, ye, yh)
+                assert ge <= 2 * ye + TOL[FDTD_F32] and gh <= 2 * yh + TOL[FDTD_F32], (name, cp, ge, gh, ye, yh)
             print(line)
         sims[run] = (o, gpus, o32)
     So = _s_column(sims["inc"][0], sims["tot"][0], 2, osp)
