@@ -298,6 +298,103 @@ def job_throughput(n_cells, steps, world, seconds):
 
 
 # --------------------------------------------------------------------------------------------------------------------
+# the other configurations of BASELINE.json (and the paper's production grid shape) as short legs of the default run
+# --------------------------------------------------------------------------------------------------------------------
+OTHER_LEGS = (("c4", 150, 5), ("c2", 2000, 20), ("x3", 2000, 20), ("c1", 20000, 200), ("c0", 20000, 200))
+
+
+def other_leg(name, K, Wm, dev, local_rank):
+    """One short device-resident leg (W warm-up steps, K timed steps, CUDA events on the solver's stream, clocks sampled) of
+    another workload: what fdtd_commit selects for it, its step time, and its own roofline object.  Grids that live in L2 (C0,
+    C1) are launch- / barrier-bound, not bandwidth-bound: they report steps per second instead of a fraction."""
+    import torch
+
+    from paper_2208_04371_b200 import Solver
+    t0 = time.perf_counter()
+    w = workload(name, K)
+    gen_s = time.perf_counter() - t0
+    n_cells = w["nx"] * w["ny"] * w["nz"]
+    s = Solver.from_workload(w, device=str(dev))
+    s.step(Wm)
+    torch.cuda.synchronize(dev)
+    ck = ClockSampler(local_rank)
+    ck.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = s.launch_count
+    e0.record(s.stream)
+    s.step(K)
+    e1.record(s.stream)
+    torch.cuda.synchronize(dev)
+    clocks = ck.stop()
+    t_s = e0.elapsed_time(e1) * 1e-3
+    es = 4 if w["precision"] == 32 else 8
+    leg = {"grid": [w["nx"], w["ny"], w["nz"]], "dtype": "f32" if es == 4 else "f64", "materials": w["materials"]["mode"],
+           "steps": K, "warmup": Wm, "ms_per_step": t_s / K * 1e3, "value": n_cells * K / t_s / 1e6, "unit": UNIT,
+           "step_impl": s.impl_name, "fused_kz": s.fused_kz, "fused_tile": s.fused_tile, "commit_s": s.commit_s,
+           "generator_s": gen_s, "gpu_launches": s.launch_count - l0, "clocks": clocks}
+    if s.impl_name == "persistent" or n_cells * 12 * es <= 100e6:
+        leg["roofline"] = {"bound": "launch/barrier", "note": "grid and coefficients live in L2 (126 MB): no HBM roofline applies",
+                           "steps_per_s": K / t_s, "us_per_step": t_s / K * 1e6}
+    else:
+        leg["roofline"], _ = kernel_roofline(s, w, K, t_s, name)
+    s.destroy()
+    del s
+    torch.cuda.empty_cache()
+    return leg
+
+
+def kernel_roofline(s, w, K, t_s, workload_name):
+    """The roofline object of one handle: per-kernel durations from fdtd_profile_step (CUDA events between the kernels, on the
+    solver's stream), algorithmic bytes of the dominant kernel from the per-cell figures of DESIGN.md, the measured copy peak.
+    Returns (roofline, bytes one step must move under the scheme in use)."""
+    n_cells = w["nx"] * w["ny"] * w["nz"]
+    ms = s.profile_step(max(3, min(20, K)))
+    impl = s.impl_name
+    es = 4 if w["precision"] == 32 else 8
+    peak, peak_src = measured_peak()
+    extra = {}
+    if impl == "two_step":
+        # the dominant kernel advances its box TWO steps per launch: every field of the box read once and written once (+1 B
+        # index) per two cell-updates; profile_step's figures are per STEP, a launch lasts two of them.  The shell around the
+        # box (CPML layers, port planes) is advanced step by step by the two-pass kernels on region grids (ms[1]).
+        b = s.two_step_box
+        box_cells = (b[1] - b[0]) * (b[3] - b[2]) * (b[5] - b[4])
+        full = w["materials"]["mode"] == "full"
+        kname, kms = "k_step2", 2.0 * ms[0]
+        ab = box_cells * (12 * es + (6 * es if full else 1))
+        shell_cells = n_cells - box_cells
+        # what one STEP must move under this scheme: half a box pass + the shell's two-pass traffic (73 B fp32 indexed + psi)
+        step_bytes = ab / 2 + (algorithmic_bytes(w, "two_pass", "H") + algorithmic_bytes(w, "two_pass", "E")) * shell_cells / n_cells
+        one_step_model = algorithmic_bytes(w, "fused", "H")      # the 49 B + psi model of the one-step fused kernel, for comparison
+        extra = {"box": b, "box_cells": box_cells, "shell_cells": shell_cells, "shell_ms_per_step": ms[1],
+                 "bytes_per_cell_update_box": ab / 2 / box_cells,
+                 "one_step_byte_model": {"bytes_per_cell_update": one_step_model / n_cells,
+                                         "equivalent_gbs": one_step_model * K / t_s / 1e9,
+                                         "equivalent_frac": one_step_model * K / t_s / 1e9 / peak,
+                                         "note": "throughput expressed in the one-step fused kernel's byte model (49 B + psi per "
+                                                 "cell-update): may exceed 1 because two steps per pass move fewer bytes"}}
+    elif impl == "fused":
+        kname, kms = "k_step_fused", ms[0]
+        ab = algorithmic_bytes(w, impl, "H")
+        step_bytes = ab
+    else:
+        kname, kms = ("k_update_E", ms[1]) if ms[1] >= ms[0] else ("k_update_H", ms[0])
+        ab = algorithmic_bytes(w, impl, "E" if kname == "k_update_E" else "H")
+        step_bytes = algorithmic_bytes(w, impl, "H") + algorithmic_bytes(w, impl, "E")
+    achieved = ab / (kms * 1e-3) / 1e9
+    # DRAM bytes of one launch from the committed `ncu --set full` capture of this workload and kernel (profiles/), else null
+    traffic, traffic_src = ncu_traffic(workload_name, kname, "f32" if w["precision"] == 32 else "f64", s.fused_kz)
+    roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": ab, "kernel_ms": kms,
+                "kernel_ms_all": {"H_or_fused_or_box": ms[0], "E_or_shell": ms[1], "source": ms[2], "probe_dft": ms[3]},
+                "bytes_per_cell_update_step": step_bytes / n_cells,
+                "step_achieved_gbs": step_bytes * K / t_s / 1e9, "frac_of_8000": step_bytes * K / t_s / 1e9 / 8000.0}
+    roofline.update(extra)
+    return roofline, step_bytes
+
+
+# --------------------------------------------------------------------------------------------------------------------
 # our arm
 # --------------------------------------------------------------------------------------------------------------------
 def run_ours(args, rank, world, local_rank):
@@ -348,49 +445,9 @@ def run_ours(args, rank, world, local_rank):
     value = job_throughput(n_cells, K, world, t_s)
 
     # ---- per-kernel durations (CUDA events between the kernels, on the solver's stream) ------------------------------
-    ms = s.profile_step(max(3, min(20, K)))
     impl = s.impl_name
-    es = 4 if w["precision"] == 32 else 8
     peak, peak_src = measured_peak()
-    extra = {}
-    if impl == "two_step":
-        # the dominant kernel advances its box TWO steps per launch: every field of the box read once and written once (+1 B
-        # index) per two cell-updates; profile_step's figures are per STEP, a launch lasts two of them.  The shell around the
-        # box (CPML layers, port planes) is advanced step by step by the two-pass kernels on region grids (ms[1]).
-        b = s.two_step_box
-        box_cells = (b[1] - b[0]) * (b[3] - b[2]) * (b[5] - b[4])
-        full = w["materials"]["mode"] == "full"
-        kname, kms = "k_step2", 2.0 * ms[0]
-        ab = box_cells * (12 * es + (6 * es if full else 1))
-        shell_cells = n_cells - box_cells
-        # what one STEP must move under this scheme: half a box pass + the shell's two-pass traffic (73 B fp32 indexed + psi)
-        step_bytes = ab / 2 + (algorithmic_bytes(w, "two_pass", "H") + algorithmic_bytes(w, "two_pass", "E")) * shell_cells / n_cells
-        one_step_model = algorithmic_bytes(w, "fused", "H")      # the 49 B + psi model of the one-step fused kernel, for comparison
-        extra = {"box": b, "box_cells": box_cells, "shell_cells": shell_cells, "shell_ms_per_step": ms[1],
-                 "bytes_per_cell_update_box": ab / 2 / box_cells,
-                 "one_step_byte_model": {"bytes_per_cell_update": one_step_model / n_cells,
-                                         "equivalent_gbs": one_step_model * K / t_s / 1e9,
-                                         "equivalent_frac": one_step_model * K / t_s / 1e9 / peak,
-                                         "note": "throughput expressed in the one-step fused kernel's byte model (49 B + psi per "
-                                                 "cell-update): may exceed 1 because two steps per pass move fewer bytes"}}
-    elif impl == "fused":
-        kname, kms = "k_step_fused", ms[0]
-        ab = algorithmic_bytes(w, impl, "H")
-        step_bytes = ab
-    else:
-        kname, kms = ("k_update_E", ms[1]) if ms[1] >= ms[0] else ("k_update_H", ms[0])
-        ab = algorithmic_bytes(w, impl, "E" if kname == "k_update_E" else "H")
-        step_bytes = algorithmic_bytes(w, impl, "H") + algorithmic_bytes(w, impl, "E")
-    achieved = ab / (kms * 1e-3) / 1e9
-    # DRAM bytes of one launch from the committed `ncu --set full` capture of this workload and kernel (profiles/), else null
-    traffic, traffic_src = ncu_traffic(args.workload, kname, "f32" if w["precision"] == 32 else "f64", s.fused_kz)
-    roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": ab, "kernel_ms": kms,
-                "kernel_ms_all": {"H_or_fused_or_box": ms[0], "E_or_shell": ms[1], "source": ms[2], "probe_dft": ms[3]},
-                "bytes_per_cell_update_step": step_bytes / n_cells,
-                "step_achieved_gbs": step_bytes * K / t_s / 1e9, "frac_of_8000": step_bytes * K / t_s / 1e9 / 8000.0}
-    roofline.update(extra)
+    roofline, step_bytes = kernel_roofline(s, w, K, t_s, args.workload)
 
     # ---- sustained: BASELINE.json's "2000 steps timed" on C3, own clock samples ---------------------------------------
     sustained = None
@@ -435,7 +492,7 @@ def run_ours(args, rank, world, local_rank):
             "dtype": "f32" if w["precision"] == 32 else "f64", "data": "synthetic",
             "config": {"workload": args.workload, "grid": [w["nx"], w["ny"], w["nz"]], "cells": n_cells,
                        "materials": m["mode"], "cpml_cells": w["pml"], "ports": len(w["ports"]), "dft_freqs": len(w["freqs"]),
-                       "step_impl": impl, "fused_kz": s.fused_kz, "fused_tile": s.fused_tile, "l2": "inputs larger than L2 (no flush needed)" if n_cells * 24 > 2.6e8 else
+                       "step_impl": impl, "commit_s": s.commit_s, "fused_kz": s.fused_kz, "fused_tile": s.fused_tile, "l2": "inputs larger than L2 (no flush needed)" if n_cells * 24 > 2.6e8 else
                        "grid fits in L2: launch-bound case, not a roofline case",
                        "parallelism": "replicas only" if world > 1 else "1 GPU", "library": os.path.basename(binding.library_path())},
             "clocks": ck, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "sustained": sustained}
@@ -466,6 +523,8 @@ def run_ours(args, rank, world, local_rank):
         s1.destroy()
         del s1
         torch.cuda.empty_cache()
+    if rank == 0 and world == 1 and args.workload == "c3" and not args.no_others:
+        line["others"] = {name: other_leg(name, k, wm, dev, local_rank) for name, k, wm in OTHER_LEGS}
     if rank == 0 and world == 1 and not args.no_cpu:
         r = oracle_sample(budget_s=args.cpu_budget, one_thread=True)
         line["cpu_baseline"] = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"],
@@ -593,6 +652,7 @@ def main():
     ap.add_argument("--fused-tile", type=int, default=0, help="FDTD_OPT_FUSED_TILE: 0 measured at commit, 1 = 14-row tiles, 2 = 6-row tiles")
     ap.add_argument("--no-fused-leg", action="store_true", help="c3, two steps per pass selected: skip the one-step fused kernel's leg")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-others", action="store_true", help="c3: skip the short legs of the other configurations (c4, c2, x3, c1, c0)")
     ap.add_argument("--cpu-budget", type=float, default=15.0)
     ap.add_argument("--sustained-steps", type=int, default=2000,
                     help="steps of the sustained leg on c3 (BASELINE.json: '2000 steps timed'); 0 = off")

@@ -74,9 +74,20 @@ enum {
   FDTD_OPT_FUSED_KZ = 4,    /* planes per z chunk of the fused kernel (0 = auto: measured at commit)                    */
   FDTD_OPT_Z_SPIN = 5,      /* linked z slabs: polls of a hand-over counter before a wait gives up (default 2e7; a poll sleeps
                                about 1 us, so about 20 s).  After the first time-out the slab's later waits return at once    */
-  FDTD_OPT_FUSED_TILE = 6   /* tile of the fused kernel: 0 = auto (measured at commit), 1 = 128 x 14 cells (fp64: 64 x 14), one
+  FDTD_OPT_FUSED_TILE = 6,  /* tile of the fused kernel: 0 = auto (measured at commit), 1 = 128 x 14 cells (fp64: 64 x 14), one
                                block per SM; 2 = 128 x 6 (64 x 6), two blocks per SM: twice the tiles and two z marches per
                                SM for mid-size grids.  The results are the same cell by cell whatever the tile            */
+  FDTD_OPT_TUNE_MEMO = 7    /* 1 (default) = what fdtd_commit measured for a configuration (device, precision, grid, material
+                               mode, CPML thicknesses, STEP_IMPL / FUSED_KZ / FUSED_TILE, z interfaces, port / source /
+                               frequency counts) is remembered for the life of the process and taken again, unmeasured, by
+                               every later commit of the same configuration: one program always runs one implementation.
+                               0 = measure afresh.  Reproducibility: results are bit-identical for a given implementation,
+                               tile and chunk length (fdtd_impl_name, fdtd_fused_kz, fdtd_fused_tile report them); between
+                               implementations they agree to the parity tolerance only (different fma / summation order), and
+                               with two steps per pass (4, or 0 where it is selected) an odd fdtd_step(n) runs its last step
+                               with the one-step kernels -- so how a caller batches its steps is part of that configuration.
+                               Across processes the automatic choice may differ: pin it with FDTD_OPT_STEP_IMPL / FUSED_KZ /
+                               FUSED_TILE from a reported run where bitwise repeatability matters                             */
 };
 
 /* A port (Fig. 1a): a soft E_z source on a box of the plane i = is (surface 'e'), a voltage box and

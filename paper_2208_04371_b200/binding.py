@@ -19,6 +19,7 @@ FDTD_W_DGAUSS, FDTD_W_GAUSS, FDTD_W_GSINE = 0, 1, 2
 FDTD_MAT_INDEXED, FDTD_MAT_FULL = 0, 1
 FDTD_EX, FDTD_EY, FDTD_EZ, FDTD_HX, FDTD_HY, FDTD_HZ = range(6)
 FDTD_OPT_STEP_IMPL, FDTD_OPT_USE_GRAPH, FDTD_OPT_GRAPH_UNROLL, FDTD_OPT_FUSED_KZ, FDTD_OPT_Z_SPIN, FDTD_OPT_FUSED_TILE = 1, 2, 3, 4, 5, 6
+FDTD_OPT_TUNE_MEMO = 7
 
 _ERRNAMES = {-1: "FDTD_EINVAL", -2: "FDTD_ECFL", -3: "FDTD_ESTATE", -4: "FDTD_ENOMEM", -5: "FDTD_ECUDA", -6: "FDTD_ERANGE"}
 

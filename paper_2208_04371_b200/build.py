@@ -30,11 +30,6 @@ def up_to_date():
 
 
 def build(force=False, verbose=False):
-    override = os.environ.get("FDTD_B200_LIB")   # a pre-built variant of the library (tuning builds: nvcc -D...), used as it is
-    if override:
-        if not os.path.exists(override):
-            raise RuntimeError(f"FDTD_B200_LIB={override} does not exist")
-        return override
     if not force and up_to_date():
         return LIB
     nvcc = os.environ.get("NVCC", "nvcc")

@@ -14,6 +14,8 @@
 #include <limits>
 #include <new>
 #include <string>
+#include <map>
+#include <mutex>
 #include <vector>
 
 #include <cuda.h>
@@ -54,7 +56,7 @@ struct fdtd {
   int has_mu = 0;
   std::vector<PortDev> ports;
   std::vector<double> freqs;
-  long opt_impl = 0, opt_graph = 1, opt_unroll = 8, opt_kz = 0, opt_tile = 0;
+  long opt_impl = 0, opt_graph = 1, opt_unroll = 8, opt_kz = 0, opt_tile = 0, opt_tune_memo = 1;
   int z_lo_open = 0, z_hi_open = 0;   // this grid is a z slab of a larger one (fdtd_set_z_interfaces)
   bool z_linked[2] = {false, false};  // fdtd_z_link: the kernels push my boundary planes into the neighbour on that side
   long opt_zspin = 20000000;          // polls of a hand-over flag before the wait kernel gives up (>= 1 us each: about 20 s)
@@ -120,6 +122,20 @@ struct fdtd {
   virtual const int* two_step_box() const = 0;
   virtual int fused_tile() const = 0;
 };
+
+// Commit-time measurements remembered for the life of the process.  fdtd_commit chooses between step implementations, tile
+// shapes and chunk lengths by timing them; two measurements of near-equal candidates can come out either way, and the
+// implementations differ in rounding order (to tolerance, not bitwise).  So the FIRST verdict for a configuration -- device,
+// precision, grid, material mode, CPML thicknesses, the options that steer the choice, port / source counts -- is kept and every
+// later commit of the same configuration in this process takes it without measuring again: the same program gives the same
+// fields however often it builds the solver (and later commits are faster).  FDTD_OPT_TUNE_MEMO = 0 measures afresh.
+struct TuneMemo {
+  bool have_fused = false, fused = false; int kz = 0, shape = 0; double ms = -1.0;     // autotune()
+  bool have_two = false, two = false; int kz2 = 0; double ms2 = -1.0;                  // autotune_two_step()
+  bool have_pers = false, pers = false;                                               // setup_persistent()
+};
+static std::mutex g_tune_lock;
+static std::map<std::string, TuneMemo> g_tune;
 
 namespace {
 
@@ -288,6 +304,27 @@ struct Solver : fdtd {
   }
   int autotune();
   int autotune_two_step();
+  std::string tune_key() const {
+    int nsrc = 0;
+    for (const PortDev& d : ports) nsrc += d.has_source ? 1 : 0;
+    char b[384];
+    snprintf(b, sizeof b, "%d|%zu|%d,%d,%d|%d,%d|%d,%d,%d,%d,%d,%d|%ld,%ld,%ld|%d,%d|%zu,%d,%zu", device, sizeof(T), nx, ny, nz, mat_mode,
+             has_mu, npml[0], npml[1], npml[2], npml[3], npml[4], npml[5], opt_impl, opt_kz, opt_tile, z_lo_open, z_hi_open,
+             ports.size(), nsrc, freqs.size());
+    return b;
+  }
+  bool memo_get(TuneMemo* m) const {
+    if (!opt_tune_memo) return false;
+    std::lock_guard<std::mutex> hold(g_tune_lock);
+    auto it = g_tune.find(tune_key());
+    if (it == g_tune.end()) return false;
+    *m = it->second;
+    return true;
+  }
+  template <typename F> void memo_put(F&& fill) const {
+    std::lock_guard<std::mutex> hold(g_tune_lock);
+    fill(g_tune[tune_key()]);
+  }
   double tuned_ms = -1.0;    // device time per step of the choice autotune() made
   int autotune_kz_only() { const long keep = opt_impl; opt_impl = 2; const int r = autotune(); opt_impl = keep; return r; }
   int setup_persistent();
@@ -625,13 +662,9 @@ static PFN_cuTensorMapEncodeTiled_v12000 tensor_map_encoder() {
   return fn;
 }
 
-// tile rows and TMA stages of the fused kernel (compile-time; -DFDTD_FUSED_TY / -DFDTD_FUSED_NS for tuning builds)
-#ifndef FDTD_FUSED_TY
+// tile rows and TMA stages of the fused kernel (compile-time; the sweep that chose them: profiles/r01_final.md)
 #define FDTD_FUSED_TY 14
-#endif
-#ifndef FDTD_FUSED_NS
 #define FDTD_FUSED_NS 3
-#endif
 // two tile shapes: 0 = FDTD_FUSED_TY rows, one block per SM (large grids: the longest rows-per-halo ratio); 1 = 6 rows, two
 // blocks per SM (mid-size grids: twice the tiles, two z marches per SM).  fdtd_commit measures both (autotune()).
 constexpr int kFusedTileShapes = 2;
@@ -760,6 +793,18 @@ double Solver<T>::time_field_kernels(int reps) {
 //   FDTD_OPT_STEP_IMPL 2 with FDTD_OPT_FUSED_KZ 0: the kz candidates compete.
 template <typename T>
 int Solver<T>::autotune() {
+  TuneMemo memo;
+  if (memo_get(&memo) && memo.have_fused) {      // this configuration was measured earlier in this process: same verdict
+    fused = memo.fused; kz = memo.kz; tuned_ms = memo.ms;
+    if (tile_shape != memo.shape) {
+      tile_shape = memo.shape;
+      const int r = build_fused();
+      if (r != FDTD_OK) return r;
+    }
+    fpar[0].kz = fpar[1].kz = kz;
+    cur = 0;
+    return FDTD_OK;
+  }
   const int reps = (long long)nx * ny * nz >= (64LL << 20) ? 2 : 4;
   double best = -1.0;
   int best_kz = kz, best_shape = tile_shape;
@@ -822,6 +867,7 @@ int Solver<T>::autotune() {
   cudaError_t e = cudaMemsetAsync(sp.nstep, 0, sizeof(long long), stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
   if (e != cudaSuccess) return cuda_fail(e, "fdtd_commit: autotune");
+  memo_put([&](TuneMemo& m) { m.have_fused = true; m.fused = fused; m.kz = kz; m.shape = tile_shape; m.ms = tuned_ms; });
   return FDTD_OK;
 }
 
@@ -833,10 +879,27 @@ template <typename T>
 int Solver<T>::autotune_two_step() {
   const bool asked = two_step;
   const int kz_before = kz;
+  TuneMemo memo;
+  if (memo_get(&memo) && memo.have_two) {
+    if (!memo.two) return FDTD_OK;               // measured before: the two-step kernel lost (or the grid leaves no box)
+    if (!asked) {
+      kz = memo.kz2;
+      const int r = build_step2();
+      if (r != FDTD_OK) return r;
+    }
+    two_step = true; fused = false; kz = memo.kz2; tuned_ms = memo.ms2;
+    s2par[0].kz = s2par[1].kz = kz;
+    cur = 0;
+    return FDTD_OK;
+  }
   if (!asked) {
     const std::string keep_err = err;
     kz = 24;
-    if (build_step2() != FDTD_OK) { err = keep_err; kz = kz_before; return FDTD_OK; }
+    if (build_step2() != FDTD_OK) {
+      err = keep_err; kz = kz_before;
+      memo_put([&](TuneMemo& m) { m.have_two = true; m.two = false; });
+      return FDTD_OK;
+    }
   }
   std::vector<PortDev> no_ports;
   no_ports.swap(ports);
@@ -878,6 +941,7 @@ int Solver<T>::autotune_two_step() {
     kz = kz_before;
   }
   s2par[0].kz = s2par[1].kz = two_step ? kz : s2par[0].kz;
+  memo_put([&](TuneMemo& m) { m.have_two = true; m.two = two_step; m.kz2 = kz; m.ms2 = tuned_ms; });
   return FDTD_OK;
 }
 
@@ -947,6 +1011,10 @@ int Solver<T>::setup_persistent() {
   // one more resident block per port for the probes and their DFT terms, where the device has room for them
   persist_probe = (!ports.empty() && persist_blocks + (long long)ports.size() <= cap) ? (int)ports.size() : 0;
   if (opt_impl == 3) { persistent = true; return FDTD_OK; }
+  {
+    TuneMemo memo;
+    if (memo_get(&memo) && memo.have_pers) { persistent = memo.pers; return FDTD_OK; }
+  }
   // measure: 16 steps either way
   const int reps = 16;
   PortParams<T> none = pp;
@@ -979,16 +1047,13 @@ int Solver<T>::setup_persistent() {
   if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
   if (e != cudaSuccess || msp < 0.f) return cuda_fail(e, "fdtd_commit: timing the persistent step kernel");
   persistent = msp < ms2;
+  memo_put([&](TuneMemo& m) { m.have_pers = true; m.pers = persistent; });
   return FDTD_OK;
 }
 
 // ---- two steps per pass (fdtd_step2.cuh): the box, its tensor maps, the shell passes ----------------------------------------
-#ifndef FDTD_STEP2_R
-#define FDTD_STEP2_R 11
-#endif
-#ifndef FDTD_STEP2_NS
+#define FDTD_STEP2_R 11     // computed rows per tile and TMA stages of the two-step kernel (profiles/r02_c3_two_step.md)
 #define FDTD_STEP2_NS 4
-#endif
 static_assert(Step2Cfg<float, FDTD_STEP2_R, FDTD_STEP2_NS>::SMEM <= 232448 && Step2Cfg<double, FDTD_STEP2_R, FDTD_STEP2_NS>::SMEM <= 232448,
               "two-step kernel: rows x stages exceed the 227 KB shared memory of an sm_100 CTA");
 template <typename T, int MODE>
@@ -1668,6 +1733,7 @@ int fdtd_set_option(fdtd_t* h, int option, long value) {
     case FDTD_OPT_GRAPH_UNROLL: if (value < 1 || value > 1024) break; h->opt_unroll = value; return FDTD_OK;
     case FDTD_OPT_FUSED_KZ: if (value < 0 || value > 65535) break; h->opt_kz = value; return FDTD_OK;
     case FDTD_OPT_Z_SPIN: if (value < 1) break; h->opt_zspin = value; return FDTD_OK;
+    case FDTD_OPT_TUNE_MEMO: if (value < 0 || value > 1) break; h->opt_tune_memo = value; return FDTD_OK;
     case FDTD_OPT_FUSED_TILE: if (value < 0 || value > kFusedTileShapes) break; h->opt_tile = value; return FDTD_OK;
   }
   return h->fail(FDTD_EINVAL, "fdtd_set_option: unknown option %d or bad value %ld", option, value);

@@ -281,6 +281,19 @@ class DistributedSlab:
             self.solver.step_end()
             self._exchange(False, (EX, EY))
 
+    def step_lockstep(self, n=1):
+        """n steps with a host barrier after every half step -- for ranks that SHARE one GPU (time-sliced processes: a kernel
+        of one process must never spin on a counter that only a kernel of another process can post, the GPU may not be running
+        that process).  The hand-over itself is unchanged: the kernels store the planes into the neighbour's halo (CUDA-IPC
+        mapped memory) and post its counter; the barriers only make sure every wait finds its counter already posted."""
+        for _ in range(n):
+            self.solver.step_begin()
+            self.solver.synchronize()
+            self.dist.barrier()
+            self.solver.step_end()
+            self.solver.synchronize()
+            self.dist.barrier()
+
     def upload_materials(self, w, pinned=False):
         import torch
         m = w["materials"]

@@ -8,6 +8,8 @@ Fields come back as torch CUDA tensors shaped [nz, ny, nx] (x fastest).
 """
 from __future__ import annotations
 
+import time
+
 import numpy as np
 
 from . import binding as B
@@ -67,7 +69,9 @@ class Solver:
             self.workspace = torch.empty(self.workspace_bytes(), dtype=torch.uint8, device=self.device)
             self.stream = stream if stream is not None else torch.cuda.Stream(self.device)
             self.stream.wait_stream(torch.cuda.current_stream(self.device))   # the allocator may still be clearing the block
+            t0 = time.perf_counter()
             B.fdtd_commit(self.h, self.workspace, self.stream.cuda_stream)
+            self.commit_s = time.perf_counter() - t0      # wall time of fdtd_commit (tables, clears, commit-time measurements)
 
     # ---- ordering against torch's current stream for tensors that cross the boundary -------------------------------
     def _before_read_of(self, *tensors):

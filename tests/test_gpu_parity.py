@@ -495,3 +495,27 @@ def test_five_driving_ports_two_step_by_name_is_refused_and_the_automatic_choice
     assert_fields(rep, FDTD_F32)
     assert max(rep["dft_err"]) <= 1e-4
     s.destroy()
+
+
+@pytest.mark.parametrize("name", ["c2", "c1"])
+def test_commit_choice_is_remembered_within_a_process(name):
+    """fdtd_commit measures its candidates (step implementation, tile, chunk length); near-equal candidates could come out either
+    way and differ in rounding order.  The first verdict for a configuration is kept for the life of the process
+    (FDTD_OPT_TUNE_MEMO, default on): every later commit of the same workload runs the same implementation -- and gives the same
+    bits -- without measuring again."""
+    w = W.interconnect_c2(run="tot", steps=6) if name == "c2" else W.microstrip_c1(steps=6)
+    first = Solver.from_workload(w)
+    choice, t_first = (first.impl_name, first.fused_kz, first.fused_tile), first.commit_s
+    first.step(6)
+    ref = [first.read_fields(c).clone() for c in range(6)]
+    first.destroy()
+    for _ in range(3):
+        s = Solver.from_workload(w)
+        assert (s.impl_name, s.fused_kz, s.fused_tile) == choice
+        t_again = s.commit_s
+        s.step(6)
+        for c in range(6):
+            assert bool((s.read_fields(c) == ref[c]).all())
+        s.destroy()
+    print(f"{name}: choice {choice}, fdtd_commit {t_first * 1e3:.1f} ms measured, {t_again * 1e3:.1f} ms remembered")
+    assert t_again < t_first

@@ -221,3 +221,27 @@ def test_a_wait_that_times_out_is_reported_and_later_waits_return_at_once():
     s.step(1)                                        # step 1 waits for "0 steps delivered": satisfied
     s.read_fields(0)
     s.destroy()
+
+
+@pytest.mark.parametrize("prec", [32, 64])
+def test_two_processes_on_one_gpu_exchange_over_cuda_ipc(prec):
+    """The cross-process path of f4 on the hardware that exists here: two torch.distributed ranks, both on cuda:0, one z slab
+    each, linked through CUDA IPC (DistributedSlab(transport="peer")): the kernels of one process store their boundary planes
+    into the other process's halo and post its arrival counter.  Lockstep under host barriers (time-sliced processes); each
+    rank checks its slab against the fp64 oracle on the undivided grid, then resets and reruns bit-identically.
+    tests/ipc_two_ranks.py is the rank program.  (Two GPUs, concurrent kernels over NVLink: not available on this pool.)"""
+    import os
+    import socket
+    import subprocess
+    import sys
+    with socket.socket() as so:
+        so.bind(("127.0.0.1", 0))
+        port = so.getsockname()[1]
+    here = os.path.dirname(os.path.abspath(__file__))
+    r = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2", "--master-addr", "127.0.0.1",
+                        "--master-port", str(port), os.path.join(here, "ipc_two_ranks.py"), str(prec), "60"],
+                       capture_output=True, text=True, timeout=600)
+    line = [l for l in r.stdout.splitlines() if l.startswith("IPC2 ")]
+    print(line[0] if line else r.stdout[-2000:] + r.stderr[-4000:])
+    assert r.returncode == 0, r.stderr[-4000:]
+    assert line and "rerun_identical=True" in line[0]
