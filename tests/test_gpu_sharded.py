@@ -245,3 +245,30 @@ def test_two_processes_on_one_gpu_exchange_over_cuda_ipc(prec):
     print(line[0] if line else r.stdout[-2000:] + r.stderr[-4000:])
     assert r.returncode == 0, r.stderr[-4000:]
     assert line and "rerun_identical=True" in line[0]
+
+
+def test_slabs_on_two_gpus_match_the_oracle():
+    """The path no box of this pool can run (one GPU each): one slab per GPU in one process -- peer access enabled by
+    fdtd_z_link, the slabs' kernels running concurrently and waiting on each other's counters over NVLink, fdtd_step(n) with
+    graphs on both handles.  Skipped on one GPU; the first box with two runs it."""
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs")
+    w = W.interconnect_c2(run="tot", div=4, steps=600, npml=6, nf=16)
+    o = YeeOracle.from_workload(w, track_max=True)
+    sh = ShardedSolver(w, ["cuda:0", "cuda:1"])
+    assert sh.concurrent
+    o.step(600)
+    sh.step(600)
+    emax, hmax = o.running_max()
+    for c in range(6):
+        g = sh.read_fields(c).cpu().numpy().astype(np.float64)
+        assert np.abs(g - o.read_field(c)).max() <= 1e-4 * (emax if c < 3 else hmax)
+    sh.reset()
+    sh.step(600)
+    again = [sh.read_fields(c) for c in range(6)]
+    sh.reset()
+    sh.step(600)
+    for c in range(6):
+        assert bool((sh.read_fields(c) == again[c]).all())
+    sh.destroy()
