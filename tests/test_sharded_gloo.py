@@ -151,3 +151,53 @@ def test_three_ranks_link_to_the_facing_halo_of_each_neighbour_and_step_without_
     # a linked slab is advanced by fdtd_step(n) alone: no begin / end / host-issued exchange
     assert all(r[k]["stepped"] == [5] and r[k]["log"] == [] for k in range(3))
     assert all(r[k]["owner"] == {p: (1, p) for p in range(4)} for k in range(3))
+
+
+class _FakeResettable(_FakeLinkedSolver):
+    """Logs synchronize / reset into a list shared by the ranks; one rank is slow to drain."""
+    def __init__(self, ws, rank, z_open, events):
+        super().__init__(ws, rank, z_open)
+        self.events, self.drains = events, 0
+
+    def synchronize(self):
+        import time
+        if self.rank == 1 and self.drains == 0:
+            time.sleep(0.4)                                   # still finishing its last step while the others are ready to reset
+        self.drains += 1
+        self.events.append(("sync", self.rank))
+
+    def reset(self):
+        self.events.append(("reset", self.rank))
+
+
+def _worker_reset(rank, world, port, events):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    w = W.throughput_c3(div=8, steps=4, npml=6, nf=4)
+    d = S.DistributedSlab(w, "cpu", make_solver=lambda ws, o, dev, zo: _FakeResettable(ws, rank, zo, events), transport="peer")
+    d.step(3)
+    d.reset()
+    events.append(("done", rank))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_reset_of_linked_ranks_drains_everybody_before_the_first_clear_and_after_the_last():
+    """A neighbour's last kernels store into my halo planes and post my counters: no rank may clear before EVERY rank has
+    drained, and no rank may go on (and step) before EVERY rank's clear has landed (include/fdtd.h, fdtd_z_link)."""
+    world = 3
+    with mp.Manager() as m:
+        events = m.list()
+        mp.spawn(_worker_reset, args=(world, _free_port(), events), nprocs=world, join=True)
+        ev = list(events)
+    pos = {kind: [i for i, e in enumerate(ev) if e[0] == kind] for kind in ("sync", "reset", "done")}
+    assert len(pos["sync"]) == 2 * world and len(pos["reset"]) == world and len(pos["done"]) == world
+    first_syncs = sorted(pos["sync"])[:world]
+    assert {ev[i][1] for i in first_syncs} == set(range(world))          # everybody drained ...
+    assert max(first_syncs) < min(pos["reset"])                             # ... before the first clear
+    assert max(pos["reset"]) < min(pos["done"])                             # and nobody goes on before the last clear
+    for r in range(world):                                                  # each rank waits for its own clear to land
+        mine = [i for i in pos["sync"] if ev[i][1] == r]
+        own_reset = [i for i in pos["reset"] if ev[i][1] == r][0]
+        assert mine[0] < own_reset < mine[1]
