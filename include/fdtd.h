@@ -20,7 +20,9 @@
  *             which.  All other pointers are host pointers.  Nothing is retained after a call returns except the
  *             workspace given to fdtd_commit().
  *   Memory    the CALLER owns all device memory: one buffer of fdtd_workspace_bytes() bytes (256-byte aligned), and
- *             a CUDA stream.  The library never allocates device memory.
+ *             a CUDA stream.  The library never allocates device memory.  (The one piece of device memory that is the
+ *             library's own is the fixed FDTD_NOALLOC_SCRATCH_BYTES array inside its image that fdtd_port_probe_noalloc uses;
+ *             see the end of this file.)
  *   Errors    every int-returning call returns FDTD_OK (0) or a negative code; fdtd_last_error() gives a message.
  *             No exceptions, no abort, no printing.  There is NO CPU fallback: without a CUDA device
  *             fdtd_commit() fails with FDTD_ECUDA.
